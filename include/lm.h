@@ -1,0 +1,153 @@
+/*
+ * lm.h -- C ABI of the B200-native open-boundary RPY mobility solver ("liblm").
+ *
+ * The calls follow the solver interface of libMobility (arXiv 2510.02135; citations are
+ * PAPER.md:LINE of the paper text this repo was built from):
+ *
+ *   paper                                            here
+ *   -----------------------------------------------  ---------------------------------
+ *   NBody("open","open","open") + initialize(         lm_create
+ *     viscosity, hydrodynamicRadius, includeAngular)
+ *   setPositions                                      lm_set_positions
+ *   Mdot(forces, torques) -> (linear, angular)        lm_mdot, lm_mdot_batch
+ *   sqrtMdotW()           -> (linear, angular)        lm_sqrt_mdot_w
+ *   mf + dwf + drift (the sum the example forms)      lm_hydrodynamic_velocities PAPER.md:78 (eq. 9), 137-138
+ *   divM()                                            not exported: identically zero for open
+ *                                                     boundaries
+ *
+ * What is computed.  U = M.[F;T] with M the 6N x 6N grand mobility of eq. (7)
+ * whose blocks are the free-space Rotne-Prager-Yamakawa pair tensors, summed over
+ * all ordered pairs (i,j) INCLUDING j = i (self term = r -> 0 limit), with the overlap (r < 2a)
+ * regularisation; and y = M^{1/2} W by the Lanczos iteration.  The closed
+ * forms and every reading of the paper are listed in DESIGN.md.
+ *
+ * Conventions for every call
+ *   - Precision is fixed per handle (LM_F32 / LM_F64); all `void*` arrays hold that type.
+ *   - Arrays are interleaved xyz, length 3N: element 3*i+k is component k of particle i (the
+ *     (N,3) row-major arrays of PAPER.md:128-138).  Batches are [nrhs][3N], contiguous.
+ *   - Plain entry points take DEVICE pointers; the `_host` variants take HOST pointers and do
+ *     the host<->device copies themselves on the given stream ("the library will
+ *     automatically copy the data to the GPU").  Pinned host memory makes those copies async.
+ *   - The caller owns every buffer it passes; the library never frees or retains them beyond
+ *     the call (`_host` variants and Lanczos calls return only after the stream has drained).
+ *     The handle owns its packed position copy, staging and Lanczos workspace (freed by
+ *     lm_destroy).  Inputs and outputs must not alias.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  lm_set_positions,
+ *     lm_mdot and lm_mdot_batch are asynchronous on it.  lm_sqrt_mdot_w and
+ *     lm_hydrodynamic_velocities (with noise) synchronise the stream internally: the Lanczos
+ *     stopping test reads two scalars per iteration on the host.
+ *   - Return value: LM_OK (0) or a negative LM_E_* code; lm_last_error(h) gives the message of
+ *     the last failing call on that handle.  No exceptions, no global state, no CPU fallback:
+ *     without a CUDA device every compute call returns LM_E_CUDA.
+ *   - A handle must not be used from two threads at once.
+ */
+#ifndef LM_H
+#define LM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lm_solver lm_solver; /* opaque */
+
+enum { LM_F32 = 0, LM_F64 = 1 };
+
+enum {
+    LM_OK = 0,
+    LM_E_INVALID = -1, /* bad argument: N <= 0, eta <= 0, a <= 0, unknown precision, nrhs < 1, tol <= 0 */
+    LM_E_NOPOS = -2,   /* compute call before lm_set_positions */
+    LM_E_ANGULAR = -3, /* torques / angular output given but include_angular == 0, or angular output missing */
+    LM_E_NULL = -4,    /* a required pointer is NULL */
+    LM_E_CUDA = -5,    /* CUDA runtime error (message in lm_last_error) */
+    LM_E_NOCONV = -6   /* Lanczos reached max_iter before meeting tol; the last iterate IS written */
+};
+
+/* Create a solver for N equal spheres of hydrodynamic radius a in an unbounded fluid of viscosity
+ * eta.  include_angular != 0: torques are accepted and angular velocities returned (dof = 6N),
+ * else forces -> linear velocities only (dof = 3N; "more efficient").  Uses the
+ * current CUDA device; all later calls on the handle must run with that device current. */
+int lm_create(lm_solver** out, int precision, int64_t N, double eta, double a, int include_angular);
+int lm_destroy(lm_solver* h);
+
+/* Store the particle positions (3N).  The library keeps its own packed copy; `pos` may be reused
+ * by the caller as soon as the stream has passed this call. */
+int lm_set_positions(lm_solver* h, const void* pos, void* stream);
+
+/* U = M.[F;T]  (eq. (7)).  forces / torques: 3N each or NULL; NULL means zeros
+ * ("one or both of forces and torques"), but not both NULL.  lin_out: 3N, required.  ang_out: 3N,
+ * required iff include_angular.  torques != NULL or ang_out != NULL without include_angular
+ * -> LM_E_ANGULAR. */
+int lm_mdot(lm_solver* h, const void* forces, const void* torques, void* lin_out, void* ang_out, void* stream);
+
+/* nrhs independent right-hand sides sharing one position set: the pair geometry is evaluated
+ * once per pair and applied to every force vector.  forces/torques [nrhs][3N] -> lin_out/ang_out
+ * [nrhs][3N].  Same NULL rules as lm_mdot. */
+int lm_mdot_batch(lm_solver* h, int nrhs, const void* forces, const void* torques, void* lin_out,
+                  void* ang_out, void* stream);
+
+/* y = M^{1/2} W by Lanczos.  noise: dof values, [3N linear | 3N angular]
+ * (the caller draws W ~ N(0,1); the paper's sqrtMdotW() draws it internally).
+ * tol: stop when the relative change between successive iterates is <= tol (S3).
+ * lin_out 3N, ang_out 3N (iff include_angular).  iters_out: HOST int*, may be NULL.
+ * LM_E_NOCONV if max_iter is reached (result still written). */
+int lm_sqrt_mdot_w(lm_solver* h, const void* noise, double tol, void* lin_out, void* ang_out,
+                   int* iters_out, void* stream);
+
+/* out = M.[F;T] + noise_prefactor * M^{1/2} W  (+ 0 thermal drift): the right-hand
+ * side of eq. (9) for dt = 1 with noise_prefactor = sqrt(2 k_B T / dt) supplied by the caller
+ * (PAPER.md:116-118).  noise == NULL: deterministic part only (tol ignored). */
+int lm_hydrodynamic_velocities(lm_solver* h, const void* forces, const void* torques, const void* noise,
+                               double noise_prefactor, double tol, void* lin_out, void* ang_out, void* stream);
+
+/* Host-pointer variants: identical semantics, all array pointers are HOST memory in the handle's
+ * precision.  Each copies its inputs to the device, runs the device path above and copies the
+ * results back, all on `stream`, and returns after the results have landed. */
+int lm_set_positions_host(lm_solver* h, const void* pos, void* stream);
+int lm_mdot_host(lm_solver* h, const void* forces, const void* torques, void* lin_out, void* ang_out, void* stream);
+int lm_mdot_batch_host(lm_solver* h, int nrhs, const void* forces, const void* torques, void* lin_out,
+                       void* ang_out, void* stream);
+int lm_sqrt_mdot_w_host(lm_solver* h, const void* noise, double tol, void* lin_out, void* ang_out,
+                        int* iters_out, void* stream);
+int lm_hydrodynamic_velocities_host(lm_solver* h, const void* forces, const void* torques, const void* noise,
+                                    double noise_prefactor, double tol, void* lin_out, void* ang_out, void* stream);
+
+/* Lanczos controls and introspection. */
+int lm_set_max_iter(lm_solver* h, int max_iter);     /* default 100; 1 <= max_iter <= 1000 */
+int lm_last_iterations(const lm_solver* h);           /* iterations of the last Lanczos call (or < 0) */
+const char* lm_last_error(const lm_solver* h);        /* never NULL; "" if the last call succeeded */
+
+/* Launch accounting for benchmarks.  Counters accumulate from lm_create or the last reset.
+ * With profiling on (lm_set_profiling(h, 1)) every pair-kernel launch is bracketed by CUDA events
+ * on its stream; lm_get_stats then waits for those events and reports their summed time.
+ * pair_kernel_launches: O(N^2) kernel launches; aux_launches: O(N) pack / reduce / vector kernels;
+ * pair_kernel_ms: summed device time of the pair kernel (0 unless profiling);
+ * pairs: ordered (i,j) pair evaluations performed (N^2 per launch, all right-hand sides share it). */
+int lm_set_profiling(lm_solver* h, int on);
+int lm_reset_stats(lm_solver* h);
+int lm_get_stats(lm_solver* h, int64_t* pair_kernel_launches, int64_t* aux_launches, double* pair_kernel_ms,
+                 double* pairs);
+
+/* The launch configuration the next lm_mdot_batch(nrhs) would use: grid = i_tiles x j_splits CTAs
+ * of `block` threads, `targets_per_thread` targets each, `smem_bytes` dynamic shared memory. */
+int lm_pair_launch_config(lm_solver* h, int nrhs, int* i_tiles, int* j_splits, int* block,
+                          int* targets_per_thread, int* smem_bytes);
+
+/* Host-only helper of the Lanczos driver, exported so that it can be tested without a GPU:
+ * c = T^{1/2} e_1 for the symmetric tridiagonal T = tridiag(beta[0..k-2]; alpha[0..k-1]) by an
+ * implicit-shift QL eigensolve in fp64, negative eigenvalues clamped to 0.  c_out: k doubles. */
+int lm_host_tridiag_sqrt_e1(int k, const double* alpha, const double* beta, double* c_out);
+
+/* Diagnostic: measured FMA-pipe peak of the current device, in lane-operations per second
+ * (one lane-op = one fp32 / fp64 FMA on one lane), from a register-only FFMA2 / DFMA loop run for
+ * about `seconds`.  This is the roofline denominator bench.py reports next to the nominal one. */
+int lm_probe_fma_peak(int precision, double seconds, double* lane_ops_per_s);
+
+/* Library version string (static storage). */
+const char* lm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LM_H */

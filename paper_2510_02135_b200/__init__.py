@@ -1,0 +1,11 @@
+"""B200-native open-boundary RPY mobility (M.F) and Lanczos sqrt(M).W -- Python binding of liblm.
+
+The product is the C-ABI CUDA library ``liblm.so`` (``include/lm.h``).  This package only
+marshals arguments (``binding.py``); every step of the path runs in the library's kernels.
+``workloads.py`` holds the seeded synthetic inputs of the five benchmark configs.
+"""
+from . import workloads  # noqa: F401
+from .binding import (  # noqa: F401
+    LM_E_ANGULAR, LM_E_CUDA, LM_E_INVALID, LM_E_NOCONV, LM_E_NOPOS, LM_E_NULL, LM_F32, LM_F64, LM_OK,
+    LmError, Solver, lib, lm_host_tridiag_sqrt_e1, lm_probe_fma_peak, lm_version,
+)

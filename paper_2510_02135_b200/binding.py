@@ -1,0 +1,245 @@
+"""ctypes binding of liblm.so -- argument marshalling only.
+
+Module-level ``lib()`` returns the loaded library with every ``lm_*`` symbol of ``include/lm.h``
+typed; ``Solver`` wraps a handle and forwards to the same-named C calls (``mdot`` -> ``lm_mdot``
+...).  Tensors are torch CUDA tensors (device entry points) or numpy / CPU tensors (``*_host``
+entry points); torch is used for device memory and streams only.
+
+There is no fallback: if the library cannot be built or loaded, importing ``lib()`` raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, c_char_p, c_double, c_int, c_int64, c_void_p
+
+import numpy as np
+
+LM_F32, LM_F64 = 0, 1
+LM_OK, LM_E_INVALID, LM_E_NOPOS, LM_E_ANGULAR, LM_E_NULL, LM_E_CUDA, LM_E_NOCONV = 0, -1, -2, -3, -4, -5, -6
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "liblm.so")
+_lib = None
+
+# name -> (restype, argtypes); mirrors include/lm.h one to one
+SIGNATURES = {
+    "lm_create": (c_int, [POINTER(c_void_p), c_int, c_int64, c_double, c_double, c_int]),
+    "lm_destroy": (c_int, [c_void_p]),
+    "lm_set_positions": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "lm_mdot": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "lm_mdot_batch": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "lm_sqrt_mdot_w": (c_int, [c_void_p, c_void_p, c_double, c_void_p, c_void_p, POINTER(c_int), c_void_p]),
+    "lm_hydrodynamic_velocities": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_void_p, c_void_p, c_void_p]),
+    "lm_set_positions_host": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "lm_mdot_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "lm_mdot_batch_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "lm_sqrt_mdot_w_host": (c_int, [c_void_p, c_void_p, c_double, c_void_p, c_void_p, POINTER(c_int), c_void_p]),
+    "lm_hydrodynamic_velocities_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_void_p, c_void_p, c_void_p]),
+    "lm_set_max_iter": (c_int, [c_void_p, c_int]),
+    "lm_last_iterations": (c_int, [c_void_p]),
+    "lm_last_error": (c_char_p, [c_void_p]),
+    "lm_set_profiling": (c_int, [c_void_p, c_int]),
+    "lm_reset_stats": (c_int, [c_void_p]),
+    "lm_get_stats": (c_int, [c_void_p, POINTER(c_int64), POINTER(c_int64), POINTER(c_double), POINTER(c_double)]),
+    "lm_pair_launch_config": (c_int, [c_void_p, c_int, POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int)]),
+    "lm_host_tridiag_sqrt_e1": (c_int, [c_int, POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
+    "lm_probe_fma_peak": (c_int, [c_int, c_double, POINTER(c_double)]),
+    "lm_version": (c_char_p, []),
+}
+
+
+class LmError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"liblm error {code}: {message}")
+        self.code = code
+
+
+def lib():
+    """Load liblm.so (building it in-tree with nvcc if it is missing or stale)."""
+    global _lib
+    if _lib is None:
+        from . import build as _build
+        path = _build.build() if (not os.path.exists(_LIB_PATH) or _build.stale()) else _LIB_PATH
+        cdll = ctypes.CDLL(path)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(cdll, name)          # AttributeError here = the library is missing a declared symbol
+            fn.restype, fn.argtypes = res, args
+        _lib = cdll
+    return _lib
+
+
+def lm_version() -> str:
+    return lib().lm_version().decode()
+
+
+def lm_host_tridiag_sqrt_e1(alpha, beta) -> np.ndarray:
+    alpha = np.ascontiguousarray(alpha, dtype=np.float64)
+    beta = np.ascontiguousarray(beta, dtype=np.float64)
+    k = alpha.size
+    out = np.zeros(k)
+    dp = POINTER(c_double)
+    rc = lib().lm_host_tridiag_sqrt_e1(k, alpha.ctypes.data_as(dp), beta.ctypes.data_as(dp) if k > 1 else None, out.ctypes.data_as(dp))
+    if rc != LM_OK:
+        raise LmError(rc, "lm_host_tridiag_sqrt_e1")
+    return out
+
+
+def lm_probe_fma_peak(precision: int, seconds: float = 0.2) -> float:
+    out = c_double(0.0)
+    rc = lib().lm_probe_fma_peak(precision, seconds, ctypes.byref(out))
+    if rc != LM_OK:
+        raise LmError(rc, "lm_probe_fma_peak")
+    return out.value
+
+
+def _ptr(x):
+    """Raw address of a torch tensor / numpy array (None -> NULL).  No copies, no conversions."""
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        if not x.flags["C_CONTIGUOUS"]:
+            raise ValueError("array must be C-contiguous")
+        return c_void_p(x.ctypes.data)
+    if not x.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    return c_void_p(x.data_ptr())
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return c_void_p(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return c_void_p(stream)
+    return c_void_p(stream.cuda_stream)
+
+
+class Solver:
+    """A handle of liblm.  Methods map 1:1 to the C calls and only marshal arguments."""
+
+    def __init__(self, precision: str | int, N: int, eta: float = 1.0, a: float = 1.0, include_angular: bool = False):
+        self.precision = {"f32": LM_F32, "f64": LM_F64}.get(precision, precision)
+        self.N, self.eta, self.a, self.angular = int(N), float(eta), float(a), bool(include_angular)
+        self._h = c_void_p()
+        rc = lib().lm_create(ctypes.byref(self._h), self.precision, self.N, self.eta, self.a, int(self.angular))
+        if rc != LM_OK:
+            self._h = c_void_p()
+            raise LmError(rc, "lm_create failed (bad argument, or no CUDA device)")
+
+    # -- helpers
+    @property
+    def torch_dtype(self):
+        import torch
+        return torch.float32 if self.precision == LM_F32 else torch.float64
+
+    @property
+    def np_dtype(self):
+        return np.float32 if self.precision == LM_F32 else np.float64
+
+    def _check(self, rc, allow=()):
+        if rc != LM_OK and rc not in allow:
+            raise LmError(rc, lib().lm_last_error(self._h).decode())
+        return rc
+
+    def _expect(self, x, n, host):
+        if x is None:
+            return
+        dt = self.np_dtype if host else self.torch_dtype
+        if x.dtype != dt:
+            raise TypeError(f"expected dtype {dt}, got {x.dtype}")
+        size = x.size if isinstance(x, np.ndarray) else x.numel()
+        if size != n:
+            raise ValueError(f"expected {n} elements, got {size}")
+        if not host and not x.is_cuda:
+            raise TypeError("device entry point needs a CUDA tensor (use the *_host call for host arrays)")
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib().lm_destroy(self._h)
+            self._h = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- device entry points (torch CUDA tensors)
+    def set_positions(self, pos, stream=None):
+        self._expect(pos, 3 * self.N, False)
+        self._check(lib().lm_set_positions(self._h, _ptr(pos), _stream_ptr(stream)))
+
+    def mdot(self, forces, torques, lin_out, ang_out=None, stream=None):
+        for x in (forces, torques, lin_out, ang_out):
+            self._expect(x, 3 * self.N, False)
+        self._check(lib().lm_mdot(self._h, _ptr(forces), _ptr(torques), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+
+    def mdot_batch(self, nrhs, forces, torques, lin_out, ang_out=None, stream=None):
+        for x in (forces, torques, lin_out, ang_out):
+            self._expect(x, nrhs * 3 * self.N, False)
+        self._check(lib().lm_mdot_batch(self._h, int(nrhs), _ptr(forces), _ptr(torques), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+
+    def sqrt_mdot_w(self, noise, tol, lin_out, ang_out=None, stream=None, allow_noconv=False) -> int:
+        self._expect(noise, (6 if self.angular else 3) * self.N, False)
+        iters = c_int(0)
+        self._check(lib().lm_sqrt_mdot_w(self._h, _ptr(noise), float(tol), _ptr(lin_out), _ptr(ang_out), ctypes.byref(iters),
+                                         _stream_ptr(stream)), allow=(LM_E_NOCONV,) if allow_noconv else ())
+        return iters.value
+
+    def hydrodynamic_velocities(self, forces, torques, noise, noise_prefactor, tol, lin_out, ang_out=None, stream=None):
+        self._check(lib().lm_hydrodynamic_velocities(self._h, _ptr(forces), _ptr(torques), _ptr(noise), float(noise_prefactor),
+                                                     float(tol), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+
+    # -- host entry points (numpy arrays; pinned memory makes the copies asynchronous)
+    def set_positions_host(self, pos, stream=None):
+        self._expect(pos, 3 * self.N, True)
+        self._check(lib().lm_set_positions_host(self._h, _ptr(pos), _stream_ptr(stream)))
+
+    def mdot_host(self, forces, torques, lin_out, ang_out=None, stream=None):
+        for x in (forces, torques, lin_out, ang_out):
+            self._expect(x, 3 * self.N, True)
+        self._check(lib().lm_mdot_host(self._h, _ptr(forces), _ptr(torques), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+
+    def mdot_batch_host(self, nrhs, forces, torques, lin_out, ang_out=None, stream=None):
+        for x in (forces, torques, lin_out, ang_out):
+            self._expect(x, nrhs * 3 * self.N, True)
+        self._check(lib().lm_mdot_batch_host(self._h, int(nrhs), _ptr(forces), _ptr(torques), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+
+    def sqrt_mdot_w_host(self, noise, tol, lin_out, ang_out=None, stream=None) -> int:
+        self._expect(noise, (6 if self.angular else 3) * self.N, True)
+        iters = c_int(0)
+        self._check(lib().lm_sqrt_mdot_w_host(self._h, _ptr(noise), float(tol), _ptr(lin_out), _ptr(ang_out), ctypes.byref(iters),
+                                              _stream_ptr(stream)))
+        return iters.value
+
+    def hydrodynamic_velocities_host(self, forces, torques, noise, noise_prefactor, tol, lin_out, ang_out=None, stream=None):
+        self._check(lib().lm_hydrodynamic_velocities_host(self._h, _ptr(forces), _ptr(torques), _ptr(noise), float(noise_prefactor),
+                                                          float(tol), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+
+    # -- controls / introspection
+    def set_max_iter(self, n):
+        self._check(lib().lm_set_max_iter(self._h, int(n)))
+
+    def last_iterations(self) -> int:
+        return lib().lm_last_iterations(self._h)
+
+    def last_error(self) -> str:
+        return lib().lm_last_error(self._h).decode()
+
+    def set_profiling(self, on: bool):
+        self._check(lib().lm_set_profiling(self._h, int(on)))
+
+    def reset_stats(self):
+        self._check(lib().lm_reset_stats(self._h))
+
+    def get_stats(self) -> dict:
+        a, b, ms, pairs = c_int64(0), c_int64(0), c_double(0), c_double(0)
+        self._check(lib().lm_get_stats(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(ms), ctypes.byref(pairs)))
+        return dict(pair_kernel_launches=a.value, aux_launches=b.value, pair_kernel_ms=ms.value, pairs=pairs.value)
+
+    def pair_launch_config(self, nrhs: int = 1) -> dict:
+        v = [c_int(0) for _ in range(5)]
+        self._check(lib().lm_pair_launch_config(self._h, int(nrhs), *[ctypes.byref(x) for x in v]))
+        keys = ("i_tiles", "j_splits", "block", "targets_per_thread", "smem_bytes")
+        return {k: x.value for k, x in zip(keys, v)}

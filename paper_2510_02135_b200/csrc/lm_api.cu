@@ -1,0 +1,819 @@
+// lm_api.cu -- C ABI of liblm (include/lm.h): handle, launch configuration, Lanczos driver.
+//
+// Everything numerical runs in the kernels of rpy_pair.cuh / vector_kernels.cuh; the only host
+// arithmetic is the k x k tridiagonal problem of the Lanczos stopping test (tridiag_host.h).
+// There is no CPU fallback: without a CUDA device every compute call returns LM_E_CUDA.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/lm.h"
+#include "rpy_pair.cuh"
+#include "tridiag_host.h"
+#include "vector_kernels.cuh"
+
+namespace lm {
+
+// ---------------------------------------------------------------- pair-kernel variants
+// LARGE: 256 threads x 2 targets, 512-source tiles.  SMALL: 128 x 1, 128-source tiles (fills
+// 148 SMs when N is small, SURVEY.md sec. 7 "Small N").  npad is a multiple of NPAD_QUANTUM so
+// that either variant tiles it exactly.
+constexpr int NPAD_QUANTUM = 512;
+constexpr int L_BLOCK = 256, L_TPT = 2, L_TJ = 512, L_STAGES = 2;
+constexpr int S_BLOCK = 128, S_TPT = 1, S_TJ = 128, S_STAGES = 2;
+
+template <typename T> struct Variant {
+    void (*kernel)(const PairParams<T>);
+    int nrhs, ang, block, tpt, tj, smem;
+    int ctas_per_sm;      // filled at first use (occupancy API)
+    double efficiency;    // relative per-pair throughput used by the launch chooser
+};
+
+template <typename T, int NRHS, bool ANG, int MINB> Variant<T> make_large()
+{
+    using Tr = PairKernelTraits<T, NRHS, ANG, L_TPT, L_BLOCK, L_TJ, L_STAGES>;
+    return {rpy_pair_kernel<T, NRHS, ANG, L_TPT, L_BLOCK, L_TJ, L_STAGES, MINB>, NRHS, ANG, L_BLOCK, L_TPT, L_TJ, Tr::SMEM_BYTES, 0, 1.0};
+}
+template <typename T, int NRHS, bool ANG, int MINB> Variant<T> make_small()
+{
+    using Tr = PairKernelTraits<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES>;
+    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, MINB>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, Tr::SMEM_BYTES, 0, 0.85};
+}
+
+template <typename T> std::vector<Variant<T>> build_variants();
+template <> std::vector<Variant<float>> build_variants<float>()
+{
+    return {make_large<float, 1, false, 2>(), make_large<float, 2, false, 2>(), make_large<float, 4, false, 1>(),
+            make_large<float, 1, true, 2>(),  make_large<float, 2, true, 1>(),
+            make_small<float, 1, false, 3>(), make_small<float, 2, false, 3>(), make_small<float, 4, false, 3>(),
+            make_small<float, 1, true, 3>(),  make_small<float, 2, true, 3>()};
+}
+template <> std::vector<Variant<double>> build_variants<double>()
+{
+    return {make_large<double, 1, false, 2>(), make_large<double, 2, false, 1>(), make_large<double, 4, false, 1>(),
+            make_large<double, 1, true, 1>(),  make_large<double, 2, true, 1>(),
+            make_small<double, 1, false, 3>(), make_small<double, 2, false, 3>(), make_small<double, 4, false, 2>(),
+            make_small<double, 1, true, 3>(),  make_small<double, 2, true, 2>()};
+}
+
+struct LaunchPlan {
+    int variant = -1;
+    int i_tiles = 0, j_splits = 0, tiles_per_split = 0, n_tiles = 0;
+};
+
+}  // namespace lm
+
+using namespace lm;
+
+// ---------------------------------------------------------------- handle
+struct lm_solver {
+    int precision = LM_F32;
+    int64_t N = 0, npad = 0;
+    double eta = 1.0, a = 1.0;
+    int angular = 0;
+    int max_iter = 100;
+    int device = 0, sm_count = 0;
+    bool have_pos = false;
+    std::string err;
+    int last_iters = -1;
+
+    void* pos_soa = nullptr;
+    void* vec_soa = nullptr;   size_t vec_soa_bytes = 0;
+    void* partial = nullptr;   size_t partial_bytes = 0;
+
+    // Lanczos workspace
+    void* V = nullptr;         size_t V_bytes = 0;
+    void* w = nullptr;         size_t w_bytes = 0;
+    double* d_scal = nullptr;  // [0] |z|^2  [1] alpha  [2] beta^2
+    double* d_block = nullptr; // block partials of the reductions
+    unsigned int* d_ticket = nullptr;
+    double* d_coef = nullptr;  size_t coef_cap = 0;   // coef_cap also sizes the Gram buffers below
+    double* h_scal = nullptr;  // pinned, 4 doubles
+    double* d_gram = nullptr;  // Gram column V[j].V[k], j <= k
+    double* d_gram_part = nullptr;
+    double* h_gram = nullptr;  // pinned
+
+    // staging for the _host entry points
+    void* st[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // pos, f, t, noise, lin, ang
+    size_t st_bytes[6] = {0, 0, 0, 0, 0, 0};
+
+    // variants (typed; only the handle's precision is populated)
+    std::vector<Variant<float>> vf;
+    std::vector<Variant<double>> vd;
+
+    // stats
+    int64_t n_pair = 0, n_aux = 0;
+    double pairs = 0.0, pair_ms = 0.0;
+    bool profiling = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> pending;
+    std::vector<cudaEvent_t> event_pool;
+};
+
+namespace {
+
+int fail(lm_solver* h, int code, const std::string& msg)
+{
+    if (h) h->err = msg;
+    return code;
+}
+
+#define LM_CUDA(h, expr)                                                                              \
+    do {                                                                                              \
+        cudaError_t e__ = (expr);                                                                     \
+        if (e__ != cudaSuccess) {                                                                     \
+            char buf__[512];                                                                          \
+            std::snprintf(buf__, sizeof buf__, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+            return fail(h, LM_E_CUDA, buf__);                                                         \
+        }                                                                                             \
+    } while (0)
+
+size_t esize(const lm_solver* h) { return h->precision == LM_F32 ? 4 : 8; }
+int64_t dof_of(const lm_solver* h) { return (h->angular ? 6 : 3) * h->N; }
+
+int ensure(lm_solver* h, void** ptr, size_t* cap, size_t bytes)
+{
+    if (*cap >= bytes && *ptr) return LM_OK;
+    if (*ptr) LM_CUDA(h, cudaFree(*ptr));
+    *ptr = nullptr;
+    *cap = 0;
+    LM_CUDA(h, cudaMalloc(ptr, bytes));
+    *cap = bytes;
+    return LM_OK;
+}
+
+template <typename T> PairConsts<T> make_consts(double eta, double a)
+{
+    const double pi = 3.14159265358979323846264338327950288;
+    PairConsts<T> c;
+    const double C1 = 1.0 / (8.0 * pi * eta);          // Oseen prefactor
+    const double C4 = 1.0 / (6.0 * pi * eta * a);      // translational self mobility
+    const double C7 = 1.0 / (16.0 * pi * eta);
+    const double C8 = 1.0 / (8.0 * pi * eta * a * a * a);  // rotational self mobility
+    // floor of r^2: r = 0 becomes r = a 2^-40 (fp32) / a 2^-100 (fp64): a relative perturbation of the
+    // self term far below the type's epsilon, while 1/r^3 stays finite (1/r^5 may overflow to +inf in
+    // fp32; it only feeds the far branch, which the select discards for r < 2a)
+    c.tiny = (T)std::max(a * a * std::ldexp(1.0, sizeof(T) == 4 ? -80 : -200), sizeof(T) == 4 ? 4.8e-38 : 1e-300);
+    c.four_a2 = (T)(4.0 * a * a);
+    c.C1 = (T)C1;
+    c.C2 = (T)(C1 * 2.0 * a * a / 3.0);
+    c.nC3 = (T)(-C1 * 2.0 * a * a);
+    c.C4 = (T)C4;
+    c.nC5 = (T)(-C4 * 9.0 / (32.0 * a));
+    c.C6 = (T)(C4 * 3.0 / (32.0 * a));
+    c.nC7 = (T)(-C7);
+    c.C7x3 = (T)(3.0 * C7);
+    c.C8 = (T)C8;
+    c.K1 = (T)(-C8 * 27.0 / (32.0 * a));
+    c.K2 = (T)(C8 * 5.0 / (64.0 * a * a * a));
+    c.K3 = (T)(C8 * 9.0 / (32.0 * a));
+    c.K4 = (T)(-C8 * 3.0 / (64.0 * a * a * a));
+    c.K5 = (T)(1.0 / (16.0 * pi * eta * a * a * a));
+    c.K6 = (T)(-3.0 / (128.0 * pi * eta * a * a * a * a));
+    return c;
+}
+
+template <typename T> std::vector<Variant<T>>& variants(lm_solver* h);
+template <> std::vector<Variant<float>>& variants<float>(lm_solver* h) { return h->vf; }
+template <> std::vector<Variant<double>>& variants<double>(lm_solver* h) { return h->vd; }
+
+template <typename T> int init_variants(lm_solver* h)
+{
+    auto& vs = variants<T>(h);
+    vs = build_variants<T>();
+    for (auto& v : vs) {
+        LM_CUDA(h, cudaFuncSetAttribute((const void*)v.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem));
+        int nb = 0;
+        LM_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)v.kernel, v.block, v.smem));
+        v.ctas_per_sm = std::max(nb, 1);
+    }
+    return LM_OK;
+}
+
+// Pick the variant and the number of j-splits: minimise (waves) x (tiles per CTA) x (cost of a
+// CTA-tile), where a wave is one resident set of CTAs.  Grid sizing in multiples of the SM count
+// x resident CTAs is what keeps the tail small (148 SMs).
+template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
+{
+    const auto& vs = variants<T>(h);
+    LaunchPlan best;
+    double best_cost = 1e300;
+    for (int vi = 0; vi < (int)vs.size(); ++vi) {
+        const auto& v = vs[vi];
+        if (v.nrhs != nrhs || v.ang != h->angular) continue;
+        const int targets = v.block * v.tpt;
+        const int i_tiles = (int)((h->N + targets - 1) / targets);
+        const int n_tiles = (int)(h->npad / v.tj);
+        const int64_t slots = (int64_t)h->sm_count * v.ctas_per_sm;
+        const int max_splits = std::min(n_tiles, 128);
+        for (int s = 1; s <= max_splits; ++s) {
+            const int tps = (n_tiles + s - 1) / s;
+            const int s_eff = (n_tiles + tps - 1) / tps;   // splits actually needed with that tile count
+            if (s_eff != s) continue;
+            const int64_t ctas = (int64_t)i_tiles * s;
+            const int64_t waves = (ctas + slots - 1) / slots;
+            // time of one wave-tile: ctas_per_sm CTAs share an SM
+            // (+0.35 tile per CTA: prologue, pipeline fill and epilogue of a CTA, measured order of magnitude)
+            double cost = (double)waves * (tps + 0.35) * v.ctas_per_sm * ((double)v.tj * targets) / v.efficiency;
+            // cost is in pairs evaluated back to back on one SM (~1e4 per microsecond): the reduce pass
+            // adds a ~3 us launch plus writing and re-reading s partial vectors
+            if (s > 1) cost += 3.0e4 + 0.1 * (double)s * (double)h->N;
+            if (cost < best_cost) {
+                best_cost = cost;
+                best.variant = vi;
+                best.i_tiles = i_tiles;
+                best.j_splits = s;
+                best.tiles_per_split = tps;
+                best.n_tiles = n_tiles;
+            }
+        }
+    }
+    return best;
+}
+
+cudaEvent_t get_event(lm_solver* h)
+{
+    if (!h->event_pool.empty()) {
+        cudaEvent_t e = h->event_pool.back();
+        h->event_pool.pop_back();
+        return e;
+    }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+
+int grid_1d(int64_t n) { return (int)std::max<int64_t>(1, (n + VEC_BLOCK - 1) / VEC_BLOCK); }
+int grid_red(int64_t n) { return (int)std::min<int64_t>(RED_MAX_BLOCKS, std::max<int64_t>(1, (n + VEC_BLOCK - 1) / VEC_BLOCK)); }
+
+// ---------------------------------------------------------------- device apply: out = M . rhs  (nrhs <= MAX_RHS)
+template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& in, const RhsOut<T>& out, cudaStream_t st)
+{
+    const int nc = h->angular ? 6 : 3;
+    const LaunchPlan plan = choose_plan<T>(h, nrhs);
+    if (plan.variant < 0) return fail(h, LM_E_INVALID, "no pair-kernel variant for this nrhs");
+    const auto& v = variants<T>(h)[plan.variant];
+
+    int rc = ensure(h, &h->vec_soa, &h->vec_soa_bytes, (size_t)nrhs * nc * h->npad * sizeof(T));
+    if (rc != LM_OK) return rc;
+    if (plan.j_splits > 1) {
+        rc = ensure(h, &h->partial, &h->partial_bytes, (size_t)plan.j_splits * nrhs * nc * h->npad * sizeof(T));
+        if (rc != LM_OK) return rc;
+    }
+    pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>(in, nrhs, nc, h->N, h->npad, (T*)h->vec_soa);
+    h->n_aux++;
+
+    PairParams<T> p;
+    p.pos = (const T*)h->pos_soa;
+    p.vec = (const T*)h->vec_soa;
+    p.out = out;
+    p.partial = (T*)h->partial;
+    p.N = h->N;
+    p.npad = h->npad;
+    p.tiles_per_split = plan.tiles_per_split;
+    p.n_tiles = plan.n_tiles;
+    p.c = make_consts<T>(h->eta, h->a);
+
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (h->profiling) {
+        e0 = get_event(h);
+        e1 = get_event(h);
+        LM_CUDA(h, cudaEventRecord(e0, st));
+    }
+    v.kernel<<<dim3(plan.i_tiles, plan.j_splits), v.block, v.smem, st>>>(p);
+    if (h->profiling) {
+        LM_CUDA(h, cudaEventRecord(e1, st));
+        h->pending.emplace_back(e0, e1);
+    }
+    h->n_pair++;
+    h->pairs += (double)h->N * (double)h->N;
+    if (plan.j_splits > 1) {
+        reduce_partials_kernel<T><<<grid_1d(h->N), VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc, h->N, h->npad, out);
+        h->n_aux++;
+    }
+    LM_CUDA(h, cudaGetLastError());
+    return LM_OK;
+}
+
+// any nrhs: chunks of 4, 2, 1 right-hand sides per launch
+template <typename T>
+int apply_batch(lm_solver* h, int nrhs, const T* forces, const T* torques, T* lin_out, T* ang_out, cudaStream_t st)
+{
+    const int64_t n3 = 3 * h->N;
+    int q = 0;
+    while (q < nrhs) {
+        int chunk = nrhs - q >= 4 ? 4 : (nrhs - q >= 2 ? 2 : 1);
+        if (h->angular && chunk > 2) chunk = 2;     // angular variants exist for 1 and 2 right-hand sides
+        RhsIn<T> in{};
+        RhsOut<T> out{};
+        for (int r = 0; r < chunk; ++r) {
+            in.f[r] = forces ? forces + (q + r) * n3 : nullptr;
+            in.t[r] = torques ? torques + (q + r) * n3 : nullptr;
+            out.lin[r] = lin_out + (q + r) * n3;
+            out.ang[r] = ang_out ? ang_out + (q + r) * n3 : nullptr;
+        }
+        const int rc = apply_device<T>(h, chunk, in, out, st);
+        if (rc != LM_OK) return rc;
+        q += chunk;
+    }
+    return LM_OK;
+}
+
+// ---------------------------------------------------------------- Lanczos driver (a7-a10)
+template <typename T>
+int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_out, double scale, int accumulate, cudaStream_t st)
+{
+    const int64_t dof = dof_of(h), n3 = 3 * h->N;
+    const int kmax = h->max_iter;
+    int rc;
+    if ((rc = ensure(h, &h->V, &h->V_bytes, (size_t)(kmax + 1) * dof * sizeof(T))) != LM_OK) return rc;
+    if ((rc = ensure(h, &h->w, &h->w_bytes, (size_t)dof * sizeof(T))) != LM_OK) return rc;
+    if (!h->d_scal) {
+        LM_CUDA(h, cudaMalloc((void**)&h->d_scal, 4 * sizeof(double)));
+        LM_CUDA(h, cudaMalloc((void**)&h->d_block, RED_MAX_BLOCKS * sizeof(double)));
+        LM_CUDA(h, cudaMalloc((void**)&h->d_ticket, sizeof(unsigned int)));
+        LM_CUDA(h, cudaMemsetAsync(h->d_ticket, 0, sizeof(unsigned int), st));
+        LM_CUDA(h, cudaMallocHost((void**)&h->h_scal, 4 * sizeof(double)));
+    }
+    if (h->coef_cap < (size_t)(kmax + 2)) {
+        if (h->d_coef) { LM_CUDA(h, cudaFree(h->d_coef)); LM_CUDA(h, cudaFree(h->d_gram)); LM_CUDA(h, cudaFree(h->d_gram_part)); LM_CUDA(h, cudaFreeHost(h->h_gram)); }
+        h->d_coef = nullptr;
+        h->coef_cap = 0;
+        LM_CUDA(h, cudaMalloc((void**)&h->d_coef, (size_t)(kmax + 2) * sizeof(double)));
+        LM_CUDA(h, cudaMalloc((void**)&h->d_gram, (size_t)(kmax + 2) * sizeof(double)));
+        LM_CUDA(h, cudaMalloc((void**)&h->d_gram_part, (size_t)(kmax + 2) * GRAM_MAX_BLOCKS * sizeof(double)));
+        LM_CUDA(h, cudaMallocHost((void**)&h->h_gram, (size_t)(kmax + 2) * sizeof(double)));
+        h->coef_cap = (size_t)(kmax + 2);
+    }
+    T* V = (T*)h->V;
+    T* w = (T*)h->w;
+    const int gr = grid_red(dof);
+    const int gg = (int)std::min<int64_t>(GRAM_MAX_BLOCKS, std::max<int64_t>(1, dof / (4 * VEC_BLOCK)));
+    const int64_t gchunk = (dof + gg - 1) / gg;
+    // Gram matrix of the basis, G[i][j] = V[i].V[j], filled one column per new basis vector
+    std::vector<double> G((size_t)(kmax + 1) * (kmax + 1), 0.0);
+    const int ldg = kmax + 1;
+    auto gram_launch = [&](int m) {   // column m: V[j].V[m], j <= m  -> pinned h_gram
+        gram_column_kernel<T><<<gg, VEC_BLOCK, 0, st>>>(V, dof, m, gchunk, h->d_gram_part, h->d_ticket, h->d_gram);
+        h->n_aux++;
+        return cudaMemcpyAsync(h->h_gram, h->d_gram, (size_t)(m + 1) * sizeof(double), cudaMemcpyDeviceToHost, st);
+    };
+    auto gram_store = [&](int m) { for (int j = 0; j <= m; ++j) G[(size_t)j * ldg + m] = G[(size_t)m * ldg + j] = h->h_gram[j]; };
+
+    // v_1 = z / |z|
+    sumsq_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise, dof, h->d_block, h->d_ticket, h->d_scal + 0);
+    scale_by_inv_norm_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise, dof, h->d_scal + 0, V);
+    h->n_aux += 2;
+    LM_CUDA(h, cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(double), cudaMemcpyDeviceToHost, st));
+    LM_CUDA(h, gram_launch(0));
+    LM_CUDA(h, cudaStreamSynchronize(st));
+    gram_store(0);
+    const double znorm = std::sqrt(h->h_scal[0]);
+    h->last_iters = 0;
+    if (!(znorm > 0.0)) {            // zero noise: M^{1/2} 0 = 0
+        if (!accumulate) {
+            LM_CUDA(h, cudaMemsetAsync(lin_out, 0, (size_t)n3 * sizeof(T), st));
+            if (h->angular) LM_CUDA(h, cudaMemsetAsync(ang_out, 0, (size_t)n3 * sizeof(T), st));
+        }
+        return LM_OK;
+    }
+
+    std::vector<double> alphas, betas, c_prev, c_cur;
+    bool converged = false;
+    const bool debug = std::getenv("LM_DEBUG_LANCZOS") != nullptr;   // per-iteration trace on stderr
+    const double breakdown = (h->precision == LM_F32) ? 1e-6 : 1e-14;
+    int k = 0;
+    for (k = 1; k <= kmax; ++k) {
+        T* vk = V + (size_t)(k - 1) * dof;
+        RhsIn<T> in{};
+        RhsOut<T> out{};
+        in.f[0] = vk;
+        in.t[0] = h->angular ? vk + n3 : nullptr;
+        out.lin[0] = w;
+        out.ang[0] = h->angular ? w + n3 : nullptr;
+        if ((rc = apply_device<T>(h, 1, in, out, st)) != LM_OK) return rc;          // w = M v_k
+        lanczos_alpha_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(w, vk, k > 1 ? vk - dof : nullptr, h->d_scal + 2, dof, h->d_block, h->d_ticket,
+                                                          h->d_scal + 1);           // w -= beta_{k-1} v_{k-1}; alpha_k
+        lanczos_beta_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(w, vk, h->d_scal + 1, dof, h->d_block, h->d_ticket, h->d_scal + 2);  // w -= alpha v; beta^2
+        LM_CUDA(h, cudaMemcpyAsync(h->h_scal + 1, h->d_scal + 1, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        scale_by_inv_norm_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(w, dof, h->d_scal + 2, vk + dof);    // v_{k+1} = w / beta_k
+        h->n_aux += 3;
+        if (k < kmax) LM_CUDA(h, gram_launch(k));                                                  // V[k] = v_{k+1} against V[0..k]
+        LM_CUDA(h, cudaStreamSynchronize(st));
+        const double alpha = h->h_scal[1], beta = std::sqrt(std::max(h->h_scal[2], 0.0));
+        if (!std::isfinite(alpha) || !std::isfinite(beta)) return fail(h, LM_E_CUDA, "Lanczos: non-finite alpha/beta (non-finite input?)");
+        alphas.push_back(alpha);
+        c_cur.assign(k, 0.0);
+        if (!tridiag_sqrt_e1(k, alphas.data(), betas.data(), c_cur.data())) return fail(h, LM_E_NOCONV, "Lanczos: tridiagonal eigensolve did not converge");
+        if (k >= 2) {
+            // |y_k - y_{k-1}|^2 / |z|^2 = delta^T G_k delta,  |y_{k-1}|^2 / |z|^2 = c_{k-1}^T G_{k-1} c_{k-1}
+            std::vector<double> delta(c_cur);
+            for (int i = 0; i < k - 1; ++i) delta[i] -= c_prev[i];
+            double num = 0.0, den = 0.0;
+            for (int i = 0; i < k; ++i)
+                for (int j = 0; j < k; ++j) num += delta[i] * G[(size_t)i * ldg + j] * delta[j];
+            for (int i = 0; i < k - 1; ++i)
+                for (int j = 0; j < k - 1; ++j) den += c_prev[i] * G[(size_t)i * ldg + j] * c_prev[j];
+            if (std::sqrt(std::max(num, 0.0)) <= tol * std::sqrt(std::max(den, 0.0))) converged = true;
+            if (debug) std::fprintf(stderr, "[lm lanczos] k=%d alpha=%.9e beta=%.9e step=%.3e\n", k, alpha, beta, std::sqrt(std::max(num, 0.0) / den));
+        }
+        if (beta <= breakdown * std::fabs(alpha)) converged = true;   // invariant subspace: iterate is exact
+        if (converged) break;
+        if (k < kmax) gram_store(k);
+        betas.push_back(beta);
+        c_prev = c_cur;
+    }
+    if (k > kmax) k = kmax;
+    h->last_iters = k;
+    LM_CUDA(h, cudaMemcpyAsync(h->d_coef, c_cur.data(), (size_t)k * sizeof(double), cudaMemcpyHostToDevice, st));
+    lanczos_combine_kernel<T><<<grid_1d(dof), VEC_BLOCK, 0, st>>>(V, dof, k, h->d_coef, scale * znorm, accumulate, n3, lin_out, ang_out);
+    h->n_aux++;
+    LM_CUDA(h, cudaGetLastError());
+    LM_CUDA(h, cudaStreamSynchronize(st));      // c_cur (pageable) must outlive the copy
+    if (!converged) return fail(h, LM_E_NOCONV, "Lanczos: max_iter reached before the tolerance was met (last iterate written)");
+    return LM_OK;
+}
+
+// ---------------------------------------------------------------- typed front ends
+template <typename T> int set_positions_t(lm_solver* h, const void* pos, cudaStream_t st)
+{
+    pack_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)pos, h->N, h->npad, (T*)h->pos_soa);
+    h->n_aux++;
+    LM_CUDA(h, cudaGetLastError());
+    h->have_pos = true;
+    return LM_OK;
+}
+
+int check_io(lm_solver* h, const void* forces, const void* torques, const void* lin_out, const void* ang_out, bool need_input)
+{
+    if (!h) return LM_E_NULL;
+    h->err.clear();
+    if (!h->have_pos) return fail(h, LM_E_NOPOS, "positions not set: call lm_set_positions first");
+    if (!lin_out) return fail(h, LM_E_NULL, "lin_out is NULL");
+    if (!h->angular && (torques || ang_out)) return fail(h, LM_E_ANGULAR, "torques / ang_out given but the solver was created with include_angular = 0");
+    if (h->angular && !ang_out) return fail(h, LM_E_ANGULAR, "include_angular = 1 requires ang_out");
+    if (need_input && !forces && !torques) return fail(h, LM_E_NULL, "forces and torques are both NULL");
+    return LM_OK;
+}
+
+int stage_in(lm_solver* h, int slot, const void* host, size_t bytes, cudaStream_t st, void** dev)
+{
+    *dev = nullptr;
+    if (!host) return LM_OK;
+    int rc = ensure(h, &h->st[slot], &h->st_bytes[slot], bytes);
+    if (rc != LM_OK) return rc;
+    LM_CUDA(h, cudaMemcpyAsync(h->st[slot], host, bytes, cudaMemcpyHostToDevice, st));
+    *dev = h->st[slot];
+    return LM_OK;
+}
+int stage_out_alloc(lm_solver* h, int slot, const void* host, size_t bytes, void** dev)
+{
+    *dev = nullptr;
+    if (!host) return LM_OK;
+    int rc = ensure(h, &h->st[slot], &h->st_bytes[slot], bytes);
+    if (rc != LM_OK) return rc;
+    *dev = h->st[slot];
+    return LM_OK;
+}
+
+// register-only FMA loops for lm_probe_fma_peak
+__global__ void probe_ffma2_kernel(float* out, float a, float b, int iters)
+{
+    float2 x[8];
+    const float2 aa = make_float2(a, a), bb = make_float2(b, b);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = make_float2(threadIdx.x * 1e-3f + i, (float)i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = __ffma2_rn(x[i], aa, bb);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i].x + x[i].y;
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+__global__ void probe_dfma_kernel(double* out, double a, double b, int iters)
+{
+    double x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = threadIdx.x * 1e-3 + i;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = fma(x[i], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+}  // namespace
+
+// ================================================================ C ABI
+extern "C" {
+
+const char* lm_version(void) { return "liblm 0.1 (sm_100a)"; }
+
+int lm_create(lm_solver** out, int precision, int64_t N, double eta, double a, int include_angular)
+{
+    if (!out) return LM_E_NULL;
+    *out = nullptr;
+    if ((precision != LM_F32 && precision != LM_F64) || N <= 0 || !(eta > 0.0) || !(a > 0.0) || !std::isfinite(eta) || !std::isfinite(a))
+        return LM_E_INVALID;
+    if (N > (int64_t)1 << 28) return LM_E_INVALID;
+    lm_solver* h = new lm_solver();
+    h->precision = precision;
+    h->N = N;
+    h->eta = eta;
+    h->a = a;
+    h->angular = include_angular ? 1 : 0;
+    h->npad = (N + NPAD_QUANTUM - 1) / NPAD_QUANTUM * NPAD_QUANTUM;
+    auto bail = [&](int code) { lm_destroy(h); return code; };
+    if (cudaGetDevice(&h->device) != cudaSuccess) return bail(LM_E_CUDA);
+    if (cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess) return bail(LM_E_CUDA);
+    if (cudaMalloc(&h->pos_soa, (size_t)3 * h->npad * esize(h)) != cudaSuccess) return bail(LM_E_CUDA);
+    const int rc = precision == LM_F32 ? init_variants<float>(h) : init_variants<double>(h);
+    if (rc != LM_OK) return bail(rc);
+    *out = h;
+    return LM_OK;
+}
+
+int lm_destroy(lm_solver* h)
+{
+    if (!h) return LM_OK;
+    cudaFree(h->pos_soa);
+    cudaFree(h->vec_soa);
+    cudaFree(h->partial);
+    cudaFree(h->V);
+    cudaFree(h->w);
+    cudaFree(h->d_scal);
+    cudaFree(h->d_block);
+    cudaFree(h->d_ticket);
+    cudaFree(h->d_coef);
+    cudaFree(h->d_gram);
+    cudaFree(h->d_gram_part);
+    if (h->h_gram) cudaFreeHost(h->h_gram);
+    if (h->h_scal) cudaFreeHost(h->h_scal);
+    for (void* p : h->st) cudaFree(p);
+    for (auto& pr : h->pending) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+    for (auto e : h->event_pool) cudaEventDestroy(e);
+    cudaGetLastError();
+    delete h;
+    return LM_OK;
+}
+
+const char* lm_last_error(const lm_solver* h) { return h ? h->err.c_str() : "null handle"; }
+
+int lm_set_max_iter(lm_solver* h, int max_iter)
+{
+    if (!h) return LM_E_NULL;
+    if (max_iter < 1 || max_iter > 1000) return fail(h, LM_E_INVALID, "max_iter must be in [1, 1000]");
+    h->max_iter = max_iter;
+    return LM_OK;
+}
+
+int lm_last_iterations(const lm_solver* h) { return h ? h->last_iters : -1; }
+
+int lm_set_positions(lm_solver* h, const void* pos, void* stream)
+{
+    if (!h) return LM_E_NULL;
+    h->err.clear();
+    if (!pos) return fail(h, LM_E_NULL, "pos is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    return h->precision == LM_F32 ? set_positions_t<float>(h, pos, st) : set_positions_t<double>(h, pos, st);
+}
+
+int lm_mdot_batch(lm_solver* h, int nrhs, const void* forces, const void* torques, void* lin_out, void* ang_out, void* stream)
+{
+    int rc = check_io(h, forces, torques, lin_out, ang_out, true);
+    if (rc != LM_OK) return rc;
+    if (nrhs < 1) return fail(h, LM_E_INVALID, "nrhs must be >= 1");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (h->precision == LM_F32) return apply_batch<float>(h, nrhs, (const float*)forces, (const float*)torques, (float*)lin_out, (float*)ang_out, st);
+    return apply_batch<double>(h, nrhs, (const double*)forces, (const double*)torques, (double*)lin_out, (double*)ang_out, st);
+}
+
+int lm_mdot(lm_solver* h, const void* forces, const void* torques, void* lin_out, void* ang_out, void* stream)
+{
+    return lm_mdot_batch(h, 1, forces, torques, lin_out, ang_out, stream);
+}
+
+int lm_sqrt_mdot_w(lm_solver* h, const void* noise, double tol, void* lin_out, void* ang_out, int* iters_out, void* stream)
+{
+    int rc = check_io(h, noise, nullptr, lin_out, ang_out, false);
+    if (rc != LM_OK) return rc;
+    if (!noise) return fail(h, LM_E_NULL, "noise is NULL");
+    if (!(tol > 0.0) || !std::isfinite(tol)) return fail(h, LM_E_INVALID, "tol must be > 0");
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = h->precision == LM_F32 ? lanczos_device<float>(h, (const float*)noise, tol, (float*)lin_out, (float*)ang_out, 1.0, 0, st)
+                                : lanczos_device<double>(h, (const double*)noise, tol, (double*)lin_out, (double*)ang_out, 1.0, 0, st);
+    if (iters_out) *iters_out = h->last_iters;
+    return rc;
+}
+
+int lm_hydrodynamic_velocities(lm_solver* h, const void* forces, const void* torques, const void* noise, double noise_prefactor, double tol,
+                               void* lin_out, void* ang_out, void* stream)
+{
+    int rc = check_io(h, forces, torques, lin_out, ang_out, noise == nullptr);
+    if (rc != LM_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool have_det = forces || torques;
+    if (have_det) {
+        rc = lm_mdot_batch(h, 1, forces, torques, lin_out, ang_out, stream);
+        if (rc != LM_OK) return rc;
+    }
+    if (!noise) return LM_OK;
+    if (!(tol > 0.0) || !std::isfinite(tol)) return fail(h, LM_E_INVALID, "tol must be > 0");
+    const int acc = have_det ? 1 : 0;
+    return h->precision == LM_F32
+               ? lanczos_device<float>(h, (const float*)noise, tol, (float*)lin_out, (float*)ang_out, noise_prefactor, acc, st)
+               : lanczos_device<double>(h, (const double*)noise, tol, (double*)lin_out, (double*)ang_out, noise_prefactor, acc, st);
+}
+
+// ---------------------------------------------------------------- host-pointer variants
+int lm_set_positions_host(lm_solver* h, const void* pos, void* stream)
+{
+    if (!h) return LM_E_NULL;
+    h->err.clear();
+    if (!pos) return fail(h, LM_E_NULL, "pos is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    void* d = nullptr;
+    int rc = stage_in(h, 0, pos, (size_t)3 * h->N * esize(h), st, &d);
+    if (rc != LM_OK) return rc;
+    rc = lm_set_positions(h, d, stream);
+    if (rc != LM_OK) return rc;
+    LM_CUDA(h, cudaStreamSynchronize(st));
+    return LM_OK;
+}
+
+int lm_mdot_batch_host(lm_solver* h, int nrhs, const void* forces, const void* torques, void* lin_out, void* ang_out, void* stream)
+{
+    int rc = check_io(h, forces, torques, lin_out, ang_out, true);
+    if (rc != LM_OK) return rc;
+    if (nrhs < 1) return fail(h, LM_E_INVALID, "nrhs must be >= 1");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)nrhs * 3 * h->N * esize(h);
+    void *df, *dt, *dl, *da;
+    if ((rc = stage_in(h, 1, forces, bytes, st, &df)) != LM_OK) return rc;
+    if ((rc = stage_in(h, 2, torques, bytes, st, &dt)) != LM_OK) return rc;
+    if ((rc = stage_out_alloc(h, 4, lin_out, bytes, &dl)) != LM_OK) return rc;
+    if ((rc = stage_out_alloc(h, 5, ang_out, bytes, &da)) != LM_OK) return rc;
+    if ((rc = lm_mdot_batch(h, nrhs, df, dt, dl, da, stream)) != LM_OK) return rc;
+    LM_CUDA(h, cudaMemcpyAsync(lin_out, dl, bytes, cudaMemcpyDeviceToHost, st));
+    if (ang_out) LM_CUDA(h, cudaMemcpyAsync(ang_out, da, bytes, cudaMemcpyDeviceToHost, st));
+    LM_CUDA(h, cudaStreamSynchronize(st));
+    return LM_OK;
+}
+
+int lm_mdot_host(lm_solver* h, const void* forces, const void* torques, void* lin_out, void* ang_out, void* stream)
+{
+    return lm_mdot_batch_host(h, 1, forces, torques, lin_out, ang_out, stream);
+}
+
+int lm_hydrodynamic_velocities_host(lm_solver* h, const void* forces, const void* torques, const void* noise, double noise_prefactor,
+                                    double tol, void* lin_out, void* ang_out, void* stream)
+{
+    int rc = check_io(h, forces, torques, lin_out, ang_out, noise == nullptr);
+    if (rc != LM_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)3 * h->N * esize(h);
+    void *df, *dt, *dn, *dl, *da;
+    if ((rc = stage_in(h, 1, forces, bytes, st, &df)) != LM_OK) return rc;
+    if ((rc = stage_in(h, 2, torques, bytes, st, &dt)) != LM_OK) return rc;
+    if ((rc = stage_in(h, 3, noise, (size_t)dof_of(h) * esize(h), st, &dn)) != LM_OK) return rc;
+    if ((rc = stage_out_alloc(h, 4, lin_out, bytes, &dl)) != LM_OK) return rc;
+    if ((rc = stage_out_alloc(h, 5, ang_out, bytes, &da)) != LM_OK) return rc;
+    rc = lm_hydrodynamic_velocities(h, df, dt, dn, noise_prefactor, tol, dl, da, stream);
+    if (rc != LM_OK && rc != LM_E_NOCONV) return rc;
+    LM_CUDA(h, cudaMemcpyAsync(lin_out, dl, bytes, cudaMemcpyDeviceToHost, st));
+    if (ang_out) LM_CUDA(h, cudaMemcpyAsync(ang_out, da, bytes, cudaMemcpyDeviceToHost, st));
+    LM_CUDA(h, cudaStreamSynchronize(st));
+    return rc;
+}
+
+int lm_sqrt_mdot_w_host(lm_solver* h, const void* noise, double tol, void* lin_out, void* ang_out, int* iters_out, void* stream)
+{
+    if (h && !noise) { h->err.clear(); return fail(h, LM_E_NULL, "noise is NULL"); }
+    const int rc = lm_hydrodynamic_velocities_host(h, nullptr, nullptr, noise, 1.0, tol, lin_out, ang_out, stream);
+    if (iters_out && h) *iters_out = h->last_iters;
+    return rc;
+}
+
+// ---------------------------------------------------------------- stats / introspection
+int lm_set_profiling(lm_solver* h, int on)
+{
+    if (!h) return LM_E_NULL;
+    h->profiling = on != 0;
+    return LM_OK;
+}
+
+static int drain_events(lm_solver* h)
+{
+    for (auto& pr : h->pending) {
+        LM_CUDA(h, cudaEventSynchronize(pr.second));
+        float ms = 0.f;
+        LM_CUDA(h, cudaEventElapsedTime(&ms, pr.first, pr.second));
+        h->pair_ms += ms;
+        h->event_pool.push_back(pr.first);
+        h->event_pool.push_back(pr.second);
+    }
+    h->pending.clear();
+    return LM_OK;
+}
+
+int lm_reset_stats(lm_solver* h)
+{
+    if (!h) return LM_E_NULL;
+    const int rc = drain_events(h);
+    h->n_pair = h->n_aux = 0;
+    h->pairs = h->pair_ms = 0.0;
+    return rc;
+}
+
+int lm_get_stats(lm_solver* h, int64_t* pair_kernel_launches, int64_t* aux_launches, double* pair_kernel_ms, double* pairs)
+{
+    if (!h) return LM_E_NULL;
+    const int rc = drain_events(h);
+    if (pair_kernel_launches) *pair_kernel_launches = h->n_pair;
+    if (aux_launches) *aux_launches = h->n_aux;
+    if (pair_kernel_ms) *pair_kernel_ms = h->pair_ms;
+    if (pairs) *pairs = h->pairs;
+    return rc;
+}
+
+int lm_pair_launch_config(lm_solver* h, int nrhs, int* i_tiles, int* j_splits, int* block, int* targets_per_thread, int* smem_bytes)
+{
+    if (!h) return LM_E_NULL;
+    LaunchPlan plan;
+    int blk = 0, tpt = 0, smem = 0;
+    if (h->precision == LM_F32) {
+        plan = choose_plan<float>(h, nrhs);
+        if (plan.variant >= 0) { blk = h->vf[plan.variant].block; tpt = h->vf[plan.variant].tpt; smem = h->vf[plan.variant].smem; }
+    } else {
+        plan = choose_plan<double>(h, nrhs);
+        if (plan.variant >= 0) { blk = h->vd[plan.variant].block; tpt = h->vd[plan.variant].tpt; smem = h->vd[plan.variant].smem; }
+    }
+    if (plan.variant < 0) return fail(h, LM_E_INVALID, "no pair-kernel variant for this nrhs (use 1, 2 or 4; angular: 1 or 2)");
+    if (i_tiles) *i_tiles = plan.i_tiles;
+    if (j_splits) *j_splits = plan.j_splits;
+    if (block) *block = blk;
+    if (targets_per_thread) *targets_per_thread = tpt;
+    if (smem_bytes) *smem_bytes = smem;
+    return LM_OK;
+}
+
+int lm_host_tridiag_sqrt_e1(int k, const double* alpha, const double* beta, double* c_out)
+{
+    if (k < 1) return LM_E_INVALID;
+    if (!alpha || !c_out || (k > 1 && !beta)) return LM_E_NULL;
+    return tridiag_sqrt_e1(k, alpha, beta, c_out) ? LM_OK : LM_E_NOCONV;
+}
+
+int lm_probe_fma_peak(int precision, double seconds, double* lane_ops_per_s)
+{
+    if (!lane_ops_per_s) return LM_E_NULL;
+    if (precision != LM_F32 && precision != LM_F64) return LM_E_INVALID;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return LM_E_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return LM_E_CUDA;
+    const int threads = 256, grid = sms * 8, iters = 8192;
+    void* buf = nullptr;
+    if (cudaMalloc(&buf, (size_t)grid * threads * 8) != cudaSuccess) return LM_E_CUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    auto launch = [&]() {
+        if (precision == LM_F32) probe_ffma2_kernel<<<grid, threads>>>((float*)buf, 1.0001f, 0.5f, iters);
+        else probe_dfma_kernel<<<grid, threads>>>((double*)buf, 1.0001, 0.5, iters);
+    };
+    const double ops_per_launch = (double)grid * threads * iters * (precision == LM_F32 ? 16.0 : 8.0);
+    launch();
+    launch();
+    cudaDeviceSynchronize();
+    double best = 0.0, elapsed = 0.0;
+    int reps = 0;
+    while (elapsed < seconds * 1e3 || reps < 3) {
+        cudaEventRecord(e0);
+        launch();
+        cudaEventRecord(e1);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        elapsed += ms;
+        best = std::max(best, ops_per_launch / (ms * 1e-3));
+        if (++reps > 100000) break;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (cudaGetLastError() != cudaSuccess) return LM_E_CUDA;
+    *lane_ops_per_s = best;
+    return LM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,217 @@
+// vector_kernels.cuh -- the O(N) kernels around the pair kernel: packing to structure-of-arrays,
+// split-j reduction, and the Lanczos vector operations.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "lm_common.cuh"
+
+namespace lm {
+
+constexpr int VEC_BLOCK = 256;       // threads per block of every kernel in this file
+constexpr int RED_MAX_BLOCKS = 1024; // upper bound on the grid of the reduction kernels
+
+// a1: interleaved positions (3N) -> x | y | z, each npad long, ghosts zero.
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) pack_positions_kernel(const T* __restrict__ pos, int64_t N, int64_t npad, T* __restrict__ soa)
+{
+    const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
+    if (i >= npad) return;
+    T x = T(0), y = T(0), z = T(0);
+    if (i < N) { x = pos[3 * i]; y = pos[3 * i + 1]; z = pos[3 * i + 2]; }
+    soa[i] = x;
+    soa[npad + i] = y;
+    soa[2 * npad + i] = z;
+}
+
+// a2: right-hand sides -> [nrhs*NC][npad] component arrays (NC = 3: Fx Fy Fz; NC = 6: + Tx Ty Tz),
+// ghosts zero; a null force / torque pointer means zeros.
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) pack_rhs_kernel(RhsIn<T> in, int nrhs, int nc, int64_t N, int64_t npad, T* __restrict__ soa)
+{
+    const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
+    if (i >= npad) return;
+    for (int q = 0; q < nrhs; ++q) {
+        T v[6] = {T(0), T(0), T(0), T(0), T(0), T(0)};
+        if (i < N) {
+            if (in.f[q]) { v[0] = in.f[q][3 * i]; v[1] = in.f[q][3 * i + 1]; v[2] = in.f[q][3 * i + 2]; }
+            if (nc == 6 && in.t[q]) { v[3] = in.t[q][3 * i]; v[4] = in.t[q][3 * i + 1]; v[5] = in.t[q][3 * i + 2]; }
+        }
+        for (int k = 0; k < nc; ++k) soa[(size_t)(q * nc + k) * npad + i] = v[k];
+    }
+}
+
+// a6: sum the j-split partials in a fixed order (deterministic) and write interleaved outputs.
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) reduce_partials_kernel(const T* __restrict__ partial, int splits, int nrhs, int nc, int64_t N,
+                                                                    int64_t npad, RhsOut<T> out)
+{
+    const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
+    if (i >= N) return;
+    const size_t stride = (size_t)nrhs * nc * npad;
+    for (int q = 0; q < nrhs; ++q) {
+        for (int k = 0; k < nc; ++k) {
+            const T* p = partial + (size_t)(q * nc + k) * npad + i;
+            T s = T(0);
+            for (int sidx = 0; sidx < splits; ++sidx) s += p[sidx * stride];
+            if (k < 3) out.lin[q][3 * i + k] = s;
+            else       out.ang[q][3 * i + (k - 3)] = s;
+        }
+    }
+}
+
+// ---------------------------------------------------------------- Lanczos vector operations (a7)
+// Reductions: warp shuffles -> one fp64 partial per block -> the last block to finish (ticket)
+// adds the block partials in index order, so the result is deterministic for a given grid.
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ void block_reduce_to_scalar(double v, double* block_partials, unsigned int* ticket, double* result)
+{
+    __shared__ double warp_part[VEC_BLOCK / 32];
+    __shared__ bool is_last;
+    v = warp_sum(v);
+    if ((threadIdx.x & 31) == 0) warp_part[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < VEC_BLOCK / 32; ++w) s += warp_part[w];
+        block_partials[blockIdx.x] = s;
+        __threadfence();
+        const unsigned int t = atomicAdd(ticket, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last && threadIdx.x < 32) {
+        __threadfence();
+        double s = 0.0;
+        for (unsigned int b = threadIdx.x; b < gridDim.x; b += 32) s += ((volatile double*)block_partials)[b];
+        s = warp_sum(s);
+        if (threadIdx.x == 0) { *result = s; *ticket = 0u; }
+    }
+}
+
+// result = sum_i x_i^2          (|z|^2 of the noise vector)
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) sumsq_kernel(const T* __restrict__ x, int64_t n, double* block_partials, unsigned int* ticket,
+                                                          double* result)
+{
+    double s = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * VEC_BLOCK) {
+        const double v = (double)x[i];
+        s = fma(v, v, s);
+    }
+    block_reduce_to_scalar(s, block_partials, ticket, result);
+}
+
+// v_out = x / sqrt(*sumsq)     (v_1 = z/|z| and v_{k+1} = w/beta_k)
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) scale_by_inv_norm_kernel(const T* __restrict__ x, int64_t n, const double* sumsq, T* __restrict__ v_out)
+{
+    const double nrm = sqrt(*sumsq);
+    const double inv = nrm > 0.0 ? 1.0 / nrm : 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * VEC_BLOCK)
+        v_out[i] = (T)((double)x[i] * inv);
+}
+
+// w -= sqrt(*beta_prev_sq) * v_prev  (skipped when v_prev == null);  *alpha = w . v
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) lanczos_alpha_kernel(T* __restrict__ w, const T* __restrict__ v, const T* __restrict__ v_prev,
+                                                                  const double* beta_prev_sq, int64_t n, double* block_partials,
+                                                                  unsigned int* ticket, double* alpha)
+{
+    const double bp = v_prev ? sqrt(*beta_prev_sq) : 0.0;
+    double s = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * VEC_BLOCK) {
+        double wi = (double)w[i];
+        if (v_prev) {
+            wi = fma(-bp, (double)v_prev[i], wi);
+            w[i] = (T)wi;
+            wi = (double)w[i];          // the dot product sees the stored (rounded) value
+        }
+        s = fma(wi, (double)v[i], s);
+    }
+    block_reduce_to_scalar(s, block_partials, ticket, alpha);
+}
+
+// w -= *alpha * v;  *beta_sq = |w|^2
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__ w, const T* __restrict__ v, const double* alpha, int64_t n,
+                                                                 double* block_partials, unsigned int* ticket, double* beta_sq)
+{
+    const double a = *alpha;
+    double s = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * VEC_BLOCK) {
+        const T wi = (T)fma(-a, (double)v[i], (double)w[i]);
+        w[i] = wi;
+        s = fma((double)wi, (double)wi, s);
+    }
+    block_reduce_to_scalar(s, block_partials, ticket, beta_sq);
+}
+
+// Gram column for the stopping test (a9): g[j] = V[j] . V[k], j = 0..k.  Lanczos without
+// re-orthogonalisation loses orthogonality of V, so |y_k - y_{k-1}| = |z| |V_k delta| is evaluated as
+// sqrt(delta^T G delta) with the true Gram matrix G = V^T V instead of assuming G = I.
+// Block b owns the contiguous index range [b*chunk, (b+1)*chunk); partials are [j][block].
+constexpr int GRAM_MAX_BLOCKS = 128;
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) gram_column_kernel(const T* __restrict__ V, int64_t dof, int k, int64_t chunk, double* partials,
+                                                                unsigned int* ticket, double* g)
+{
+    __shared__ double warp_part[VEC_BLOCK / 32];
+    __shared__ bool is_last;
+    const int64_t lo_i = (int64_t)blockIdx.x * chunk, hi_i = min(lo_i + chunk, dof);
+    const T* vk = V + (size_t)k * dof;
+    for (int j = 0; j <= k; ++j) {
+        const T* vj = V + (size_t)j * dof;
+        double s = 0.0;
+        for (int64_t i = lo_i + threadIdx.x; i < hi_i; i += VEC_BLOCK) s = fma((double)vj[i], (double)vk[i], s);
+        s = warp_sum(s);
+        if ((threadIdx.x & 31) == 0) warp_part[threadIdx.x >> 5] = s;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+#pragma unroll
+            for (int w = 0; w < VEC_BLOCK / 32; ++w) t += warp_part[w];
+            partials[(size_t)j * gridDim.x + blockIdx.x] = t;
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        __threadfence();
+        is_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        for (int j = threadIdx.x; j <= k; j += VEC_BLOCK) {
+            double t = 0.0;
+            for (unsigned int b = 0; b < gridDim.x; ++b) t += ((volatile double*)partials)[(size_t)j * gridDim.x + b];
+            g[j] = t;
+        }
+        if (threadIdx.x == 0) *ticket = 0u;
+    }
+}
+
+// a10: y = scale * sum_{m<k} coef[m] V[m]  split into the linear (first 3N) and angular (last 3N)
+// outputs; accumulate != 0 adds to what is already there (lm_hydrodynamic_velocities).
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) lanczos_combine_kernel(const T* __restrict__ V, int64_t dof, int k, const double* __restrict__ coef,
+                                                                    double scale, int accumulate, int64_t n_lin, T* __restrict__ out_lin,
+                                                                    T* __restrict__ out_ang)
+{
+    for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < dof; i += (int64_t)gridDim.x * VEC_BLOCK) {
+        double s = 0.0;
+        for (int m = 0; m < k; ++m) s = fma(coef[m], (double)V[(size_t)m * dof + i], s);
+        s *= scale;
+        T* dst = i < n_lin ? out_lin + i : out_ang + (i - n_lin);
+        *dst = accumulate ? (T)((double)*dst + s) : (T)s;
+    }
+}
+
+}  // namespace lm
