@@ -206,13 +206,10 @@ def main():
 
     import paper_2510_02135_b200 as lm
 
-    data = workloads.generate(args.config, args.N)
-    cfg, N = data["cfg"], data["N"]
-    if world > 1 and rank > 0:      # independent replicas: other ranks draw their own inputs of the same shape
-        cfg_r = workloads.dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
-        workloads.CONFIGS[cfg.index] = cfg_r
-        data = workloads.generate(args.config, args.N)
-        workloads.CONFIGS[cfg.index] = cfg
+    from paper_2510_02135_b200 import multi
+    cfg = workloads.CONFIGS[args.config]
+    data = workloads.generate(args.config, args.N, seed=multi.replica_seed(cfg.seed, rank))   # independent replicas
+    N = data["N"]
     f64 = cfg.precision == "f64"
     tdt = torch.float64 if f64 else torch.float32
     dof = (6 if cfg.angular else 3) * N
@@ -306,18 +303,11 @@ def main():
         e2e_ms, _, _ = timed(step_host, args.steps)
         e2e_stats = solver.get_stats()
 
-    # ---- max over ranks
-    if world > 1:
-        t = torch.tensor([ms_total, e2e_ms or 0.0], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, e2e_max = float(t[0]), float(t[1])
-        e2e_ms = e2e_max if e2e_ms is not None else None
-        p = torch.tensor([stats["pairs"], e2e_stats["pairs"] if e2e_ms is not None else 0.0], dtype=torch.float64, device="cuda")
-        dist.all_reduce(p, op=dist.ReduceOp.SUM)
-        pairs_all, e2e_pairs_all = float(p[0]), float(p[1])
-    else:
-        pairs_all = stats["pairs"]
-        e2e_pairs_all = e2e_stats["pairs"] if e2e_ms is not None else 0.0
+    # ---- max over ranks of the device time, sum over ranks of the pairs (replicas only)
+    ms_total, pairs_all = multi.aggregate_over_ranks(ms_total, stats["pairs"], device="cuda")
+    e2e_pairs_all = 0.0
+    if e2e_ms is not None:
+        e2e_ms, e2e_pairs_all = multi.aggregate_over_ranks(e2e_ms, e2e_stats["pairs"], device="cuda")
 
     if rank != 0:
         if world > 1:

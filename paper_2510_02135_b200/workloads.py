@@ -76,15 +76,15 @@ def positions(cfg: Config, rng: np.random.Generator, N: int | None = None) -> np
     raise ValueError(cfg.geometry)
 
 
-def generate(index: int, N: int | None = None) -> dict:
-    """All arrays of config ``index`` (optionally at a reduced N), already cast to its precision.
+def generate(index: int, N: int | None = None, seed: int | None = None) -> dict:
+    """All arrays of config ``index`` (optionally at a reduced N, or with another seed for a replica), already cast to its precision.
 
     Keys: cfg, N, pos (N,3), forces (nrhs,N,3) or (N,3), torques (N,3) or None, noise (dof,) or None.
     """
     cfg = CONFIGS[index]
     N = cfg.N if N is None else N
     dt = np_dtype(cfg.precision)
-    rng = np.random.default_rng(cfg.seed)
+    rng = np.random.default_rng(cfg.seed if seed is None else seed)
     pos = positions(cfg, rng, N)
     if cfg.nrhs > 1:
         forces = rng.standard_normal((cfg.nrhs, N, 3))
