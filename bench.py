@@ -44,10 +44,11 @@ UNIT = "Gpairs/s"
 # Algorithmic FP-pipe lane-operations and flops per ordered pair (counted from the
 # algebra, never from emitted instructions).  key: (angular, nrhs)
 def work_per_pair(angular: bool, nrhs: int, f64: bool):
+    """Minimal algebra of a far-field pair (r >= 2a; an overlapping pair needs fewer), DESIGN.md sec. 7."""
     if angular:
-        instr, fma = 27 + 32 * nrhs, 9 + 28 * nrhs
+        instr, fma = 19 + 32 * nrhs, 5 + 28 * nrhs
     else:
-        instr, fma = 15 + 10 * nrhs, 5 + 8 * nrhs
+        instr, fma = 12 + 10 * nrhs, 5 + 8 * nrhs
     if f64:
         instr, fma = instr + 5, fma + 3      # fp64 refinement of the rsqrt seed
     flops = instr + fma + 1                  # FMA = 2 flops, + the rsqrt

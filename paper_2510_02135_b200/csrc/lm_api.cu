@@ -11,6 +11,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "../../include/lm.h"
@@ -21,12 +22,13 @@
 namespace lm {
 
 // ---------------------------------------------------------------- pair-kernel variants
-// LARGE: 256 threads x 2 targets, 512-source tiles.  SMALL: 128 x 1, 128-source tiles (fills
-// 148 SMs when N is small, SURVEY.md sec. 7 "Small N").  npad is a multiple of NPAD_QUANTUM so
-// that either variant tiles it exactly.
+// LARGE: 256 threads x TPT targets (TPT/2 packed pairs per thread), 512-source tiles.  SMALL: 64 x 2,
+// 64-source tiles (fills 148 SMs when N is small, SURVEY.md sec. 7 "Small N").  npad is a multiple
+// of NPAD_QUANTUM so that either tile size divides it.  SUB = sources per overlap-vote chunk.
 constexpr int NPAD_QUANTUM = 512;
-constexpr int L_BLOCK = 256, L_TPT = 2, L_TJ = 512, L_STAGES = 2;
-constexpr int S_BLOCK = 128, S_TPT = 1, S_TJ = 128, S_STAGES = 2;
+constexpr int L_BLOCK = 256, L_TJ = 512, L_STAGES = 2, L_SUB = 32;
+constexpr int S_BLOCK = 64, S_TPT = 2, S_TJ = 64, S_STAGES = 2, S_SUB = 32;
+constexpr int64_t MAX_SOURCES_PER_CTA = 262144;   // bounds the top level of the two-level fp32 summation
 
 template <typename T> struct Variant {
     void (*kernel)(const PairParams<T>);
@@ -35,31 +37,31 @@ template <typename T> struct Variant {
     double efficiency;    // relative per-pair throughput used by the launch chooser
 };
 
-template <typename T, int NRHS, bool ANG, int MINB> Variant<T> make_large()
+template <typename T, int NRHS, bool ANG, int TPT, int MINB> Variant<T> make_large()
 {
-    using Tr = PairKernelTraits<T, NRHS, ANG, L_TPT, L_BLOCK, L_TJ, L_STAGES>;
-    return {rpy_pair_kernel<T, NRHS, ANG, L_TPT, L_BLOCK, L_TJ, L_STAGES, MINB>, NRHS, ANG, L_BLOCK, L_TPT, L_TJ, Tr::SMEM_BYTES, 0, 1.0};
+    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, L_SUB>;
+    return {rpy_pair_kernel<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, L_SUB, MINB>, NRHS, ANG, L_BLOCK, TPT, L_TJ, Tr::SMEM_BYTES, 0, 1.0};
 }
 template <typename T, int NRHS, bool ANG, int MINB> Variant<T> make_small()
 {
-    using Tr = PairKernelTraits<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES>;
-    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, MINB>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, Tr::SMEM_BYTES, 0, 0.85};
+    using Tr = PairKernelTraits<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, S_SUB>;
+    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, S_SUB, MINB>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, Tr::SMEM_BYTES, 0, 0.8};
 }
 
 template <typename T> std::vector<Variant<T>> build_variants();
 template <> std::vector<Variant<float>> build_variants<float>()
 {
-    return {make_large<float, 1, false, 2>(), make_large<float, 2, false, 2>(), make_large<float, 4, false, 1>(),
-            make_large<float, 1, true, 2>(),  make_large<float, 2, true, 1>(),
-            make_small<float, 1, false, 3>(), make_small<float, 2, false, 3>(), make_small<float, 4, false, 3>(),
-            make_small<float, 1, true, 3>(),  make_small<float, 2, true, 3>()};
+    return {make_large<float, 1, false, 4, 2>(), make_large<float, 2, false, 4, 1>(), make_large<float, 4, false, 2, 2>(),
+            make_large<float, 1, true, 2, 2>(),  make_large<float, 2, true, 2, 1>(),
+            make_small<float, 1, false, 8>(), make_small<float, 2, false, 8>(), make_small<float, 4, false, 6>(),
+            make_small<float, 1, true, 8>(),  make_small<float, 2, true, 6>()};
 }
 template <> std::vector<Variant<double>> build_variants<double>()
 {
-    return {make_large<double, 1, false, 2>(), make_large<double, 2, false, 1>(), make_large<double, 4, false, 1>(),
-            make_large<double, 1, true, 1>(),  make_large<double, 2, true, 1>(),
-            make_small<double, 1, false, 3>(), make_small<double, 2, false, 3>(), make_small<double, 4, false, 2>(),
-            make_small<double, 1, true, 3>(),  make_small<double, 2, true, 2>()};
+    return {make_large<double, 1, false, 2, 2>(), make_large<double, 2, false, 2, 1>(), make_large<double, 4, false, 2, 1>(),
+            make_large<double, 1, true, 2, 1>(),  make_large<double, 2, true, 2, 1>(),
+            make_small<double, 1, false, 8>(), make_small<double, 2, false, 6>(), make_small<double, 4, false, 4>(),
+            make_small<double, 1, true, 6>(),  make_small<double, 2, true, 4>()};
 }
 
 struct LaunchPlan {
@@ -211,7 +213,8 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
         const int n_tiles = (int)(h->npad / v.tj);
         const int64_t slots = (int64_t)h->sm_count * v.ctas_per_sm;
         const int max_splits = std::min(n_tiles, 128);
-        for (int s = 1; s <= max_splits; ++s) {
+        const int min_splits = (int)std::min<int64_t>(max_splits, (h->npad + MAX_SOURCES_PER_CTA - 1) / MAX_SOURCES_PER_CTA);
+        for (int s = min_splits; s <= max_splits; ++s) {
             const int tps = (n_tiles + s - 1) / s;
             const int s_eff = (n_tiles + tps - 1) / tps;   // splits actually needed with that tile count
             if (s_eff != s) continue;

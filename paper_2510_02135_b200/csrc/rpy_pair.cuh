@@ -7,23 +7,32 @@
 //   U_i = sum_j [ f_tt F_j + g_tt (rhat.F_j) rhat + g_c (T_j x rhat) ]
 //   W_i = sum_j [ f_rr T_j + g_rr (rhat.T_j) rhat + g_c (F_j x rhat) ]
 //
-// Design (B200-first):
-//   * one thread owns TPT targets; all 32 lanes of a warp walk the SAME sources, so every
-//     shared-memory read is a broadcast LDS.128 (4 fp32 / 2 fp64 sources per instruction);
+// Design (B200-first, DESIGN.md sec. 5 and the machine model of sec. 7):
+//   * one thread owns TPT targets held as TPT/2 PACKED TARGET PAIRS; all 32 lanes of a warp walk
+//     the SAME sources, so every shared-memory read is a broadcast LDS.128 (4 fp32 / 2 fp64
+//     sources per instruction) and every source value enters the arithmetic as a scalar-broadcast
+//     operand (FFMA2 Rpair, R.F32, Rpair): at most two 64-bit register operands per packed
+//     instruction, which is what the sm_100 register file can feed at the FMA pipe's rate;
 //   * sources are staged as structure-of-arrays tiles by 1-D TMA bulk copies
 //     (cp.async.bulk.shared::cluster.global, SASS UBLKCP) completing on an mbarrier,
-//     double/triple buffered -- no thread issues a global load in the main loop;
-//   * fp32 arithmetic is packed two sources per instruction (FFMA2 / FMUL2 / FADD2, the
-//     sm_100 f32x2 forms): the FMA pipe sees the same lane-ops, but the issue port is freed
-//     for the MUFU, select and LDS instructions of the same pair;
-//   * 1/r from MUFU.RSQ (fp32) or MUFU.RSQ64H + one cubically convergent correction (fp64);
-//   * both branches are evaluated and selected per lane (FSEL) -- no divergence; r = 0 is
-//     made safe by a tiny additive floor inside the r^2 FMA chain (no extra instruction);
-//   * two-level accumulation: a packed per-tile accumulator is flushed into a per-thread
-//     main accumulator at every tile end (keeps fp32 summation error ~ eps*sqrt(tile)).
+//     double buffered -- no thread issues a global load in the main loop;
+//   * fp32 arithmetic is packed two targets per instruction (FFMA2 / FMUL2 / FADD2, the
+//     sm_100 f32x2 forms);  1/r from MUFU.RSQ (fp32) or MUFU.RSQ64H + one cubically convergent
+//     correction (fp64);
+//   * overlap (r < 2a) / far-field select without divergence and without paying for it where
+//     no pair overlaps: sources are walked in chunks of SUB; a chunk is first evaluated with the
+//     FAR-FIELD formulas only while a predicate collects (r^2 < 4a^2) over all its pairs; one
+//     warp vote per chunk decides whether the chunk is accepted or re-evaluated with the
+//     GENERAL body (both branches + per-lane FSEL).  Dense regions lock the warp onto the
+//     general body, so the worst case costs what the plain select kernel costs;
+//   * r = 0 is made safe by a tiny additive floor inside the r^2 FMA chain (no extra instruction);
+//   * two-level accumulation: the per-chunk packed accumulator is flushed into a per-thread
+//     total at every chunk end (keeps the fp32 summation error ~ eps*(sqrt(SUB)+sqrt(N/SUB))).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include <type_traits>
 
 #include "lm_common.cuh"
 
@@ -49,7 +58,11 @@ __device__ __forceinline__ P2<float> add2(P2<float> a, P2<float> b) { return {__
 __device__ __forceinline__ P2<double> fma2(P2<double> a, P2<double> b, P2<double> c) { return {fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)}; }
 __device__ __forceinline__ P2<double> mul2(P2<double> a, P2<double> b) { return {a.x * b.x, a.y * b.y}; }
 __device__ __forceinline__ P2<double> add2(P2<double> a, P2<double> b) { return {a.x + b.x, a.y + b.y}; }
-template <typename T> __device__ __forceinline__ P2<T> neg2(P2<T> a) { return mk2(-lo(a), -hi(a)); }
+// scalar-broadcast forms (the scalar is a source quantity or a constant, identical for both targets)
+template <typename T> __device__ __forceinline__ P2<T> fma2(P2<T> a, T s, P2<T> c) { return fma2(a, splat(s), c); }
+template <typename T> __device__ __forceinline__ P2<T> fma2(P2<T> a, T s, T c) { return fma2(a, splat(s), splat(c)); }
+template <typename T> __device__ __forceinline__ P2<T> mul2(P2<T> a, T s) { return mul2(a, splat(s)); }
+template <typename T> __device__ __forceinline__ P2<T> add2(P2<T> a, T s) { return add2(a, splat(s)); }
 
 // 1/sqrt(x): fp32 = one MUFU.RSQ per lane (rel. error ~2^-22, far inside the 2e-5 gate).
 __device__ __forceinline__ float rsqrt1(float x)
@@ -97,7 +110,7 @@ template <typename T> struct PairParams {
     RhsOut<T> out;              // j_splits == 1: per right-hand side, 3N interleaved each
     T* __restrict__ partial;    // j_splits  > 1: [j_splits][nrhs*NC][npad]
     int64_t N;
-    int64_t npad;               // multiple of TJ and of BLOCK*TPT
+    int64_t npad;               // multiple of every TJ in use
     int tiles_per_split;        // j-tiles handled by one CTA (last split may get fewer)
     int n_tiles;                // npad / TJ
     PairConsts<T> c;
@@ -131,30 +144,36 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  : "memory");
 }
 
-// ---------------------------------------------------------------- one packed pair (2 sources) vs one target
-template <typename T, int NRHS, bool ANG>
-__device__ __forceinline__ void pair_eval(const PairConsts<T>& c, T nxi, T nyi, T nzi, P2<T> xj, P2<T> yj, P2<T> zj,
-                                          const P2<T> (&V)[NRHS * (ANG ? 6 : 3)], P2<T> (&acc)[NRHS * (ANG ? 6 : 3)])
+// ---------------------------------------------------------------- one source vs one packed target pair
+// FAR == true : far-field formulas only; `near` collects (r^2 < 4a^2) -- the caller discards the
+//               chunk if any lane of the warp saw an overlapping (or coincident) pair.
+// FAR == false: both branches, selected per lane.
+// (nx, ny, nz) = -x_i of the two targets; (xj, yj, zj), V[] = the source, warp-uniform scalars.
+template <typename T, int NRHS, bool ANG, bool FAR>
+__device__ __forceinline__ void pair_eval(const PairConsts<T>& c, P2<T> nx, P2<T> ny, P2<T> nz, T xj, T yj, T zj,
+                                          const T (&V)[NRHS * (ANG ? 6 : 3)], P2<T> (&acc)[NRHS * (ANG ? 6 : 3)], bool& near)
 {
     constexpr int NC = ANG ? 6 : 3;
-    const P2<T> dx = add2(xj, splat(nxi)), dy = add2(yj, splat(nyi)), dz = add2(zj, splat(nzi));
+    const P2<T> dx = add2(nx, xj), dy = add2(ny, yj), dz = add2(nz, zj);
     const P2<T> r2 = fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, splat(c.tiny))));
+    const bool nl = lo(r2) < c.four_a2, nh = hi(r2) < c.four_a2;
+    if constexpr (FAR) near = near || nl || nh;
     const P2<T> invr = rsqrt2(r2);
     const P2<T> u = mul2(invr, invr);
     const P2<T> w3 = mul2(invr, u);
-    const P2<T> r = mul2(r2, invr);
-    const bool nl = lo(r2) < c.four_a2, nh = hi(r2) < c.four_a2;
     // translation-translation scalars
-    const P2<T> f_far = mul2(invr, fma2(splat(c.C2), u, splat(c.C1)));
-    const P2<T> g_far = mul2(w3, fma2(splat(c.nC3), u, splat(c.C1)));
-    const P2<T> f_near = fma2(splat(c.nC5), r, splat(c.C4));
-    const P2<T> g_near = mul2(splat(c.C6), invr);
-    const P2<T> f = sel2(nl, nh, f_near, f_far);
-    const P2<T> g = sel2(nl, nh, g_near, g_far);
+    P2<T> f = mul2(invr, fma2(u, c.C2, c.C1));
+    P2<T> g = mul2(w3, fma2(u, c.nC3, c.C1));
+    P2<T> r;
+    if constexpr (!FAR) {
+        r = mul2(r2, invr);
+        f = sel2(nl, nh, fma2(r, c.nC5, c.C4), f);
+        g = sel2(nl, nh, mul2(invr, c.C6), g);
+    }
     if constexpr (!ANG) {
 #pragma unroll
         for (int q = 0; q < NRHS; ++q) {
-            const P2<T> Fx = V[q * NC + 0], Fy = V[q * NC + 1], Fz = V[q * NC + 2];
+            const T Fx = V[q * NC + 0], Fy = V[q * NC + 1], Fz = V[q * NC + 2];
             const P2<T> t = mul2(g, fma2(dz, Fz, fma2(dy, Fy, mul2(dx, Fx))));
             acc[q * NC + 0] = fma2(f, Fx, fma2(t, dx, acc[q * NC + 0]));
             acc[q * NC + 1] = fma2(f, Fy, fma2(t, dy, acc[q * NC + 1]));
@@ -162,58 +181,63 @@ __device__ __forceinline__ void pair_eval(const PairConsts<T>& c, T nxi, T nyi, 
         }
     } else {
         // rotation-rotation and coupling scalars
-        const P2<T> w5 = mul2(w3, u);
-        const P2<T> frr_far = mul2(splat(c.nC7), w3);
-        const P2<T> grr_far = mul2(splat(c.C7x3), w5);
-        const P2<T> h_far = mul2(splat(c.C1), w3);
-        const P2<T> frr_near = fma2(r, fma2(splat(c.K2), r2, splat(c.K1)), splat(c.C8));
-        const P2<T> grr_near = fma2(splat(c.K3), invr, mul2(splat(c.K4), r));
-        const P2<T> h_near = fma2(splat(c.K6), r, splat(c.K5));
-        const P2<T> frr = sel2(nl, nh, frr_near, frr_far);
-        const P2<T> grr = sel2(nl, nh, grr_near, grr_far);
-        const P2<T> h = sel2(nl, nh, h_near, h_far);
+        P2<T> frr = mul2(w3, c.nC7);
+        P2<T> grr = mul2(mul2(w3, u), c.C7x3);
+        P2<T> h = mul2(w3, c.C1);
+        if constexpr (!FAR) {
+            frr = sel2(nl, nh, fma2(r, fma2(r2, c.K2, c.K1), splat(c.C8)), frr);
+            grr = sel2(nl, nh, fma2(invr, c.K3, mul2(r, c.K4)), grr);
+            h = sel2(nl, nh, fma2(r, c.K6, c.K5), h);
+        }
         // with d = -r_vec:  g_c (T x rhat) = h (d x T),  g_c (F x rhat) = h (d x F)
         const P2<T> hx = mul2(h, dx), hy = mul2(h, dy), hz = mul2(h, dz);
-        const P2<T> nhx = neg2(hx), nhy = neg2(hy), nhz = neg2(hz);
 #pragma unroll
         for (int q = 0; q < NRHS; ++q) {
-            const P2<T> Fx = V[q * NC + 0], Fy = V[q * NC + 1], Fz = V[q * NC + 2];
-            const P2<T> Tx = V[q * NC + 3], Ty = V[q * NC + 4], Tz = V[q * NC + 5];
+            const T Fx = V[q * NC + 0], Fy = V[q * NC + 1], Fz = V[q * NC + 2];
+            const T Tx = V[q * NC + 3], Ty = V[q * NC + 4], Tz = V[q * NC + 5];
             const P2<T> t = mul2(g, fma2(dz, Fz, fma2(dy, Fy, mul2(dx, Fx))));
             const P2<T> s = mul2(grr, fma2(dz, Tz, fma2(dy, Ty, mul2(dx, Tx))));
-            // U += f F + t d + (hd) x T
-            acc[q * NC + 0] = fma2(nhz, Ty, fma2(hy, Tz, fma2(f, Fx, fma2(t, dx, acc[q * NC + 0]))));
-            acc[q * NC + 1] = fma2(nhx, Tz, fma2(hz, Tx, fma2(f, Fy, fma2(t, dy, acc[q * NC + 1]))));
-            acc[q * NC + 2] = fma2(nhy, Tx, fma2(hx, Ty, fma2(f, Fz, fma2(t, dz, acc[q * NC + 2]))));
+            // U += f F + t d + (hd) x T        ((hd) x T)_x = hy Tz - hz Ty
+            acc[q * NC + 0] = fma2(hz, -Ty, fma2(hy, Tz, fma2(f, Fx, fma2(t, dx, acc[q * NC + 0]))));
+            acc[q * NC + 1] = fma2(hx, -Tz, fma2(hz, Tx, fma2(f, Fy, fma2(t, dy, acc[q * NC + 1]))));
+            acc[q * NC + 2] = fma2(hy, -Tx, fma2(hx, Ty, fma2(f, Fz, fma2(t, dz, acc[q * NC + 2]))));
             // W += f_rr T + s d + (hd) x F
-            acc[q * NC + 3] = fma2(nhz, Fy, fma2(hy, Fz, fma2(frr, Tx, fma2(s, dx, acc[q * NC + 3]))));
-            acc[q * NC + 4] = fma2(nhx, Fz, fma2(hz, Fx, fma2(frr, Ty, fma2(s, dy, acc[q * NC + 4]))));
-            acc[q * NC + 5] = fma2(nhy, Fx, fma2(hx, Fy, fma2(frr, Tz, fma2(s, dz, acc[q * NC + 5]))));
+            acc[q * NC + 3] = fma2(hz, -Fy, fma2(hy, Fz, fma2(frr, Tx, fma2(s, dx, acc[q * NC + 3]))));
+            acc[q * NC + 4] = fma2(hx, -Fz, fma2(hz, Fx, fma2(frr, Ty, fma2(s, dy, acc[q * NC + 4]))));
+            acc[q * NC + 5] = fma2(hy, -Fx, fma2(hx, Fy, fma2(frr, Tz, fma2(s, dz, acc[q * NC + 5]))));
         }
     }
 }
 
 // ---------------------------------------------------------------- kernel
-template <typename T> struct Vec16;                   // 16-byte shared-memory load = 2 packed pairs (fp32) or 1 (fp64)
-template <> struct Vec16<float> { static constexpr int N = 4; };
-template <> struct Vec16<double> { static constexpr int N = 2; };
+template <typename T> struct Vec16;                   // 16-byte shared-memory load = 4 sources (fp32) or 2 (fp64)
+template <> struct Vec16<float> { static constexpr int N = 4; using type = float4; };
+template <> struct Vec16<double> { static constexpr int N = 2; using type = double2; };
+__device__ __forceinline__ float vget(const float4& v, int k) { return k == 0 ? v.x : (k == 1 ? v.y : (k == 2 ? v.z : v.w)); }
+__device__ __forceinline__ double vget(const double2& v, int k) { return k == 0 ? v.x : v.y; }
 
-template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES>
+constexpr int LOCK_CHUNKS = 15;   // chunks evaluated with the general body after two consecutive overlap hits
+
+template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES, int SUB>
 struct PairKernelTraits {
+    static_assert(TPT % 2 == 0, "targets are held as packed pairs");
+    static_assert(TJ % SUB == 0 && SUB % Vec16<T>::N == 0, "chunking");
     static constexpr int NC = ANG ? 6 : 3;             // components per source per right-hand side
     static constexpr int NV = NRHS * NC;               // packed vector arrays
+    static constexpr int NP = TPT / 2;                 // packed target pairs per thread
     static constexpr int ARRAYS = 3 + NV;              // x, y, z + vector components
     static constexpr int STAGE_BYTES = ARRAYS * TJ * (int)sizeof(T);
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + STAGES * 8;
     static constexpr int TARGETS = BLOCK * TPT;        // targets per CTA
 };
 
-template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES, int MINB>
+template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES, int SUB, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<T> p)
 {
-    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, BLOCK, TJ, STAGES>;
-    constexpr int NC = Tr::NC, NV = Tr::NV, ARRAYS = Tr::ARRAYS;
+    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, BLOCK, TJ, STAGES, SUB>;
+    constexpr int NC = Tr::NC, NV = Tr::NV, NP = Tr::NP, ARRAYS = Tr::ARRAYS;
     constexpr int VN = Vec16<T>::N;
+    using V16 = typename Vec16<T>::type;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     T* tiles = reinterpret_cast<T*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * Tr::STAGE_BYTES);
@@ -245,102 +269,115 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
         for (int s = 0; s < STAGES && s < my_tiles; ++s) issue(s);
     }
 
-    // targets: negated coordinates so that d = x_j + (-x_i) is one packed add
-    T nxi[TPT], nyi[TPT], nzi[TPT];
+    // targets: pair q holds targets i0 + (2q)*BLOCK + tid and i0 + (2q+1)*BLOCK + tid; negated
+    // coordinates so that d = x_j + (-x_i) is one packed add.  Targets past npad (last i-tile)
+    // re-read the last ghost; they are never stored.
+    P2<T> nx[NP], ny[NP], nz[NP];
 #pragma unroll
-    for (int t = 0; t < TPT; ++t) {
-        const int64_t i = i0 + t * BLOCK + tid;      // < npad: ghost targets read zeros
-        nxi[t] = -p.pos[i];
-        nyi[t] = -p.pos[p.npad + i];
-        nzi[t] = -p.pos[2 * p.npad + i];
+    for (int q = 0; q < NP; ++q) {
+        const int64_t ia = min(i0 + (2 * q) * BLOCK + tid, p.npad - 1), ib = min(i0 + (2 * q + 1) * BLOCK + tid, p.npad - 1);
+        nx[q] = mk2(-p.pos[ia], -p.pos[ib]);
+        ny[q] = mk2(-p.pos[p.npad + ia], -p.pos[p.npad + ib]);
+        nz[q] = mk2(-p.pos[2 * p.npad + ia], -p.pos[2 * p.npad + ib]);
     }
-    T total[TPT][NV];
+    P2<T> total[NP][NV];
 #pragma unroll
-    for (int t = 0; t < TPT; ++t)
+    for (int q = 0; q < NP; ++q)
 #pragma unroll
-        for (int k = 0; k < NV; ++k) total[t][k] = T(0);
+        for (int k = 0; k < NV; ++k) total[q][k] = splat(T(0));
+
+    int lock = 0;              // > 0: this warp evaluates chunks with the general body directly
+    bool prev_hit = false;
 
     for (int lt = 0; lt < my_tiles; ++lt) {
         const int stage = lt % STAGES;
         mbar_wait(&full[stage], (uint32_t)((lt / STAGES) & 1));
         const T* sx = tiles + (size_t)stage * ARRAYS * TJ;
-        P2<T> acc[TPT][NV];
-#pragma unroll
-        for (int t = 0; t < TPT; ++t)
-#pragma unroll
-            for (int k = 0; k < NV; ++k) acc[t][k] = splat(T(0));
 
 #pragma unroll 1
-        for (int j = 0; j < TJ; j += VN) {
-            if constexpr (VN == 4) {
-                const float4 X = *reinterpret_cast<const float4*>(sx + j);
-                const float4 Y = *reinterpret_cast<const float4*>(sx + TJ + j);
-                const float4 Z = *reinterpret_cast<const float4*>(sx + 2 * TJ + j);
-                P2<T> Va[NV], Vb[NV];
+        for (int sub = 0; sub < TJ; sub += SUB) {
+            P2<T> acc[NP][NV];
+            auto zero_acc = [&]() {
 #pragma unroll
-                for (int k = 0; k < NV; ++k) {
-                    const float4 v = *reinterpret_cast<const float4*>(sx + (3 + k) * TJ + j);
-                    Va[k] = mk2(v.x, v.y);
-                    Vb[k] = mk2(v.z, v.w);
-                }
+                for (int q = 0; q < NP; ++q)
 #pragma unroll
-                for (int t = 0; t < TPT; ++t) {
-                    pair_eval<T, NRHS, ANG>(p.c, nxi[t], nyi[t], nzi[t], mk2(X.x, X.y), mk2(Y.x, Y.y), mk2(Z.x, Z.y), Va, acc[t]);
-                    pair_eval<T, NRHS, ANG>(p.c, nxi[t], nyi[t], nzi[t], mk2(X.z, X.w), mk2(Y.z, Y.w), mk2(Z.z, Z.w), Vb, acc[t]);
+                    for (int k = 0; k < NV; ++k) acc[q][k] = splat(T(0));
+            };
+            auto chunk = [&](auto far_tag, bool& near) {
+                constexpr bool FAR = decltype(far_tag)::value;
+#pragma unroll 1
+                for (int j = sub; j < sub + SUB; j += VN) {
+                    const V16 X = *reinterpret_cast<const V16*>(sx + j);
+                    const V16 Y = *reinterpret_cast<const V16*>(sx + TJ + j);
+                    const V16 Z = *reinterpret_cast<const V16*>(sx + 2 * TJ + j);
+                    V16 Vv[NV];
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) Vv[k] = *reinterpret_cast<const V16*>(sx + (3 + k) * TJ + j);
+#pragma unroll
+                    for (int e = 0; e < VN; ++e) {
+                        T Vs[NV];
+#pragma unroll
+                        for (int k = 0; k < NV; ++k) Vs[k] = vget(Vv[k], e);
+#pragma unroll
+                        for (int q = 0; q < NP; ++q)
+                            pair_eval<T, NRHS, ANG, FAR>(p.c, nx[q], ny[q], nz[q], vget(X, e), vget(Y, e), vget(Z, e), Vs, acc[q], near);
+                    }
                 }
+            };
+            zero_acc();
+            bool hit = true;
+            if (lock == 0) {
+                bool near = false;
+                chunk(std::true_type{}, near);
+                hit = __any_sync(0xffffffffu, near);
+                if (hit) {
+                    zero_acc();
+                    if (prev_hit) lock = LOCK_CHUNKS;
+                }
+                prev_hit = hit;
             } else {
-                const double2 X = *reinterpret_cast<const double2*>(sx + j);
-                const double2 Y = *reinterpret_cast<const double2*>(sx + TJ + j);
-                const double2 Z = *reinterpret_cast<const double2*>(sx + 2 * TJ + j);
-                P2<T> Va[NV];
-#pragma unroll
-                for (int k = 0; k < NV; ++k) {
-                    const double2 v = *reinterpret_cast<const double2*>(sx + (3 + k) * TJ + j);
-                    Va[k] = mk2(v.x, v.y);
-                }
-#pragma unroll
-                for (int t = 0; t < TPT; ++t)
-                    pair_eval<T, NRHS, ANG>(p.c, nxi[t], nyi[t], nzi[t], mk2(X.x, X.y), mk2(Y.x, Y.y), mk2(Z.x, Z.y), Va, acc[t]);
+                --lock;
             }
+            if (hit) {
+                bool unused = false;
+                chunk(std::false_type{}, unused);
+            }
+            // flush the per-chunk packed accumulators (two-level summation)
+#pragma unroll
+            for (int q = 0; q < NP; ++q)
+#pragma unroll
+                for (int k = 0; k < NV; ++k) total[q][k] = add2(total[q][k], acc[q][k]);
         }
-        // flush the per-tile packed accumulators (two-level summation)
-#pragma unroll
-        for (int t = 0; t < TPT; ++t)
-#pragma unroll
-            for (int k = 0; k < NV; ++k) total[t][k] += lo(acc[t][k]) + hi(acc[t][k]);
 
         __syncthreads();                               // every warp is done reading this stage
         if (tid == 0 && lt + STAGES < my_tiles) issue(lt + STAGES);
     }
 
     // ---- epilogue
-    if (gridDim.y == 1) {
 #pragma unroll
-        for (int t = 0; t < TPT; ++t) {
-            const int64_t i = i0 + t * BLOCK + tid;
-            if (i < p.N) {
+    for (int q = 0; q < NP; ++q) {
 #pragma unroll
-                for (int q = 0; q < NRHS; ++q) {
-                    T* ul = p.out.lin[q] + 3 * i;
-                    ul[0] = total[t][q * NC + 0];
-                    ul[1] = total[t][q * NC + 1];
-                    ul[2] = total[t][q * NC + 2];
-                    if constexpr (ANG) {
-                        T* ua = p.out.ang[q] + 3 * i;
-                        ua[0] = total[t][q * NC + 3];
-                        ua[1] = total[t][q * NC + 4];
-                        ua[2] = total[t][q * NC + 5];
+        for (int half = 0; half < 2; ++half) {
+            const int64_t i = i0 + (2 * q + half) * BLOCK + tid;
+            if (gridDim.y == 1) {
+                if (i < p.N) {
+#pragma unroll
+                    for (int r = 0; r < NRHS; ++r) {
+                        T* ul = p.out.lin[r] + 3 * i;
+#pragma unroll
+                        for (int k = 0; k < 3; ++k) ul[k] = half ? hi(total[q][r * NC + k]) : lo(total[q][r * NC + k]);
+                        if constexpr (ANG) {
+                            T* ua = p.out.ang[r] + 3 * i;
+#pragma unroll
+                            for (int k = 0; k < 3; ++k) ua[k] = half ? hi(total[q][r * NC + 3 + k]) : lo(total[q][r * NC + 3 + k]);
+                        }
                     }
                 }
+            } else if (i < p.npad) {
+                T* part = p.partial + (size_t)blockIdx.y * NV * p.npad;
+#pragma unroll
+                for (int k = 0; k < NV; ++k) part[(size_t)k * p.npad + i] = half ? hi(total[q][k]) : lo(total[q][k]);
             }
-        }
-    } else {
-        T* part = p.partial + (size_t)blockIdx.y * NV * p.npad;
-#pragma unroll
-        for (int t = 0; t < TPT; ++t) {
-            const int64_t i = i0 + t * BLOCK + tid;
-#pragma unroll
-            for (int k = 0; k < NV; ++k) part[(size_t)k * p.npad + i] = total[t][k];
         }
     }
 }
