@@ -153,30 +153,26 @@ template <typename T> PairConsts<T> make_consts(double eta, double a)
 {
     const double pi = 3.14159265358979323846264338327950288;
     PairConsts<T> c;
-    const double C1 = 1.0 / (8.0 * pi * eta);          // Oseen prefactor
-    const double C4 = 1.0 / (6.0 * pi * eta * a);      // translational self mobility
-    const double C7 = 1.0 / (16.0 * pi * eta);
-    const double C8 = 1.0 / (8.0 * pi * eta * a * a * a);  // rotational self mobility
+    const double c4 = 4.0 / (3.0 * a);                 // (1/(6 pi eta a)) / C1: translational self mobility
+    const double c8 = 1.0 / (a * a * a);               // (1/(8 pi eta a^3)) / C1: rotational self mobility
     // floor of r^2: r = 0 becomes r = a 2^-40 (fp32) / a 2^-100 (fp64): a relative perturbation of the
     // self term far below the type's epsilon, while 1/r^3 stays finite (1/r^5 may overflow to +inf in
     // fp32; it only feeds the far branch, which the select discards for r < 2a)
     c.tiny = (T)std::max(a * a * std::ldexp(1.0, sizeof(T) == 4 ? -80 : -200), sizeof(T) == 4 ? 4.8e-38 : 1e-300);
     c.four_a2 = (T)(4.0 * a * a);
-    c.C1 = (T)C1;
-    c.C2 = (T)(C1 * 2.0 * a * a / 3.0);
-    c.nC3 = (T)(-C1 * 2.0 * a * a);
-    c.C4 = (T)C4;
-    c.nC5 = (T)(-C4 * 9.0 / (32.0 * a));
-    c.C6 = (T)(C4 * 3.0 / (32.0 * a));
-    c.nC7 = (T)(-C7);
-    c.C7x3 = (T)(3.0 * C7);
-    c.C8 = (T)C8;
-    c.K1 = (T)(-C8 * 27.0 / (32.0 * a));
-    c.K2 = (T)(C8 * 5.0 / (64.0 * a * a * a));
-    c.K3 = (T)(C8 * 9.0 / (32.0 * a));
-    c.K4 = (T)(-C8 * 3.0 / (64.0 * a * a * a));
-    c.K5 = (T)(1.0 / (16.0 * pi * eta * a * a * a));
-    c.K6 = (T)(-3.0 / (128.0 * pi * eta * a * a * a * a));
+    c.c2 = (T)(2.0 * a * a / 3.0);
+    c.nc3 = (T)(-2.0 * a * a);
+    c.c4 = (T)c4;
+    c.nc5 = (T)(-c4 * 9.0 / (32.0 * a));
+    c.c6 = (T)(c4 * 3.0 / (32.0 * a));
+    c.c8 = (T)c8;
+    c.k1 = (T)(-c8 * 27.0 / (32.0 * a));
+    c.k2 = (T)(c8 * 5.0 / (64.0 * a * a * a));
+    c.k3 = (T)(c8 * 9.0 / (32.0 * a));
+    c.k4 = (T)(-c8 * 3.0 / (64.0 * a * a * a));
+    c.k5 = (T)(1.0 / (2.0 * a * a * a));
+    c.k6 = (T)(-3.0 / (16.0 * a * a * a * a));
+    c.C1 = (T)(1.0 / (8.0 * pi * eta));                // Oseen prefactor, applied once per target
     return c;
 }
 

@@ -92,17 +92,37 @@ template <typename T> __device__ __forceinline__ P2<T> sel2(bool pl, bool ph, P2
 
 // ---------------------------------------------------------------- constants of the pair tensors
 // All derived on the host in fp64 from (eta, a) and rounded once to T.
-// d := x_j - x_i = -r_vec is used un-normalised; every 1/r^n needed is folded into the scalars:
-//   far  (r >= 2a): f_tt = invr (C1 + C2 u)          g_tt/r^2 = invr u (C1 - C3 u)       u = invr^2
-//                   f_rr = -C7 invr^3                g_rr/r^2 = 3 C7 invr^5              h = g_c/r = C1 invr^3
-//   near (r <  2a): f_tt = C4 - C5 r                 g_tt/r^2 = C6 invr
-//                   f_rr = C8 + r (K1 + K2 r^2)      g_rr/r^2 = K3 invr + K4 r           h = K5 + K6 r
+// d := x_j - x_i = -r_vec is used un-normalised, every 1/r^n needed is folded into the scalars, and
+// the Oseen prefactor C1 = 1/(8 pi eta) is factored out of every scalar and applied once per target
+// in the epilogue.  With s = 1/r, u = s^2, w3 = s^3, w5 = s^5 (all scalars below are "/ C1"):
+//   far  (r >= 2a): f_tt = s + c2 w3                 g_tt/r^2 = w3 (1 - c3 u)            c2 = 2a^2/3, c3 = 2a^2
+//                   f_rr = -w3/2                     g_rr/r^2 = 3 w5/2                   h = g_c/r = w3
+//   near (r <  2a): f_tt = c4 - c5 r                 g_tt/r^2 = c6 s                     c4 = 4/(3a)
+//                   f_rr = c8 + r (k1 + k2 r^2)      g_rr/r^2 = k3 s + k4 r              h = k5 + k6 r
 template <typename T> struct PairConsts {
     T tiny;    // additive floor of r^2: a^2 * 2^-80  (r = 0 -> finite 1/r, selected near branch)
     T four_a2; // (2a)^2
-    T C1, C2, nC3, C4, nC5, C6;           // translation-translation
-    T nC7, C7x3, C8, K1, K2, K3, K4, K5, K6; // rotation-rotation and coupling
+    T c2, nc3, c4, nc5, c6;               // translation-translation
+    T c8, k1, k2, k3, k4, k5, k6;         // rotation-rotation and coupling (near branch)
+    T C1;                                 // 1/(8 pi eta): applied in the epilogue
 };
+
+// overlap detector of the far-field fast path: running minimum of r^2 (fp32: one FMNMX3 per packed
+// pair) or an OR-ed predicate (fp64)
+struct NearF32 { float m; };
+struct NearF64 { bool any; };
+template <typename T> struct NearOf;
+template <> struct NearOf<float> { using type = NearF32; };
+template <> struct NearOf<double> { using type = NearF64; };
+__device__ __forceinline__ void near_init(NearF32& n) { n.m = 3.0e38f; }
+__device__ __forceinline__ void near_init(NearF64& n) { n.any = false; }
+__device__ __forceinline__ void near_update(NearF32& n, float a, float b, float)
+{
+    asm("min.f32 %0, %0, %1, %2;" : "+f"(n.m) : "f"(a), "f"(b));          // SASS: FMNMX3
+}
+__device__ __forceinline__ void near_update(NearF64& n, double a, double b, double four_a2) { n.any = n.any || a < four_a2 || b < four_a2; }
+__device__ __forceinline__ bool near_test(const NearF32& n, float four_a2) { return n.m < four_a2; }
+__device__ __forceinline__ bool near_test(const NearF64& n, double) { return n.any; }
 
 template <typename T> struct PairParams {
     const T* __restrict__ pos;  // [3][npad]  x | y | z, ghosts (index >= N) are zeros
@@ -145,30 +165,38 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 
 // ---------------------------------------------------------------- one source vs one packed target pair
-// FAR == true : far-field formulas only; `near` collects (r^2 < 4a^2) -- the caller discards the
-//               chunk if any lane of the warp saw an overlapping (or coincident) pair.
+// FAR == true : far-field formulas only; `near` collects min(r^2) / (r^2 < 4a^2) -- the caller
+//               discards the chunk if any lane of the warp saw an overlapping (or coincident) pair.
 // FAR == false: both branches, selected per lane.
 // (nx, ny, nz) = -x_i of the two targets; (xj, yj, zj), V[] = the source, warp-uniform scalars.
 template <typename T, int NRHS, bool ANG, bool FAR>
 __device__ __forceinline__ void pair_eval(const PairConsts<T>& c, P2<T> nx, P2<T> ny, P2<T> nz, T xj, T yj, T zj,
-                                          const T (&V)[NRHS * (ANG ? 6 : 3)], P2<T> (&acc)[NRHS * (ANG ? 6 : 3)], bool& near)
+                                          const T (&V)[NRHS * (ANG ? 6 : 3)], P2<T> (&acc)[NRHS * (ANG ? 6 : 3)],
+                                          typename NearOf<T>::type& near)
 {
     constexpr int NC = ANG ? 6 : 3;
     const P2<T> dx = add2(nx, xj), dy = add2(ny, yj), dz = add2(nz, zj);
     const P2<T> r2 = fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, splat(c.tiny))));
-    const bool nl = lo(r2) < c.four_a2, nh = hi(r2) < c.four_a2;
-    if constexpr (FAR) near = near || nl || nh;
+    if constexpr (FAR) near_update(near, lo(r2), hi(r2), c.four_a2);
     const P2<T> invr = rsqrt2(r2);
     const P2<T> u = mul2(invr, invr);
     const P2<T> w3 = mul2(invr, u);
+    P2<T> w5, f, g, r;
     // translation-translation scalars
-    P2<T> f = mul2(invr, fma2(u, c.C2, c.C1));
-    P2<T> g = mul2(w3, fma2(u, c.nC3, c.C1));
-    P2<T> r;
+    f = fma2(w3, c.c2, invr);
+    if constexpr (ANG) {
+        w5 = mul2(w3, u);
+        g = fma2(w5, c.nc3, w3);
+    } else {
+        g = mul2(w3, fma2(u, c.nc3, T(1)));
+    }
+    bool nl = false, nh = false;
     if constexpr (!FAR) {
+        nl = lo(r2) < c.four_a2;
+        nh = hi(r2) < c.four_a2;
         r = mul2(r2, invr);
-        f = sel2(nl, nh, fma2(r, c.nC5, c.C4), f);
-        g = sel2(nl, nh, mul2(invr, c.C6), g);
+        f = sel2(nl, nh, fma2(r, c.nc5, c.c4), f);
+        g = sel2(nl, nh, mul2(invr, c.c6), g);
     }
     if constexpr (!ANG) {
 #pragma unroll
@@ -181,13 +209,13 @@ __device__ __forceinline__ void pair_eval(const PairConsts<T>& c, P2<T> nx, P2<T
         }
     } else {
         // rotation-rotation and coupling scalars
-        P2<T> frr = mul2(w3, c.nC7);
-        P2<T> grr = mul2(mul2(w3, u), c.C7x3);
-        P2<T> h = mul2(w3, c.C1);
+        P2<T> frr = mul2(w3, T(-0.5));
+        P2<T> grr = mul2(w5, T(1.5));
+        P2<T> h = w3;
         if constexpr (!FAR) {
-            frr = sel2(nl, nh, fma2(r, fma2(r2, c.K2, c.K1), splat(c.C8)), frr);
-            grr = sel2(nl, nh, fma2(invr, c.K3, mul2(r, c.K4)), grr);
-            h = sel2(nl, nh, fma2(r, c.K6, c.K5), h);
+            frr = sel2(nl, nh, fma2(r, fma2(r2, c.k2, c.k1), splat(c.c8)), frr);
+            grr = sel2(nl, nh, fma2(invr, c.k3, mul2(r, c.k4)), grr);
+            h = sel2(nl, nh, fma2(r, c.k6, c.k5), h);
         }
         // with d = -r_vec:  g_c (T x rhat) = h (d x T),  g_c (F x rhat) = h (d x F)
         const P2<T> hx = mul2(h, dx), hy = mul2(h, dy), hz = mul2(h, dz);
@@ -303,7 +331,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 #pragma unroll
                     for (int k = 0; k < NV; ++k) acc[q][k] = splat(T(0));
             };
-            auto chunk = [&](auto far_tag, bool& near) {
+            using Near = typename NearOf<T>::type;
+            auto chunk = [&](auto far_tag, Near& near) {
                 constexpr bool FAR = decltype(far_tag)::value;
 #pragma unroll 1
                 for (int j = sub; j < sub + SUB; j += VN) {
@@ -327,9 +356,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
             zero_acc();
             bool hit = true;
             if (lock == 0) {
-                bool near = false;
+                Near near;
+                near_init(near);
                 chunk(std::true_type{}, near);
-                hit = __any_sync(0xffffffffu, near);
+                hit = __any_sync(0xffffffffu, near_test(near, p.c.four_a2));
                 if (hit) {
                     zero_acc();
                     if (prev_hit) lock = LOCK_CHUNKS;
@@ -339,7 +369,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
                 --lock;
             }
             if (hit) {
-                bool unused = false;
+                Near unused;
+                near_init(unused);
                 chunk(std::false_type{}, unused);
             }
             // flush the per-chunk packed accumulators (two-level summation)
@@ -353,7 +384,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
         if (tid == 0 && lt + STAGES < my_tiles) issue(lt + STAGES);
     }
 
-    // ---- epilogue
+    // ---- epilogue: apply the factored-out Oseen prefactor once per target
+#pragma unroll
+    for (int q = 0; q < NP; ++q)
+#pragma unroll
+        for (int k = 0; k < NV; ++k) total[q][k] = mul2(total[q][k], p.c.C1);
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
 #pragma unroll
