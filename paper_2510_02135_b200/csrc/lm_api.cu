@@ -22,51 +22,54 @@
 namespace lm {
 
 // ---------------------------------------------------------------- pair-kernel variants
-// LARGE: 256 threads x TPT targets (TPT/2 packed pairs per thread), 512-source tiles.  SMALL: 64 x 2,
-// 64-source tiles (fills 148 SMs when N is small, SURVEY.md sec. 7 "Small N").  npad is a multiple
-// of NPAD_QUANTUM so that either tile size divides it.  SUB = sources per overlap-vote chunk.
-constexpr int NPAD_QUANTUM = 512;
-constexpr int L_BLOCK = 256, L_TJ = 512, L_STAGES = 2, L_SUB = 32;
-constexpr int S_BLOCK = 64, S_TPT = 2, S_TJ = 64, S_STAGES = 2, S_SUB = 32;
+// LARGE: 256 threads x TPT targets (TPT/2 packed pairs per thread), tiles of up to 512 sources.
+// SMALL: 64 x 2, tiles of up to 64 sources (fills 148 SMs when N is small, SURVEY.md sec. 7 "Small N").
+// SUB = sources per overlap-vote chunk = the unit in which sources are dealt to the j-splits;
+// npad is a multiple of NPAD_QUANTUM, which every SUB divides.
+constexpr int NPAD_QUANTUM = 32;
+constexpr int L_BLOCK = 256, L_TJ = 512, L_STAGES = 2;
+constexpr int S_BLOCK = 64, S_TPT = 2, S_TJ = 64, S_STAGES = 2;
 constexpr int64_t MAX_SOURCES_PER_CTA = 262144;   // bounds the top level of the two-level fp32 summation
 
 template <typename T> struct Variant {
     void (*kernel)(const PairParams<T>);
-    int nrhs, ang, block, tpt, tj, smem;
+    int nrhs, ang, block, tpt, tj, sub, smem;
     int ctas_per_sm;      // filled at first use (occupancy API)
     double efficiency;    // relative per-pair throughput used by the launch chooser
 };
 
-template <typename T, int NRHS, bool ANG, int TPT, int MINB> Variant<T> make_large()
+template <typename T, int NRHS, bool ANG, int TPT, int SUB, int MINB> Variant<T> make_large()
 {
-    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, L_SUB>;
-    return {rpy_pair_kernel<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, L_SUB, MINB>, NRHS, ANG, L_BLOCK, TPT, L_TJ, Tr::SMEM_BYTES, 0, 1.0};
+    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB>;
+    static_assert(NPAD_QUANTUM % SUB == 0, "every SUB divides NPAD_QUANTUM");
+    return {rpy_pair_kernel<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB, MINB>, NRHS, ANG, L_BLOCK, TPT, L_TJ, SUB, Tr::SMEM_BYTES, 0, 1.0};
 }
-template <typename T, int NRHS, bool ANG, int MINB> Variant<T> make_small()
+template <typename T, int NRHS, bool ANG, int SUB, int MINB> Variant<T> make_small()
 {
-    using Tr = PairKernelTraits<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, S_SUB>;
-    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, S_SUB, MINB>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, Tr::SMEM_BYTES, 0, 0.8};
+    using Tr = PairKernelTraits<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB>;
+    static_assert(NPAD_QUANTUM % SUB == 0, "every SUB divides NPAD_QUANTUM");
+    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB, MINB>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, SUB, Tr::SMEM_BYTES, 0, 0.8};
 }
 
 template <typename T> std::vector<Variant<T>> build_variants();
 template <> std::vector<Variant<float>> build_variants<float>()
 {
-    return {make_large<float, 1, false, 4, 2>(), make_large<float, 2, false, 4, 1>(), make_large<float, 4, false, 2, 2>(),
-            make_large<float, 1, true, 2, 2>(),  make_large<float, 2, true, 2, 1>(),
-            make_small<float, 1, false, 8>(), make_small<float, 2, false, 8>(), make_small<float, 4, false, 6>(),
-            make_small<float, 1, true, 8>(),  make_small<float, 2, true, 6>()};
+    return {make_large<float, 1, false, 4, 32, 2>(), make_large<float, 2, false, 4, 32, 1>(), make_large<float, 4, false, 2, 32, 2>(),
+            make_large<float, 1, true, 2, 32, 2>(),  make_large<float, 2, true, 2, 32, 1>(),
+            make_small<float, 1, false, 32, 8>(), make_small<float, 2, false, 32, 8>(), make_small<float, 4, false, 32, 6>(),
+            make_small<float, 1, true, 32, 8>(),  make_small<float, 2, true, 32, 6>()};
 }
 template <> std::vector<Variant<double>> build_variants<double>()
 {
-    return {make_large<double, 1, false, 2, 2>(), make_large<double, 2, false, 2, 1>(), make_large<double, 4, false, 2, 1>(),
-            make_large<double, 1, true, 2, 1>(),  make_large<double, 2, true, 2, 1>(),
-            make_small<double, 1, false, 8>(), make_small<double, 2, false, 6>(), make_small<double, 4, false, 4>(),
-            make_small<double, 1, true, 6>(),  make_small<double, 2, true, 4>()};
+    return {make_large<double, 1, false, 2, 32, 2>(), make_large<double, 2, false, 2, 32, 1>(), make_large<double, 4, false, 2, 32, 1>(),
+            make_large<double, 1, true, 2, 32, 1>(),  make_large<double, 2, true, 2, 32, 1>(),
+            make_small<double, 1, false, 32, 8>(), make_small<double, 2, false, 32, 6>(), make_small<double, 4, false, 32, 4>(),
+            make_small<double, 1, true, 32, 6>(),  make_small<double, 2, true, 32, 4>()};
 }
 
 struct LaunchPlan {
     int variant = -1;
-    int i_tiles = 0, j_splits = 0, tiles_per_split = 0, n_tiles = 0;
+    int i_tiles = 0, j_splits = 0, n_units = 0;
 };
 
 }  // namespace lm
@@ -193,9 +196,10 @@ template <typename T> int init_variants(lm_solver* h)
     return LM_OK;
 }
 
-// Pick the variant and the number of j-splits: minimise (waves) x (tiles per CTA) x (cost of a
-// CTA-tile), where a wave is one resident set of CTAs.  Grid sizing in multiples of the SM count
-// x resident CTAs is what keeps the tail small (148 SMs).
+// Pick the variant and the number of j-splits.  Sources are dealt to the splits in units of SUB, as
+// evenly as possible, so the grid can be sized to a whole number of resident sets (148 SMs x
+// resident CTAs per SM) whatever N is.  Cost model: CTAs run in waves of `slots`; a CTA costs
+// (its sources + a fixed prologue/epilogue) x its targets; CTAs resident on one SM share it.
 template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
 {
     const auto& vs = variants<T>(h);
@@ -206,19 +210,20 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
         if (v.nrhs != nrhs || v.ang != h->angular) continue;
         const int targets = v.block * v.tpt;
         const int i_tiles = (int)((h->N + targets - 1) / targets);
-        const int n_tiles = (int)(h->npad / v.tj);
+        const int units = (int)(h->npad / v.sub);
         const int64_t slots = (int64_t)h->sm_count * v.ctas_per_sm;
-        const int max_splits = std::min(n_tiles, 128);
+        const int max_splits = std::min(units, 256);
         const int min_splits = (int)std::min<int64_t>(max_splits, (h->npad + MAX_SOURCES_PER_CTA - 1) / MAX_SOURCES_PER_CTA);
         for (int s = min_splits; s <= max_splits; ++s) {
-            const int tps = (n_tiles + s - 1) / s;
-            const int s_eff = (n_tiles + tps - 1) / tps;   // splits actually needed with that tile count
-            if (s_eff != s) continue;
+            const int64_t src = (int64_t)((units + s - 1) / s) * v.sub;            // sources of the largest split
             const int64_t ctas = (int64_t)i_tiles * s;
-            const int64_t waves = (ctas + slots - 1) / slots;
-            // time of one wave-tile: ctas_per_sm CTAs share an SM
-            // (+0.35 tile per CTA: prologue, pipeline fill and epilogue of a CTA, measured order of magnitude)
-            double cost = (double)waves * (tps + 0.35) * v.ctas_per_sm * ((double)v.tj * targets) / v.efficiency;
+            const int64_t full = ctas / slots, rem = ctas % slots;
+            const int64_t rem_per_sm = (rem + h->sm_count - 1) / h->sm_count;      // CTAs sharing an SM in the last wave
+            // prologue, pipeline fill and epilogue of a CTA ~ 0.35 tile (measured order of magnitude)
+            const double per_cta = ((double)src + 0.35 * v.tj) * targets / v.efficiency;
+            // few resident warps hide less latency: w warps per SM sub-partition cost a factor (1 + 0.15 / w)
+            auto wave = [&](int64_t resident) { return resident ? per_cta * resident * (1.0 + 0.15 * 128.0 / ((double)resident * v.block)) : 0.0; };
+            double cost = (double)full * wave(v.ctas_per_sm) + wave(rem_per_sm);
             // cost is in pairs evaluated back to back on one SM (~1e4 per microsecond): the reduce pass
             // adds a ~3 us launch plus writing and re-reading s partial vectors
             if (s > 1) cost += 3.0e4 + 0.1 * (double)s * (double)h->N;
@@ -227,8 +232,7 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
                 best.variant = vi;
                 best.i_tiles = i_tiles;
                 best.j_splits = s;
-                best.tiles_per_split = tps;
-                best.n_tiles = n_tiles;
+                best.n_units = units;
             }
         }
     }
@@ -274,8 +278,7 @@ template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& i
     p.partial = (T*)h->partial;
     p.N = h->N;
     p.npad = h->npad;
-    p.tiles_per_split = plan.tiles_per_split;
-    p.n_tiles = plan.n_tiles;
+    p.n_units = plan.n_units;
     p.c = make_consts<T>(h->eta, h->a);
 
     cudaEvent_t e0 = nullptr, e1 = nullptr;

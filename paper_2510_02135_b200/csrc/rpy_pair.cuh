@@ -130,9 +130,9 @@ template <typename T> struct PairParams {
     RhsOut<T> out;              // j_splits == 1: per right-hand side, 3N interleaved each
     T* __restrict__ partial;    // j_splits  > 1: [j_splits][nrhs*NC][npad]
     int64_t N;
-    int64_t npad;               // multiple of every TJ in use
-    int tiles_per_split;        // j-tiles handled by one CTA (last split may get fewer)
-    int n_tiles;                // npad / TJ
+    int64_t npad;               // multiple of NPAD_QUANTUM (hence of every SUB in use)
+    int n_units;                // npad / SUB: the sources are dealt to the gridDim.y j-splits in units of
+                                // SUB, as evenly as possible (split y gets units [y U / S, (y+1) U / S))
     PairConsts<T> c;
 };
 
@@ -272,19 +272,24 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 
     const int tid = threadIdx.x;
     const int64_t i0 = (int64_t)blockIdx.x * Tr::TARGETS;
-    const int jt_begin = blockIdx.y * p.tiles_per_split;
-    const int jt_end = min(jt_begin + p.tiles_per_split, p.n_tiles);
-    const int my_tiles = jt_end - jt_begin;
+    // this CTA's source range [j_begin, j_begin + j_count): a whole number of SUB-source units
+    const int u_begin = (int)((int64_t)blockIdx.y * p.n_units / gridDim.y);
+    const int u_end = (int)((int64_t)(blockIdx.y + 1) * p.n_units / gridDim.y);
+    const int64_t j_begin = (int64_t)u_begin * SUB;
+    const int j_count = (u_end - u_begin) * SUB;
+    const int my_tiles = (j_count + TJ - 1) / TJ;     // the last tile may be short
 
     auto issue = [&](int local_tile) {               // called by thread 0 only
         const int stage = local_tile % STAGES;
-        const int64_t j0 = (int64_t)(jt_begin + local_tile) * TJ;
+        const int64_t j0 = j_begin + (int64_t)local_tile * TJ;
+        const uint32_t nsrc = (uint32_t)min(TJ, j_count - local_tile * TJ);
+        const uint32_t bytes = nsrc * (uint32_t)sizeof(T);     // multiple of 16: SUB * sizeof(T) is
         T* dst = tiles + (size_t)stage * ARRAYS * TJ;
-        mbar_expect_tx(&full[stage], (uint32_t)Tr::STAGE_BYTES);
+        mbar_expect_tx(&full[stage], bytes * ARRAYS);
 #pragma unroll
-        for (int a = 0; a < 3; ++a) bulk_g2s(dst + a * TJ, p.pos + a * p.npad + j0, TJ * sizeof(T), &full[stage]);
+        for (int a = 0; a < 3; ++a) bulk_g2s(dst + a * TJ, p.pos + a * p.npad + j0, bytes, &full[stage]);
 #pragma unroll
-        for (int a = 0; a < NV; ++a) bulk_g2s(dst + (3 + a) * TJ, p.vec + a * p.npad + j0, TJ * sizeof(T), &full[stage]);
+        for (int a = 0; a < NV; ++a) bulk_g2s(dst + (3 + a) * TJ, p.vec + a * p.npad + j0, bytes, &full[stage]);
     };
 
     if (tid == 0) {
@@ -321,9 +326,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
         const int stage = lt % STAGES;
         mbar_wait(&full[stage], (uint32_t)((lt / STAGES) & 1));
         const T* sx = tiles + (size_t)stage * ARRAYS * TJ;
+        const int tile_count = min(TJ, j_count - lt * TJ);
 
 #pragma unroll 1
-        for (int sub = 0; sub < TJ; sub += SUB) {
+        for (int sub = 0; sub < tile_count; sub += SUB) {
             P2<T> acc[NP][NV];
             auto zero_acc = [&]() {
 #pragma unroll
