@@ -107,22 +107,25 @@ template <typename T> struct PairConsts {
     T C1;                                 // 1/(8 pi eta): applied in the epilogue
 };
 
-// overlap detector of the far-field fast path: running minimum of r^2 (fp32: one FMNMX3 per packed
-// pair) or an OR-ed predicate (fp64)
+// overlap detector of the far-field fast path: running minimum of r^2 over a group of pairs.
+// fp32: one FMNMX3 per packed pair.  fp64: r^2 >= 0, so IEEE order = integer order of the bit
+// pattern; the minimum is taken over the HIGH 32-bit words only (one VIMNMX3 on the integer pipe
+// instead of two FP64 compares) and the test is "<=", a superset of the exact r^2 < 4a^2: a group
+// flagged needlessly is evaluated by the general body, whose per-lane select is exact.
 struct NearF32 { float m; };
-struct NearF64 { bool any; };
+struct NearF64 { int m; };
 template <typename T> struct NearOf;
 template <> struct NearOf<float> { using type = NearF32; };
 template <> struct NearOf<double> { using type = NearF64; };
 __device__ __forceinline__ void near_init(NearF32& n) { n.m = 3.0e38f; }
-__device__ __forceinline__ void near_init(NearF64& n) { n.any = false; }
-__device__ __forceinline__ void near_update(NearF32& n, float a, float b, float)
+__device__ __forceinline__ void near_init(NearF64& n) { n.m = 0x7fffffff; }
+__device__ __forceinline__ void near_update(NearF32& n, float a, float b)
 {
     asm("min.f32 %0, %0, %1, %2;" : "+f"(n.m) : "f"(a), "f"(b));          // SASS: FMNMX3
 }
-__device__ __forceinline__ void near_update(NearF64& n, double a, double b, double four_a2) { n.any = n.any || a < four_a2 || b < four_a2; }
+__device__ __forceinline__ void near_update(NearF64& n, double a, double b) { n.m = min(n.m, min(__double2hiint(a), __double2hiint(b))); }
 __device__ __forceinline__ bool near_test(const NearF32& n, float four_a2) { return n.m < four_a2; }
-__device__ __forceinline__ bool near_test(const NearF64& n, double) { return n.any; }
+__device__ __forceinline__ bool near_test(const NearF64& n, double four_a2) { return n.m <= __double2hiint(four_a2); }
 
 template <typename T> struct PairParams {
     const T* __restrict__ pos;  // [3][npad]  x | y | z, ghosts (index >= N) are zeros
@@ -165,19 +168,33 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 
 // ---------------------------------------------------------------- one source vs one packed target pair
-// FAR == true : far-field formulas only; `near` collects min(r^2) / (r^2 < 4a^2) -- the caller
-//               discards the chunk if any lane of the warp saw an overlapping (or coincident) pair.
-// FAR == false: both branches, selected per lane.
+// Split in two so that the far / general decision of a whole group of pairs is taken BEFORE anything
+// is accumulated: pair_geom gives d = x_j - x_i and r^2 (and feeds the overlap detector); pair_apply
+// builds the scalars and accumulates.
+//   FAR == true : far-field formulas only (the caller has checked that no pair of the group overlaps).
+//   FAR == false: both branches, selected per lane.
 // (nx, ny, nz) = -x_i of the two targets; (xj, yj, zj), V[] = the source, warp-uniform scalars.
+template <typename T> struct PairGeom { P2<T> dx, dy, dz, r2; };
+
+template <typename T>
+__device__ __forceinline__ PairGeom<T> pair_geom(const PairConsts<T>& c, P2<T> nx, P2<T> ny, P2<T> nz, T xj, T yj, T zj,
+                                                 typename NearOf<T>::type& near)
+{
+    PairGeom<T> g;
+    g.dx = add2(nx, xj);
+    g.dy = add2(ny, yj);
+    g.dz = add2(nz, zj);
+    g.r2 = fma2(g.dz, g.dz, fma2(g.dy, g.dy, fma2(g.dx, g.dx, splat(c.tiny))));
+    near_update(near, lo(g.r2), hi(g.r2));
+    return g;
+}
+
 template <typename T, int NRHS, bool ANG, bool FAR>
-__device__ __forceinline__ void pair_eval(const PairConsts<T>& c, P2<T> nx, P2<T> ny, P2<T> nz, T xj, T yj, T zj,
-                                          const T (&V)[NRHS * (ANG ? 6 : 3)], P2<T> (&acc)[NRHS * (ANG ? 6 : 3)],
-                                          typename NearOf<T>::type& near)
+__device__ __forceinline__ void pair_apply(const PairConsts<T>& c, const PairGeom<T>& gm, const T (&V)[NRHS * (ANG ? 6 : 3)],
+                                           P2<T> (&acc)[NRHS * (ANG ? 6 : 3)])
 {
     constexpr int NC = ANG ? 6 : 3;
-    const P2<T> dx = add2(nx, xj), dy = add2(ny, yj), dz = add2(nz, zj);
-    const P2<T> r2 = fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, splat(c.tiny))));
-    if constexpr (FAR) near_update(near, lo(r2), hi(r2), c.four_a2);
+    const P2<T> dx = gm.dx, dy = gm.dy, dz = gm.dz, r2 = gm.r2;
     const P2<T> invr = rsqrt2(r2);
     const P2<T> u = mul2(invr, invr);
     const P2<T> w3 = mul2(invr, u);
@@ -244,12 +261,12 @@ template <> struct Vec16<double> { static constexpr int N = 2; using type = doub
 __device__ __forceinline__ float vget(const float4& v, int k) { return k == 0 ? v.x : (k == 1 ? v.y : (k == 2 ? v.z : v.w)); }
 __device__ __forceinline__ double vget(const double2& v, int k) { return k == 0 ? v.x : v.y; }
 
-constexpr int LOCK_CHUNKS = 15;   // chunks evaluated with the general body after two consecutive overlap hits
-
 template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES, int SUB>
 struct PairKernelTraits {
     static_assert(TPT % 2 == 0, "targets are held as packed pairs");
-    static_assert(TJ % SUB == 0 && SUB % Vec16<T>::N == 0, "chunking");
+    static_assert(TJ % SUB == 0 && SUB % Vec16<T>::N == 0, "source units");
+    // sources per far/general decision: the group's geometry (GS x NP packed d, r^2) stays in registers
+    static constexpr int GS = ((TPT / 2 >= 2 || NRHS * (ANG ? 6 : 3) >= 12) && Vec16<T>::N > 2) ? 2 : Vec16<T>::N;
     static constexpr int NC = ANG ? 6 : 3;             // components per source per right-hand side
     static constexpr int NV = NRHS * NC;               // packed vector arrays
     static constexpr int NP = TPT / 2;                 // packed target pairs per thread
@@ -264,7 +281,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 {
     using Tr = PairKernelTraits<T, NRHS, ANG, TPT, BLOCK, TJ, STAGES, SUB>;
     constexpr int NC = Tr::NC, NV = Tr::NV, NP = Tr::NP, ARRAYS = Tr::ARRAYS;
-    constexpr int VN = Vec16<T>::N;
+    constexpr int VN = Vec16<T>::N, GS = Tr::GS;
     using V16 = typename Vec16<T>::type;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     T* tiles = reinterpret_cast<T*>(smem_raw);
@@ -319,8 +336,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 #pragma unroll
         for (int k = 0; k < NV; ++k) total[q][k] = splat(T(0));
 
-    int lock = 0;              // > 0: this warp evaluates chunks with the general body directly
-    bool prev_hit = false;
+    using Near = typename NearOf<T>::type;
 
     for (int lt = 0; lt < my_tiles; ++lt) {
         const int stage = lt % STAGES;
@@ -328,63 +344,54 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
         const T* sx = tiles + (size_t)stage * ARRAYS * TJ;
         const int tile_count = min(TJ, j_count - lt * TJ);
 
+        // per-tile packed accumulators (two-level summation: flushed into `total` at the tile end)
+        P2<T> acc[NP][NV];
+#pragma unroll
+        for (int q = 0; q < NP; ++q)
+#pragma unroll
+            for (int k = 0; k < NV; ++k) acc[q][k] = splat(T(0));
+
+        // sources are walked in groups of GS; the geometry of the whole group (GS x NP packed pairs)
+        // comes first, one warp vote on its minimum r^2 picks the far-field or the general body
 #pragma unroll 1
-        for (int sub = 0; sub < tile_count; sub += SUB) {
-            P2<T> acc[NP][NV];
-            auto zero_acc = [&]() {
+        for (int j = 0; j < tile_count; j += VN) {
+            const V16 X = *reinterpret_cast<const V16*>(sx + j);
+            const V16 Y = *reinterpret_cast<const V16*>(sx + TJ + j);
+            const V16 Z = *reinterpret_cast<const V16*>(sx + 2 * TJ + j);
+            V16 Vv[NV];
 #pragma unroll
-                for (int q = 0; q < NP; ++q)
+            for (int k = 0; k < NV; ++k) Vv[k] = *reinterpret_cast<const V16*>(sx + (3 + k) * TJ + j);
 #pragma unroll
-                    for (int k = 0; k < NV; ++k) acc[q][k] = splat(T(0));
-            };
-            using Near = typename NearOf<T>::type;
-            auto chunk = [&](auto far_tag, Near& near) {
-                constexpr bool FAR = decltype(far_tag)::value;
-#pragma unroll 1
-                for (int j = sub; j < sub + SUB; j += VN) {
-                    const V16 X = *reinterpret_cast<const V16*>(sx + j);
-                    const V16 Y = *reinterpret_cast<const V16*>(sx + TJ + j);
-                    const V16 Z = *reinterpret_cast<const V16*>(sx + 2 * TJ + j);
-                    V16 Vv[NV];
-#pragma unroll
-                    for (int k = 0; k < NV; ++k) Vv[k] = *reinterpret_cast<const V16*>(sx + (3 + k) * TJ + j);
-#pragma unroll
-                    for (int e = 0; e < VN; ++e) {
-                        T Vs[NV];
-#pragma unroll
-                        for (int k = 0; k < NV; ++k) Vs[k] = vget(Vv[k], e);
-#pragma unroll
-                        for (int q = 0; q < NP; ++q)
-                            pair_eval<T, NRHS, ANG, FAR>(p.c, nx[q], ny[q], nz[q], vget(X, e), vget(Y, e), vget(Z, e), Vs, acc[q], near);
-                    }
-                }
-            };
-            zero_acc();
-            bool hit = true;
-            if (lock == 0) {
+            for (int e0 = 0; e0 < VN; e0 += GS) {
+                PairGeom<T> gm[GS][NP];
                 Near near;
                 near_init(near);
-                chunk(std::true_type{}, near);
-                hit = __any_sync(0xffffffffu, near_test(near, p.c.four_a2));
-                if (hit) {
-                    zero_acc();
-                    if (prev_hit) lock = LOCK_CHUNKS;
-                }
-                prev_hit = hit;
-            } else {
-                --lock;
-            }
-            if (hit) {
-                Near unused;
-                near_init(unused);
-                chunk(std::false_type{}, unused);
-            }
-            // flush the per-chunk packed accumulators (two-level summation)
 #pragma unroll
-            for (int q = 0; q < NP; ++q)
+                for (int e = 0; e < GS; ++e)
 #pragma unroll
-                for (int k = 0; k < NV; ++k) total[q][k] = add2(total[q][k], acc[q][k]);
+                    for (int q = 0; q < NP; ++q)
+                        gm[e][q] = pair_geom<T>(p.c, nx[q], ny[q], nz[q], vget(X, e0 + e), vget(Y, e0 + e), vget(Z, e0 + e), near);
+                const bool hit = __any_sync(0xffffffffu, near_test(near, p.c.four_a2));
+                auto body = [&](auto far_tag) {
+                    constexpr bool FAR = decltype(far_tag)::value;
+#pragma unroll
+                    for (int e = 0; e < GS; ++e) {
+                        T Vs[NV];
+#pragma unroll
+                        for (int k = 0; k < NV; ++k) Vs[k] = vget(Vv[k], e0 + e);
+#pragma unroll
+                        for (int q = 0; q < NP; ++q) pair_apply<T, NRHS, ANG, FAR>(p.c, gm[e][q], Vs, acc[q]);
+                    }
+                };
+                if (!hit) body(std::true_type{});
+                else body(std::false_type{});
+            }
         }
+        // flush the per-tile packed accumulators
+#pragma unroll
+        for (int q = 0; q < NP; ++q)
+#pragma unroll
+            for (int k = 0; k < NV; ++k) total[q][k] = add2(total[q][k], acc[q][k]);
 
         __syncthreads();                               // every warp is done reading this stage
         if (tid == 0 && lt + STAGES < my_tiles) issue(lt + STAGES);
