@@ -205,9 +205,12 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
     const auto& vs = variants<T>(h);
     LaunchPlan best;
     double best_cost = 1e300;
+    int dbg_block = 0, dbg_splits = 0;                       // TUNING ONLY
+    if (const char* e = std::getenv("LM_PLAN")) std::sscanf(e, "%d,%d", &dbg_block, &dbg_splits);
     for (int vi = 0; vi < (int)vs.size(); ++vi) {
         const auto& v = vs[vi];
         if (v.nrhs != nrhs || v.ang != h->angular) continue;
+        if (dbg_block && v.block != dbg_block) continue;
         const int targets = v.block * v.tpt;
         const int i_tiles = (int)((h->N + targets - 1) / targets);
         const int units = (int)(h->npad / v.sub);
@@ -215,14 +218,15 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
         const int max_splits = std::min(units, 256);
         const int min_splits = (int)std::min<int64_t>(max_splits, (h->npad + MAX_SOURCES_PER_CTA - 1) / MAX_SOURCES_PER_CTA);
         for (int s = min_splits; s <= max_splits; ++s) {
+            if (dbg_splits && s != std::min(dbg_splits, max_splits)) continue;
             const int64_t src = (int64_t)((units + s - 1) / s) * v.sub;            // sources of the largest split
             const int64_t ctas = (int64_t)i_tiles * s;
             const int64_t full = ctas / slots, rem = ctas % slots;
             const int64_t rem_per_sm = (rem + h->sm_count - 1) / h->sm_count;      // CTAs sharing an SM in the last wave
-            // prologue, pipeline fill and epilogue of a CTA ~ 0.35 tile (measured order of magnitude)
-            const double per_cta = ((double)src + 0.35 * v.tj) * targets / v.efficiency;
-            // few resident warps hide less latency: w warps per SM sub-partition cost a factor (1 + 0.15 / w)
-            auto wave = [&](int64_t resident) { return resident ? per_cta * resident * (1.0 + 0.15 * 128.0 / ((double)resident * v.block)) : 0.0; };
+            // prologue, pipeline fill and epilogue of a CTA ~ 0.1 tile (fitted to plan sweeps on B200)
+            const double per_cta = ((double)src + 0.1 * v.tj) * targets / v.efficiency;
+            // few resident warps hide less latency: w warps per SM sub-partition cost a factor (1 + 0.3 / w)
+            auto wave = [&](int64_t resident) { return resident ? per_cta * resident * (1.0 + 0.3 * 128.0 / ((double)resident * v.block)) : 0.0; };
             double cost = (double)full * wave(v.ctas_per_sm) + wave(rem_per_sm);
             // cost is in pairs evaluated back to back on one SM (~1e4 per microsecond): the reduce pass
             // adds a ~3 us launch plus writing and re-reading s partial vectors

@@ -272,7 +272,7 @@ struct PairKernelTraits {
     static constexpr int NP = TPT / 2;                 // packed target pairs per thread
     static constexpr int ARRAYS = 3 + NV;              // x, y, z + vector components
     static constexpr int STAGE_BYTES = ARRAYS * TJ * (int)sizeof(T);
-    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + STAGES * 8;
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + STAGES * 8 + STAGES * 8;   // tiles | full mbarriers | done counters
     static constexpr int TARGETS = BLOCK * TPT;        // targets per CTA
 };
 
@@ -286,6 +286,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
     extern __shared__ __align__(128) unsigned char smem_raw[];
     T* tiles = reinterpret_cast<T*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * Tr::STAGE_BYTES);
+    unsigned int* done = reinterpret_cast<unsigned int*>(full + STAGES);   // warps that finished with a stage (monotonic)
+    constexpr unsigned int NWARPS = BLOCK / 32;
 
     const int tid = threadIdx.x;
     const int64_t i0 = (int64_t)blockIdx.x * Tr::TARGETS;
@@ -311,7 +313,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(&full[s], 1);
+            done[s] = 0u;
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -393,8 +398,13 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 #pragma unroll
             for (int k = 0; k < NV; ++k) total[q][k] = add2(total[q][k], acc[q][k]);
 
-        __syncthreads();                               // every warp is done reading this stage
-        if (tid == 0 && lt + STAGES < my_tiles) issue(lt + STAGES);
+        // release the stage without a CTA-wide barrier: every warp counts itself out, the LAST one to
+        // leave refills the stage (TMA) -- no warp ever waits for another except on the data it needs
+        __syncwarp();
+        if ((tid & 31) == 0) {
+            const unsigned int left = atomicAdd(&done[stage], 1u) + 1u;
+            if (left % NWARPS == 0u && lt + STAGES < my_tiles) issue(lt + STAGES);
+        }
     }
 
     // ---- epilogue: apply the factored-out Oseen prefactor once per target
