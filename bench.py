@@ -42,17 +42,24 @@ METRIC = "rpy_pair_interactions_per_s"
 UNIT = "Gpairs/s"
 
 # Algorithmic FP-pipe lane-operations and flops per ordered pair (counted from the
-# algebra, never from emitted instructions).  key: (angular, nrhs)
+# algebra of a far-field pair, never from emitted instructions; an overlapping pair needs fewer).
+#   translational: d 3, r^2 3, u = s^2 and s^3 2, f 1, g 2 -> 11;  per right-hand side: d.F 3, t 1, U += fF + td 6 -> 10
+#   angular      : + s^5 1, f_rr 1, g_rr 1, h d 3, g one fewer -> 16;  per right-hand side: d.F, d.T 6, t, s 2, 24 FMAs -> 32
 def work_per_pair(angular: bool, nrhs: int, f64: bool):
-    """Minimal algebra of a far-field pair (r >= 2a; an overlapping pair needs fewer), DESIGN.md sec. 7."""
     if angular:
-        instr, fma = 19 + 32 * nrhs, 5 + 28 * nrhs
+        instr, fma = 16 + 32 * nrhs, 4 + 28 * nrhs
     else:
-        instr, fma = 12 + 10 * nrhs, 5 + 8 * nrhs
+        instr, fma = 11 + 10 * nrhs, 4 + 8 * nrhs
     if f64:
         instr, fma = instr + 5, fma + 3      # fp64 refinement of the rsqrt seed
     flops = instr + fma + 1                  # FMA = 2 flops, + the rsqrt
     return instr, flops
+
+
+# DRAM traffic of ONE pair-kernel launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
+# `ncu --set full` captures profiles/r1_c<N>_pair_kernel_ncu_full.md (same launch configuration); it is a
+# recorded profile value, not measured by this run.  Configs 4 and 5 are dominated by the j-split partials.
+NCU_DRAM_BYTES_PER_LAUNCH = {1: 64.512e3, 2: 610.56e3, 3: 3.183104e6, 4: 161.415168e6 + 638.553344e6, 5: 27.725056e6 + 114.036736e6}
 
 
 def nominal_lanes(f64: bool) -> int:
@@ -336,7 +343,9 @@ def main():
     probe = lm.lm_probe_fma_peak(lm.LM_F64 if f64 else lm.LM_F32, 0.3) / 1e12
     roofline = {
         "bound": "alu", "kernel": f"rpy_pair_kernel<{cfg.precision}, nrhs={nrhs_launch}, angular={int(cfg.angular)}>",
-        "achieved": achieved, "peak": peak, "unit": "T FP-pipe lane-ops/s", "frac": achieved / peak, "traffic": None,
+        "achieved": achieved, "peak": peak, "unit": "T FP-pipe lane-ops/s", "frac": achieved / peak,
+        "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if args.N is None else None,
+        "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_c%d_pair_kernel_ncu_full.md)" % args.config,
         "peak_source": f"derived: {sms} SMs x {nominal_lanes(f64)} lanes x {sm_max_mhz:.0f} MHz (clocks.max.sm); MEASURED_PEAKS.json has no ALU entry",
         "lane_ops_per_pair": instr, "flops_per_pair": flops, "pairs_per_launch": float(N) * float(N),
         "launch_ms_avg": pair_ms_avg, "launches_timed": launches_pair,
