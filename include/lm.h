@@ -12,6 +12,7 @@
  *   Mdot(forces, torques) -> (linear, angular)        lm_mdot, lm_mdot_batch
  *   sqrtMdotW()           -> (linear, angular)        lm_sqrt_mdot_w
  *   mf + dwf + drift (the sum the example forms)      lm_hydrodynamic_velocities PAPER.md:78 (eq. 9), 137-138
+ *   eq. (13) steric force, eq. (14) AB time step       lm_steric_forces, lm_bd_step
  *   divM()                                            not exported: identically zero for open
  *                                                     boundaries
  *
@@ -112,6 +113,33 @@ int lm_sqrt_mdot_w_host(lm_solver* h, const void* noise, double tol, void* lin_o
                         int* iters_out, void* stream);
 int lm_hydrodynamic_velocities_host(lm_solver* h, const void* forces, const void* torques, const void* noise,
                                     double noise_prefactor, double tol, void* lin_out, void* ang_out, void* stream);
+
+/* ---- Free-space Brownian-dynamics step built on the calls above (sec. 5.1) ----
+ *
+ * lm_steric_forces: forces_out = ext_forces + the soft pairwise repulsion of eq. (13)
+ *   U(r) = U0 (1 + (d - r)/b) for r < d,  U0 exp((d - r)/b) for r >= d,  d = 2a (particle-particle),
+ * summed over all ordered pairs j != i at the positions of the last lm_set_positions:
+ *   F_i = ext_i + sum_j m(r_ij) (x_i - x_j)/r_ij,  m = -U' = U0/b (r < d), (U0/b) exp((d - r)/b) (r >= d).
+ * Pairs beyond r_c = d + 20 b (fp32) / d + 40 b (fp64) are dropped (exp below the type's epsilon);
+ * exactly coincident particles exert nothing on each other.  ext_forces: 3N or NULL.  forces_out: 3N.
+ * Asynchronous on `stream`.  b <= 0 -> LM_E_INVALID.
+ *
+ * lm_bd_step: one step of the stochastic Adams-Bashforth scheme, eq. (14), in place:
+ *   X^{n+1} = X^n + dt (3/2 M^n F^n - 1/2 M^{n-1} F^{n-1}) + sqrt(2 kT dt) (M^n)^{1/2} W^n
+ * with F^n = lm_steric_forces(X^n; U0, b) + ext_forces (U0 == 0: no steric term), external torques
+ * ext_torques (include_angular only; the spheres' orientations are not tracked), and the thermal-drift
+ * terms of eq. (14) identically zero for open boundaries.  The first step after
+ * lm_create / lm_bd_reset has no history and is forward Euler.  pos: 3N, read and overwritten.
+ * noise: W^n, dof values as for lm_sqrt_mdot_w, or NULL (or kT == 0) for a deterministic step; tol:
+ * Lanczos tolerance.  The handle keeps M^n F^n for the next step.  Synchronises the stream when noise
+ * is given.  After the call the handle's packed positions are X^n (stale): call lm_set_positions
+ * before lm_mdot etc.  Returns LM_E_NOCONV if Lanczos hit max_iter (the step is still taken). */
+int lm_steric_forces(lm_solver* h, double U0, double b, const void* ext_forces, void* forces_out, void* stream);
+int lm_bd_step(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise,
+               double dt, double kT, double U0, double b, double tol, void* stream);
+int lm_bd_step_host(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise,
+                    double dt, double kT, double U0, double b, double tol, void* stream);
+int lm_bd_reset(lm_solver* h);                        /* forget the Adams-Bashforth history */
 
 /* Lanczos controls and introspection. */
 int lm_set_max_iter(lm_solver* h, int max_iter);     /* default 100; 1 <= max_iter <= 1000 */

@@ -33,19 +33,21 @@ def steric_potential(r, U0: float, b: float, d: float):
     return np.where(r < d, U0 * (1.0 + (d - r) / b), U0 * np.exp((d - r) / b))
 
 
-def steric_forces(pos, U0: float, b: float, d: float) -> np.ndarray:
-    """(N,3) forces from eq. (13), all ordered pairs j != i, row by row."""
+def steric_forces(pos, U0: float, b: float, d: float, rows=None) -> np.ndarray:
+    """Forces from eq. (13), all ordered pairs j != i, row by row.  (N,3), or (len(rows),3) for the
+    listed target rows only (rows are independent, so a sample is exact for its rows)."""
     x = np.asarray(pos, dtype=np.float64).reshape(-1, 3)
     N = x.shape[0]
-    F = np.zeros((N, 3))
-    for i in range(N):
+    targets = range(N) if rows is None else [int(i) for i in rows]
+    F = np.zeros((len(targets), 3))
+    for out, i in enumerate(targets):
         rv = x[i] - x                              # r_vec = x_i - x_j, points from j to i
         r = np.sqrt(np.sum(rv * rv, axis=1))
         ok = r > 0.0                               # skips j = i and exactly coincident particles
         rr = r[ok]
         # -dU/dr: U0/b inside the core, (U0/b) exp((d - r)/b) outside
         mag = np.where(rr < d, U0 / b, (U0 / b) * np.exp((d - rr) / b))
-        F[i] = np.sum((mag / rr)[:, None] * rv[ok], axis=0)
+        F[out] = np.sum((mag / rr)[:, None] * rv[ok], axis=0)
     return F
 
 

@@ -36,6 +36,10 @@ SIGNATURES = {
     "lm_mdot_batch_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "lm_sqrt_mdot_w_host": (c_int, [c_void_p, c_void_p, c_double, c_void_p, c_void_p, POINTER(c_int), c_void_p]),
     "lm_hydrodynamic_velocities_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_void_p, c_void_p, c_void_p]),
+    "lm_steric_forces": (c_int, [c_void_p, c_double, c_double, c_void_p, c_void_p, c_void_p]),
+    "lm_bd_step": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_double, c_double, c_double, c_void_p]),
+    "lm_bd_step_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_double, c_double, c_double, c_void_p]),
+    "lm_bd_reset": (c_int, [c_void_p]),
     "lm_set_max_iter": (c_int, [c_void_p, c_int]),
     "lm_last_iterations": (c_int, [c_void_p]),
     "lm_last_error": (c_char_p, [c_void_p]),
@@ -216,6 +220,29 @@ class Solver:
     def hydrodynamic_velocities_host(self, forces, torques, noise, noise_prefactor, tol, lin_out, ang_out=None, stream=None):
         self._check(lib().lm_hydrodynamic_velocities_host(self._h, _ptr(forces), _ptr(torques), _ptr(noise), float(noise_prefactor),
                                                           float(tol), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+
+    # -- free-space Brownian-dynamics step (eqs. (13), (14))
+    def steric_forces(self, U0, b, ext_forces, forces_out, stream=None):
+        for x in (ext_forces, forces_out):
+            self._expect(x, 3 * self.N, False)
+        self._check(lib().lm_steric_forces(self._h, float(U0), float(b), _ptr(ext_forces), _ptr(forces_out), _stream_ptr(stream)))
+
+    def bd_step(self, pos, ext_forces, ext_torques, noise, dt, kT, U0, b, tol, stream=None, allow_noconv=False) -> int:
+        for x in (pos, ext_forces, ext_torques):
+            self._expect(x, 3 * self.N, False)
+        self._expect(noise, (6 if self.angular else 3) * self.N, False)
+        return self._check(lib().lm_bd_step(self._h, _ptr(pos), _ptr(ext_forces), _ptr(ext_torques), _ptr(noise), float(dt), float(kT),
+                                            float(U0), float(b), float(tol), _stream_ptr(stream)), allow=(LM_E_NOCONV,) if allow_noconv else ())
+
+    def bd_step_host(self, pos, ext_forces, ext_torques, noise, dt, kT, U0, b, tol, stream=None, allow_noconv=False) -> int:
+        for x in (pos, ext_forces, ext_torques):
+            self._expect(x, 3 * self.N, True)
+        self._expect(noise, (6 if self.angular else 3) * self.N, True)
+        return self._check(lib().lm_bd_step_host(self._h, _ptr(pos), _ptr(ext_forces), _ptr(ext_torques), _ptr(noise), float(dt), float(kT),
+                                                 float(U0), float(b), float(tol), _stream_ptr(stream)), allow=(LM_E_NOCONV,) if allow_noconv else ())
+
+    def bd_reset(self):
+        self._check(lib().lm_bd_reset(self._h))
 
     # -- controls / introspection
     def set_max_iter(self, n):

@@ -16,6 +16,7 @@
 
 #include "../../include/lm.h"
 #include "rpy_pair.cuh"
+#include "steric_pair.cuh"
 #include "tridiag_host.h"
 #include "vector_kernels.cuh"
 
@@ -103,6 +104,11 @@ struct lm_solver {
     double* d_gram = nullptr;  // Gram column V[j].V[k], j <= k
     double* d_gram_part = nullptr;
     double* h_gram = nullptr;  // pinned
+
+    // Brownian-dynamics step (lm_bd_step): F, v_n, v_{n-1}, noise velocity, angular scratch x2, position staging
+    void* bd[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    size_t bd_bytes[7] = {0, 0, 0, 0, 0, 0, 0};
+    bool bd_have_prev = false;
 
     // staging for the _host entry points
     void* st[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // pos, f, t, noise, lin, ang
@@ -445,6 +451,80 @@ int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_
     return LM_OK;
 }
 
+// ---------------------------------------------------------------- steric forces and the BD step
+template <typename T> int set_positions_t(lm_solver* h, const void* pos, cudaStream_t st);
+
+template <typename T>
+int steric_device(lm_solver* h, double U0, double b, const T* ext, T* out, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        LM_CUDA(h, cudaFuncSetAttribute((const void*)steric_pair_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, steric_smem_bytes<T>()));
+        attr_set = true;
+    }
+    const int units = (int)(h->npad / STERIC_SUB);
+    const int i_tiles = (int)((h->N + STERIC_TARGETS - 1) / STERIC_TARGETS);
+    // about four resident sets of CTAs (2 per SM): the work per CTA depends on how many groups are within the cut-off
+    const int splits = (int)std::max<int64_t>(1, std::min<int64_t>(units, ((int64_t)8 * h->sm_count + i_tiles - 1) / i_tiles));
+    int rc = ensure(h, &h->partial, &h->partial_bytes, (size_t)splits * 3 * h->npad * sizeof(T));
+    if (rc != LM_OK) return rc;
+    const double K = sizeof(T) == 4 ? 20.0 : 40.0;           // exp(-K) below the type's epsilon
+    StericParams<T> p;
+    p.pos = (const T*)h->pos_soa;
+    p.partial = (T*)h->partial;
+    p.N = h->N;
+    p.npad = h->npad;
+    p.n_units = units;
+    p.tiny = make_consts<T>(h->eta, h->a).tiny;
+    p.d = (T)(2.0 * h->a);
+    p.rc2 = (T)((2.0 * h->a + K * b) * (2.0 * h->a + K * b));
+    p.m0 = (T)(U0 / b);
+    p.inv_b = (T)(sizeof(T) == 4 ? 1.4426950408889634 / b : 1.0 / b);
+    steric_pair_kernel<T><<<dim3(i_tiles, splits), STERIC_BLOCK, steric_smem_bytes<T>(), st>>>(p);
+    steric_reduce_kernel<T><<<grid_1d(h->N), VEC_BLOCK, 0, st>>>((const T*)h->partial, splits, h->N, h->npad, ext, out);
+    h->n_aux += 2;
+    LM_CUDA(h, cudaGetLastError());
+    return LM_OK;
+}
+
+template <typename T>
+int bd_step_device(lm_solver* h, T* pos, const T* ext_f, const T* ext_t, const T* noise, double dt, double kT, double U0, double b, double tol,
+                   cudaStream_t st)
+{
+    const int64_t n3 = 3 * h->N;
+    const size_t bytes = (size_t)n3 * sizeof(T);
+    int rc;
+    for (int k = 0; k < 6; ++k)
+        if ((rc = ensure(h, &h->bd[k], &h->bd_bytes[k], bytes)) != LM_OK) return rc;
+    T *F = (T*)h->bd[0], *vn = (T*)h->bd[1], *vprev = (T*)h->bd[2], *y = (T*)h->bd[3], *ang = (T*)h->bd[4], *yang = (T*)h->bd[5];
+    if ((rc = set_positions_t<T>(h, pos, st)) != LM_OK) return rc;
+    // F^n = steric(X^n) + external;  v_n = M^n [F^n; T]
+    const bool have_force = U0 != 0.0 || ext_f;
+    if (U0 != 0.0) {
+        if ((rc = steric_device<T>(h, U0, b, ext_f, F, st)) != LM_OK) return rc;
+    }
+    const T* Fin = U0 != 0.0 ? F : ext_f;
+    if (have_force || ext_t) {
+        if ((rc = apply_batch<T>(h, 1, Fin, ext_t, vn, h->angular ? ang : nullptr, st)) != LM_OK) return rc;
+    } else {
+        LM_CUDA(h, cudaMemsetAsync(vn, 0, bytes, st));
+    }
+    int rc_noise = LM_OK;
+    const bool noisy = noise && kT > 0.0;
+    if (noisy) {
+        rc_noise = lanczos_device<T>(h, noise, tol, y, h->angular ? yang : nullptr, 1.0, 0, st);
+        if (rc_noise != LM_OK && rc_noise != LM_E_NOCONV) return rc_noise;
+    }
+    const double cn = h->bd_have_prev ? 1.5 : 1.0, cp = h->bd_have_prev ? 0.5 : 0.0;
+    bd_update_kernel<T><<<grid_1d(n3), VEC_BLOCK, 0, st>>>(pos, vn, vprev, noisy ? y : nullptr, n3, (T)(dt * cn), (T)(dt * cp),
+                                                           (T)std::sqrt(2.0 * kT * dt));
+    h->n_aux++;
+    LM_CUDA(h, cudaGetLastError());
+    h->bd_have_prev = true;
+    h->have_pos = false;       // the packed copy now holds X^n, not the caller's X^{n+1}
+    return rc_noise;
+}
+
 // ---------------------------------------------------------------- typed front ends
 template <typename T> int set_positions_t(lm_solver* h, const void* pos, cudaStream_t st)
 {
@@ -566,6 +646,7 @@ int lm_destroy(lm_solver* h)
     if (h->h_gram) cudaFreeHost(h->h_gram);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     for (void* p : h->st) cudaFree(p);
+    for (void* p : h->bd) cudaFree(p);
     for (auto& pr : h->pending) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
     for (auto e : h->event_pool) cudaEventDestroy(e);
     cudaGetLastError();
@@ -707,6 +788,65 @@ int lm_sqrt_mdot_w_host(lm_solver* h, const void* noise, double tol, void* lin_o
     if (h && !noise) { h->err.clear(); return fail(h, LM_E_NULL, "noise is NULL"); }
     const int rc = lm_hydrodynamic_velocities_host(h, nullptr, nullptr, noise, 1.0, tol, lin_out, ang_out, stream);
     if (iters_out && h) *iters_out = h->last_iters;
+    return rc;
+}
+
+// ---------------------------------------------------------------- Brownian-dynamics step (eqs. (13), (14))
+int lm_steric_forces(lm_solver* h, double U0, double b, const void* ext_forces, void* forces_out, void* stream)
+{
+    if (!h) return LM_E_NULL;
+    h->err.clear();
+    if (!h->have_pos) return fail(h, LM_E_NOPOS, "positions not set: call lm_set_positions first");
+    if (!forces_out) return fail(h, LM_E_NULL, "forces_out is NULL");
+    if (!(b > 0.0) || !std::isfinite(b) || !std::isfinite(U0)) return fail(h, LM_E_INVALID, "steric potential needs b > 0 and finite U0");
+    cudaStream_t st = (cudaStream_t)stream;
+    return h->precision == LM_F32 ? steric_device<float>(h, U0, b, (const float*)ext_forces, (float*)forces_out, st)
+                                  : steric_device<double>(h, U0, b, (const double*)ext_forces, (double*)forces_out, st);
+}
+
+int lm_bd_reset(lm_solver* h)
+{
+    if (!h) return LM_E_NULL;
+    h->bd_have_prev = false;
+    return LM_OK;
+}
+
+int lm_bd_step(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise, double dt, double kT, double U0,
+               double b, double tol, void* stream)
+{
+    if (!h) return LM_E_NULL;
+    h->err.clear();
+    if (!pos) return fail(h, LM_E_NULL, "pos is NULL");
+    if (!h->angular && ext_torques) return fail(h, LM_E_ANGULAR, "torques given but the solver was created with include_angular = 0");
+    if (!(dt > 0.0) || !std::isfinite(dt) || !(kT >= 0.0) || !std::isfinite(kT)) return fail(h, LM_E_INVALID, "dt must be > 0 and kT >= 0");
+    if (U0 != 0.0 && (!(b > 0.0) || !std::isfinite(b) || !std::isfinite(U0))) return fail(h, LM_E_INVALID, "steric potential needs b > 0 and finite U0");
+    if (noise && kT > 0.0 && (!(tol > 0.0) || !std::isfinite(tol))) return fail(h, LM_E_INVALID, "tol must be > 0");
+    cudaStream_t st = (cudaStream_t)stream;
+    return h->precision == LM_F32
+               ? bd_step_device<float>(h, (float*)pos, (const float*)ext_forces, (const float*)ext_torques, (const float*)noise, dt, kT, U0, b, tol, st)
+               : bd_step_device<double>(h, (double*)pos, (const double*)ext_forces, (const double*)ext_torques, (const double*)noise, dt, kT, U0, b, tol, st);
+}
+
+int lm_bd_step_host(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise, double dt, double kT,
+                    double U0, double b, double tol, void* stream)
+{
+    if (!h) return LM_E_NULL;
+    h->err.clear();
+    if (!pos) return fail(h, LM_E_NULL, "pos is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)3 * h->N * esize(h);
+    void *dp = nullptr, *df, *dt_, *dn;
+    int rc = ensure(h, &h->bd[6], &h->bd_bytes[6], bytes);
+    if (rc != LM_OK) return rc;
+    dp = h->bd[6];
+    LM_CUDA(h, cudaMemcpyAsync(dp, pos, bytes, cudaMemcpyHostToDevice, st));
+    if ((rc = stage_in(h, 1, ext_forces, bytes, st, &df)) != LM_OK) return rc;
+    if ((rc = stage_in(h, 2, ext_torques, bytes, st, &dt_)) != LM_OK) return rc;
+    if ((rc = stage_in(h, 3, noise, (size_t)dof_of(h) * esize(h), st, &dn)) != LM_OK) return rc;
+    rc = lm_bd_step(h, dp, df, dt_, dn, dt, kT, U0, b, tol, stream);
+    if (rc != LM_OK && rc != LM_E_NOCONV) return rc;
+    LM_CUDA(h, cudaMemcpyAsync(pos, dp, bytes, cudaMemcpyDeviceToHost, st));
+    LM_CUDA(h, cudaStreamSynchronize(st));
     return rc;
 }
 
