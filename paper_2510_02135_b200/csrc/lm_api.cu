@@ -103,7 +103,8 @@ struct lm_solver {
     double* h_scal = nullptr;  // pinned, 4 doubles
     double* d_gram = nullptr;  // Gram column V[j].V[k], j <= k
     double* d_gram_part = nullptr;
-    double* h_gram = nullptr;  // pinned
+    double* h_gram = nullptr;  // pinned, two slots (iteration parity)
+    cudaEvent_t lz_ev[2] = {nullptr, nullptr};   // iteration k's scalars have landed in the pinned slot k & 1
 
     // Brownian-dynamics step (lm_bd_step): F, v_n, v_{n-1}, noise velocity, angular scratch x2, position staging
     void* bd[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -305,7 +306,7 @@ template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& i
     h->n_pair++;
     h->pairs += (double)h->N * (double)h->N;
     if (plan.j_splits > 1) {
-        reduce_partials_kernel<T><<<grid_1d(h->N), VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc, h->N, h->npad, out);
+        reduce_partials_kernel<T><<<dim3(grid_1d(h->N), nrhs * nc), VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc, h->N, h->npad, out);
         h->n_aux++;
     }
     LM_CUDA(h, cudaGetLastError());
@@ -350,7 +351,8 @@ int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_
         LM_CUDA(h, cudaMalloc((void**)&h->d_block, RED_MAX_BLOCKS * sizeof(double)));
         LM_CUDA(h, cudaMalloc((void**)&h->d_ticket, sizeof(unsigned int)));
         LM_CUDA(h, cudaMemsetAsync(h->d_ticket, 0, sizeof(unsigned int), st));
-        LM_CUDA(h, cudaMallocHost((void**)&h->h_scal, 4 * sizeof(double)));
+        LM_CUDA(h, cudaMallocHost((void**)&h->h_scal, 8 * sizeof(double)));   // [0] |z|^2, [2 + 2p], [3 + 2p]: alpha, beta^2 of parity p
+        for (auto& e : h->lz_ev) LM_CUDA(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
     if (h->coef_cap < (size_t)(kmax + 2)) {
         if (h->d_coef) { LM_CUDA(h, cudaFree(h->d_coef)); LM_CUDA(h, cudaFree(h->d_gram)); LM_CUDA(h, cudaFree(h->d_gram_part)); LM_CUDA(h, cudaFreeHost(h->h_gram)); }
@@ -359,7 +361,7 @@ int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_
         LM_CUDA(h, cudaMalloc((void**)&h->d_coef, (size_t)(kmax + 2) * sizeof(double)));
         LM_CUDA(h, cudaMalloc((void**)&h->d_gram, (size_t)(kmax + 2) * sizeof(double)));
         LM_CUDA(h, cudaMalloc((void**)&h->d_gram_part, (size_t)(kmax + 2) * GRAM_MAX_BLOCKS * sizeof(double)));
-        LM_CUDA(h, cudaMallocHost((void**)&h->h_gram, (size_t)(kmax + 2) * sizeof(double)));
+        LM_CUDA(h, cudaMallocHost((void**)&h->h_gram, (size_t)2 * (kmax + 2) * sizeof(double)));
         h->coef_cap = (size_t)(kmax + 2);
     }
     T* V = (T*)h->V;
@@ -370,12 +372,15 @@ int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_
     // Gram matrix of the basis, G[i][j] = V[i].V[j], filled one column per new basis vector
     std::vector<double> G((size_t)(kmax + 1) * (kmax + 1), 0.0);
     const int ldg = kmax + 1;
-    auto gram_launch = [&](int m) {   // column m: V[j].V[m], j <= m  -> pinned h_gram
-        gram_column_kernel<T><<<gg, VEC_BLOCK, 0, st>>>(V, dof, m, gchunk, h->d_gram_part, h->d_ticket, h->d_gram);
+    auto gram_launch = [&](int m) {   // column m: V[j].V[m], j <= m  -> pinned h_gram slot (m & 1)
+        gram_column_kernel<T><<<dim3(gg, m + 1), VEC_BLOCK, 0, st>>>(V, dof, m, gchunk, h->d_gram_part, h->d_ticket, h->d_gram);
         h->n_aux++;
-        return cudaMemcpyAsync(h->h_gram, h->d_gram, (size_t)(m + 1) * sizeof(double), cudaMemcpyDeviceToHost, st);
+        return cudaMemcpyAsync(h->h_gram + (size_t)(m & 1) * (kmax + 2), h->d_gram, (size_t)(m + 1) * sizeof(double), cudaMemcpyDeviceToHost, st);
     };
-    auto gram_store = [&](int m) { for (int j = 0; j <= m; ++j) G[(size_t)j * ldg + m] = G[(size_t)m * ldg + j] = h->h_gram[j]; };
+    auto gram_store = [&](int m) {
+        const double* col = h->h_gram + (size_t)(m & 1) * (kmax + 2);
+        for (int j = 0; j <= m; ++j) G[(size_t)j * ldg + m] = G[(size_t)m * ldg + j] = col[j];
+    };
 
     // v_1 = z / |z|
     sumsq_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise, dof, h->d_block, h->d_ticket, h->d_scal + 0);
@@ -395,12 +400,10 @@ int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_
         return LM_OK;
     }
 
-    std::vector<double> alphas, betas, c_prev, c_cur;
-    bool converged = false;
-    const bool debug = std::getenv("LM_DEBUG_LANCZOS") != nullptr;   // per-iteration trace on stderr
-    const double breakdown = (h->precision == LM_F32) ? 1e-6 : 1e-14;
-    int k = 0;
-    for (k = 1; k <= kmax; ++k) {
+    // Iteration k on the device: w = M v_k; w -= beta_{k-1} v_{k-1}; alpha_k; w -= alpha_k v_k; beta_k^2;
+    // v_{k+1} = w / beta_k; Gram column k.  Everything the device needs stays on the device; the host only
+    // READS (alpha_k, beta_k^2, Gram column) for the stopping test, from the pinned slot of parity k & 1.
+    auto enqueue = [&](int k) -> int {
         T* vk = V + (size_t)(k - 1) * dof;
         RhsIn<T> in{};
         RhsOut<T> out{};
@@ -408,20 +411,45 @@ int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_
         in.t[0] = h->angular ? vk + n3 : nullptr;
         out.lin[0] = w;
         out.ang[0] = h->angular ? w + n3 : nullptr;
-        if ((rc = apply_device<T>(h, 1, in, out, st)) != LM_OK) return rc;          // w = M v_k
+        int rc2;
+        if ((rc2 = apply_device<T>(h, 1, in, out, st)) != LM_OK) return rc2;          // w = M v_k
         lanczos_alpha_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(w, vk, k > 1 ? vk - dof : nullptr, h->d_scal + 2, dof, h->d_block, h->d_ticket,
                                                           h->d_scal + 1);           // w -= beta_{k-1} v_{k-1}; alpha_k
         lanczos_beta_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(w, vk, h->d_scal + 1, dof, h->d_block, h->d_ticket, h->d_scal + 2);  // w -= alpha v; beta^2
-        LM_CUDA(h, cudaMemcpyAsync(h->h_scal + 1, h->d_scal + 1, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        LM_CUDA(h, cudaMemcpyAsync(h->h_scal + 2 + 2 * (k & 1), h->d_scal + 1, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
         scale_by_inv_norm_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(w, dof, h->d_scal + 2, vk + dof);    // v_{k+1} = w / beta_k
         h->n_aux += 3;
         if (k < kmax) LM_CUDA(h, gram_launch(k));                                                  // V[k] = v_{k+1} against V[0..k]
-        LM_CUDA(h, cudaStreamSynchronize(st));
-        const double alpha = h->h_scal[1], beta = std::sqrt(std::max(h->h_scal[2], 0.0));
-        if (!std::isfinite(alpha) || !std::isfinite(beta)) return fail(h, LM_E_CUDA, "Lanczos: non-finite alpha/beta (non-finite input?)");
+        LM_CUDA(h, cudaEventRecord(h->lz_ev[k & 1], st));
+        return LM_OK;
+    };
+    // One iteration of look-ahead when an apply is short: iteration k+1 is enqueued BEFORE the host waits
+    // for iteration k's scalars, so the device never idles on the host round trip (~70 us per iteration:
+    // launches + copy + synchronise).  The price is one wasted apply at convergence, so it is used only
+    // where an apply costs less than the round trips it saves (~25 iterations x 50 us).
+    const double apply_cost = (double)h->N * (double)h->N * (h->angular ? 2.3 : 1.0) * (h->precision == LM_F64 ? 2.5 : 1.0);
+    const bool lookahead = apply_cost < 2.0e9;
+
+    std::vector<double> alphas, betas, c_prev, c_cur;
+    bool converged = false;
+    const bool debug = std::getenv("LM_DEBUG_LANCZOS") != nullptr;   // per-iteration trace on stderr
+    const double breakdown = (h->precision == LM_F32) ? 1e-6 : 1e-14;
+    int k = 0;
+    if ((rc = enqueue(1)) != LM_OK) return rc;
+    for (k = 1; k <= kmax; ++k) {
+        if (lookahead && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
+        LM_CUDA(h, cudaEventSynchronize(h->lz_ev[k & 1]));
+        const double alpha = h->h_scal[2 + 2 * (k & 1)], beta = std::sqrt(std::max(h->h_scal[3 + 2 * (k & 1)], 0.0));
+        if (!std::isfinite(alpha) || !std::isfinite(beta)) {
+            cudaStreamSynchronize(st);
+            return fail(h, LM_E_CUDA, "Lanczos: non-finite alpha/beta (non-finite input?)");
+        }
         alphas.push_back(alpha);
         c_cur.assign(k, 0.0);
-        if (!tridiag_sqrt_e1(k, alphas.data(), betas.data(), c_cur.data())) return fail(h, LM_E_NOCONV, "Lanczos: tridiagonal eigensolve did not converge");
+        if (!tridiag_sqrt_e1(k, alphas.data(), betas.data(), c_cur.data())) {
+            cudaStreamSynchronize(st);
+            return fail(h, LM_E_NOCONV, "Lanczos: tridiagonal eigensolve did not converge");
+        }
         if (k >= 2) {
             // |y_k - y_{k-1}|^2 / |z|^2 = delta^T G_k delta,  |y_{k-1}|^2 / |z|^2 = c_{k-1}^T G_{k-1} c_{k-1}
             std::vector<double> delta(c_cur);
@@ -439,6 +467,7 @@ int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_
         if (k < kmax) gram_store(k);
         betas.push_back(beta);
         c_prev = c_cur;
+        if (!lookahead && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
     }
     if (k > kmax) k = kmax;
     h->last_iters = k;
@@ -647,6 +676,7 @@ int lm_destroy(lm_solver* h)
     if (h->h_scal) cudaFreeHost(h->h_scal);
     for (void* p : h->st) cudaFree(p);
     for (void* p : h->bd) cudaFree(p);
+    for (auto e : h->lz_ev) if (e) cudaEventDestroy(e);
     for (auto& pr : h->pending) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
     for (auto e : h->event_pool) cudaEventDestroy(e);
     cudaGetLastError();

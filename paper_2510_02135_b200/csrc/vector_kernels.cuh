@@ -42,22 +42,29 @@ __global__ void __launch_bounds__(VEC_BLOCK) pack_rhs_kernel(RhsIn<T> in, int nr
 }
 
 // a6: sum the j-split partials in a fixed order (deterministic) and write interleaved outputs.
+// One thread per (right-hand side, component, particle): consecutive threads read consecutive
+// addresses of one partial array; the loads of the splits are independent and unrolled.
 template <typename T>
 __global__ void __launch_bounds__(VEC_BLOCK) reduce_partials_kernel(const T* __restrict__ partial, int splits, int nrhs, int nc, int64_t N,
                                                                     int64_t npad, RhsOut<T> out)
 {
     const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
     if (i >= N) return;
+    const int qk = blockIdx.y, q = qk / nc, k = qk % nc;
     const size_t stride = (size_t)nrhs * nc * npad;
-    for (int q = 0; q < nrhs; ++q) {
-        for (int k = 0; k < nc; ++k) {
-            const T* p = partial + (size_t)(q * nc + k) * npad + i;
-            T s = T(0);
-            for (int sidx = 0; sidx < splits; ++sidx) s += p[sidx * stride];
-            if (k < 3) out.lin[q][3 * i + k] = s;
-            else       out.ang[q][3 * i + (k - 3)] = s;
-        }
+    const T* p = partial + (size_t)qk * npad + i;
+    T s = T(0);
+    int sidx = 0;
+    for (; sidx + 8 <= splits; sidx += 8) {
+        T v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = p[(size_t)(sidx + u) * stride];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) s += v[u];
     }
+    for (; sidx < splits; ++sidx) s += p[(size_t)sidx * stride];
+    if (k < 3) out.lin[q][3 * i + k] = s;
+    else       out.ang[q][3 * i + (k - 3)] = s;
 }
 
 // ---------------------------------------------------------------- Lanczos vector operations (a7)
@@ -157,7 +164,8 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__
 // Gram column for the stopping test (a9): g[j] = V[j] . V[k], j = 0..k.  Lanczos without
 // re-orthogonalisation loses orthogonality of V, so |y_k - y_{k-1}| = |z| |V_k delta| is evaluated as
 // sqrt(delta^T G delta) with the true Gram matrix G = V^T V instead of assuming G = I.
-// Block b owns the contiguous index range [b*chunk, (b+1)*chunk); partials are [j][block].
+// Grid (chunks, k+1): block (b, j) forms the part of V[j] . V[k] over the index range [b*chunk, (b+1)*chunk);
+// the last block to finish (ticket) adds the partials [j][b] in index order: deterministic.
 constexpr int GRAM_MAX_BLOCKS = 128;
 template <typename T>
 __global__ void __launch_bounds__(VEC_BLOCK) gram_column_kernel(const T* __restrict__ V, int64_t dof, int k, int64_t chunk, double* partials,
@@ -165,34 +173,30 @@ __global__ void __launch_bounds__(VEC_BLOCK) gram_column_kernel(const T* __restr
 {
     __shared__ double warp_part[VEC_BLOCK / 32];
     __shared__ bool is_last;
+    const int j = blockIdx.y;
     const int64_t lo_i = (int64_t)blockIdx.x * chunk, hi_i = min(lo_i + chunk, dof);
     const T* vk = V + (size_t)k * dof;
-    for (int j = 0; j <= k; ++j) {
-        const T* vj = V + (size_t)j * dof;
-        double s = 0.0;
-        for (int64_t i = lo_i + threadIdx.x; i < hi_i; i += VEC_BLOCK) s = fma((double)vj[i], (double)vk[i], s);
-        s = warp_sum(s);
-        if ((threadIdx.x & 31) == 0) warp_part[threadIdx.x >> 5] = s;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double t = 0.0;
-#pragma unroll
-            for (int w = 0; w < VEC_BLOCK / 32; ++w) t += warp_part[w];
-            partials[(size_t)j * gridDim.x + blockIdx.x] = t;
-        }
-        __syncthreads();
-    }
+    const T* vj = V + (size_t)j * dof;
+    double s = 0.0;
+    for (int64_t i = lo_i + threadIdx.x; i < hi_i; i += VEC_BLOCK) s = fma((double)vj[i], (double)vk[i], s);
+    s = warp_sum(s);
+    if ((threadIdx.x & 31) == 0) warp_part[threadIdx.x >> 5] = s;
+    __syncthreads();
     if (threadIdx.x == 0) {
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < VEC_BLOCK / 32; ++w) t += warp_part[w];
+        partials[(size_t)j * gridDim.x + blockIdx.x] = t;
         __threadfence();
-        is_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+        is_last = (atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1);
     }
     __syncthreads();
     if (is_last) {
         __threadfence();
-        for (int j = threadIdx.x; j <= k; j += VEC_BLOCK) {
+        for (int jj = threadIdx.x; jj <= k; jj += VEC_BLOCK) {
             double t = 0.0;
-            for (unsigned int b = 0; b < gridDim.x; ++b) t += ((volatile double*)partials)[(size_t)j * gridDim.x + b];
-            g[j] = t;
+            for (unsigned int b = 0; b < gridDim.x; ++b) t += ((volatile double*)partials)[(size_t)jj * gridDim.x + b];
+            g[jj] = t;
         }
         if (threadIdx.x == 0) *ticket = 0u;
     }
