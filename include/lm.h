@@ -141,7 +141,9 @@ int lm_bd_step_host(lm_solver* h, void* pos, const void* ext_forces, const void*
                     double dt, double kT, double U0, double b, double tol, void* stream);
 int lm_bd_reset(lm_solver* h);                        /* forget the Adams-Bashforth history */
 
-/* Lanczos controls and introspection. */
+/* Lanczos controls and introspection.  Diagnostics through the environment (read at call time):
+ * LM_DEBUG_LANCZOS=1 prints alpha_k, beta_k and the relative step of every iteration on stderr;
+ * LM_NO_GRAPH=1 launches the iteration's kernels one by one instead of replaying the captured CUDA graph. */
 int lm_set_max_iter(lm_solver* h, int max_iter);     /* default 100; 1 <= max_iter <= 1000 */
 int lm_last_iterations(const lm_solver* h);           /* iterations of the last Lanczos call (or < 0) */
 const char* lm_last_error(const lm_solver* h);        /* never NULL; "" if the last call succeeded */

@@ -99,12 +99,17 @@ struct lm_solver {
     double* d_scal = nullptr;  // [0] |z|^2  [1] alpha  [2] beta^2
     double* d_block = nullptr; // block partials of the reductions
     unsigned int* d_ticket = nullptr;
-    double* d_coef = nullptr;  size_t coef_cap = 0;   // coef_cap also sizes the Gram buffers below
-    double* h_scal = nullptr;  // pinned, 4 doubles
-    double* d_gram = nullptr;  // Gram column V[j].V[k], j <= k
+    int* d_newest = nullptr;   // index of the newest basis vector (read by the iteration's kernels)
+    double* d_coef = nullptr;  size_t coef_cap = 0;   // coef_cap also sizes the buffers below
     double* d_gram_part = nullptr;
-    double* h_gram = nullptr;  // pinned, two slots (iteration parity)
-    cudaEvent_t lz_ev[2] = {nullptr, nullptr};   // iteration k's scalars have landed in the pinned slot k & 1
+    // mapped pinned host memory the kernels write the stopping-test scalars into
+    double* h_ab = nullptr;    // [1] |z|^2; [2k], [2k+1]: alpha_k, beta_k^2
+    double* h_gram = nullptr;  // column c at [c * (max_iter + 2) + j] = V[j].V[c], j <= c
+    cudaEvent_t lz_ev[2] = {nullptr, nullptr};   // iteration k's scalars have landed (parity k & 1)
+    // one Lanczos iteration captured as a CUDA graph (small N: the loop is launch-bound)
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t lz_graph = nullptr;
+    struct GraphKey { const void *V, *w, *vec, *partial, *pos; int kmax, variant, splits, prec; } lz_key = {nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0};
 
     // Brownian-dynamics step (lm_bd_step): F, v_n, v_{n-1}, noise velocity, angular scratch x2, position staging
     void* bd[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -212,12 +217,9 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
     const auto& vs = variants<T>(h);
     LaunchPlan best;
     double best_cost = 1e300;
-    int dbg_block = 0, dbg_splits = 0;                       // TUNING ONLY
-    if (const char* e = std::getenv("LM_PLAN")) std::sscanf(e, "%d,%d", &dbg_block, &dbg_splits);
     for (int vi = 0; vi < (int)vs.size(); ++vi) {
         const auto& v = vs[vi];
         if (v.nrhs != nrhs || v.ang != h->angular) continue;
-        if (dbg_block && v.block != dbg_block) continue;
         const int targets = v.block * v.tpt;
         const int i_tiles = (int)((h->N + targets - 1) / targets);
         const int units = (int)(h->npad / v.sub);
@@ -225,7 +227,6 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
         const int max_splits = std::min(units, 256);
         const int min_splits = (int)std::min<int64_t>(max_splits, (h->npad + MAX_SOURCES_PER_CTA - 1) / MAX_SOURCES_PER_CTA);
         for (int s = min_splits; s <= max_splits; ++s) {
-            if (dbg_splits && s != std::min(dbg_splits, max_splits)) continue;
             const int64_t src = (int64_t)((units + s - 1) / s) * v.sub;            // sources of the largest split
             const int64_t ctas = (int64_t)i_tiles * s;
             const int64_t full = ctas / slots, rem = ctas % slots;
@@ -266,22 +267,26 @@ int grid_1d(int64_t n) { return (int)std::max<int64_t>(1, (n + VEC_BLOCK - 1) / 
 int grid_red(int64_t n) { return (int)std::min<int64_t>(RED_MAX_BLOCKS, std::max<int64_t>(1, (n + VEC_BLOCK - 1) / VEC_BLOCK)); }
 
 // ---------------------------------------------------------------- device apply: out = M . rhs  (nrhs <= MAX_RHS)
-template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& in, const RhsOut<T>& out, cudaStream_t st)
+// prepare_apply: choose the launch plan and size the packed right-hand side and the partials (no launches)
+template <typename T> int prepare_apply(lm_solver* h, int nrhs, LaunchPlan& plan)
 {
     const int nc = h->angular ? 6 : 3;
-    const LaunchPlan plan = choose_plan<T>(h, nrhs);
+    plan = choose_plan<T>(h, nrhs);
     if (plan.variant < 0) return fail(h, LM_E_INVALID, "no pair-kernel variant for this nrhs");
-    const auto& v = variants<T>(h)[plan.variant];
-
     int rc = ensure(h, &h->vec_soa, &h->vec_soa_bytes, (size_t)nrhs * nc * h->npad * sizeof(T));
     if (rc != LM_OK) return rc;
     if (plan.j_splits > 1) {
         rc = ensure(h, &h->partial, &h->partial_bytes, (size_t)plan.j_splits * nrhs * nc * h->npad * sizeof(T));
         if (rc != LM_OK) return rc;
     }
-    pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>(in, nrhs, nc, h->N, h->npad, (T*)h->vec_soa);
-    h->n_aux++;
+    return LM_OK;
+}
 
+// launch_pair: the pair kernel on the packed right-hand side already in h->vec_soa, then the split-j reduce
+template <typename T> int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>& out, cudaStream_t st, bool timed)
+{
+    const int nc = h->angular ? 6 : 3;
+    const auto& v = variants<T>(h)[plan.variant];
     PairParams<T> p;
     p.pos = (const T*)h->pos_soa;
     p.vec = (const T*)h->vec_soa;
@@ -293,23 +298,39 @@ template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& i
     p.c = make_consts<T>(h->eta, h->a);
 
     cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (h->profiling) {
+    if (timed) {
         e0 = get_event(h);
         e1 = get_event(h);
         LM_CUDA(h, cudaEventRecord(e0, st));
     }
     v.kernel<<<dim3(plan.i_tiles, plan.j_splits), v.block, v.smem, st>>>(p);
-    if (h->profiling) {
+    if (timed) {
         LM_CUDA(h, cudaEventRecord(e1, st));
         h->pending.emplace_back(e0, e1);
     }
+    if (plan.j_splits > 1)
+        reduce_partials_kernel<T><<<dim3(grid_1d(h->N), nrhs * nc), VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc, h->N, h->npad, out);
+    LM_CUDA(h, cudaGetLastError());
+    return LM_OK;
+}
+
+void count_apply(lm_solver* h, const LaunchPlan& plan)
+{
     h->n_pair++;
     h->pairs += (double)h->N * (double)h->N;
-    if (plan.j_splits > 1) {
-        reduce_partials_kernel<T><<<dim3(grid_1d(h->N), nrhs * nc), VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc, h->N, h->npad, out);
-        h->n_aux++;
-    }
-    LM_CUDA(h, cudaGetLastError());
+    if (plan.j_splits > 1) h->n_aux++;
+}
+
+template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& in, const RhsOut<T>& out, cudaStream_t st)
+{
+    const int nc = h->angular ? 6 : 3;
+    LaunchPlan plan;
+    int rc = prepare_apply<T>(h, nrhs, plan);
+    if (rc != LM_OK) return rc;
+    pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>(in, nrhs, nc, h->N, h->npad, (T*)h->vec_soa);
+    h->n_aux++;
+    if ((rc = launch_pair<T>(h, nrhs, plan, out, st, h->profiling)) != LM_OK) return rc;
+    count_apply(h, plan);
     return LM_OK;
 }
 
@@ -342,7 +363,9 @@ template <typename T>
 int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_out, double scale, int accumulate, cudaStream_t st)
 {
     const int64_t dof = dof_of(h), n3 = 3 * h->N;
+    const int nc = h->angular ? 6 : 3;
     const int kmax = h->max_iter;
+    const int ld = kmax + 2;
     int rc;
     if ((rc = ensure(h, &h->V, &h->V_bytes, (size_t)(kmax + 1) * dof * sizeof(T))) != LM_OK) return rc;
     if ((rc = ensure(h, &h->w, &h->w_bytes, (size_t)dof * sizeof(T))) != LM_OK) return rc;
@@ -350,47 +373,51 @@ int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_
         LM_CUDA(h, cudaMalloc((void**)&h->d_scal, 4 * sizeof(double)));
         LM_CUDA(h, cudaMalloc((void**)&h->d_block, RED_MAX_BLOCKS * sizeof(double)));
         LM_CUDA(h, cudaMalloc((void**)&h->d_ticket, sizeof(unsigned int)));
+        LM_CUDA(h, cudaMalloc((void**)&h->d_newest, sizeof(int)));
         LM_CUDA(h, cudaMemsetAsync(h->d_ticket, 0, sizeof(unsigned int), st));
-        LM_CUDA(h, cudaMallocHost((void**)&h->h_scal, 8 * sizeof(double)));   // [0] |z|^2, [2 + 2p], [3 + 2p]: alpha, beta^2 of parity p
         for (auto& e : h->lz_ev) LM_CUDA(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        LM_CUDA(h, cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
     }
     if (h->coef_cap < (size_t)(kmax + 2)) {
-        if (h->d_coef) { LM_CUDA(h, cudaFree(h->d_coef)); LM_CUDA(h, cudaFree(h->d_gram)); LM_CUDA(h, cudaFree(h->d_gram_part)); LM_CUDA(h, cudaFreeHost(h->h_gram)); }
+        if (h->d_coef) { LM_CUDA(h, cudaFree(h->d_coef)); LM_CUDA(h, cudaFree(h->d_gram_part)); LM_CUDA(h, cudaFreeHost(h->h_gram)); LM_CUDA(h, cudaFreeHost(h->h_ab)); }
         h->d_coef = nullptr;
         h->coef_cap = 0;
         LM_CUDA(h, cudaMalloc((void**)&h->d_coef, (size_t)(kmax + 2) * sizeof(double)));
-        LM_CUDA(h, cudaMalloc((void**)&h->d_gram, (size_t)(kmax + 2) * sizeof(double)));
         LM_CUDA(h, cudaMalloc((void**)&h->d_gram_part, (size_t)(kmax + 2) * GRAM_MAX_BLOCKS * sizeof(double)));
-        LM_CUDA(h, cudaMallocHost((void**)&h->h_gram, (size_t)2 * (kmax + 2) * sizeof(double)));
+        LM_CUDA(h, cudaHostAlloc((void**)&h->h_gram, (size_t)ld * ld * sizeof(double), cudaHostAllocMapped));
+        LM_CUDA(h, cudaHostAlloc((void**)&h->h_ab, (size_t)2 * ld * sizeof(double), cudaHostAllocMapped));
         h->coef_cap = (size_t)(kmax + 2);
     }
     T* V = (T*)h->V;
     T* w = (T*)h->w;
+    volatile const double* ab = h->h_ab;
+    volatile const double* hg = h->h_gram;
     const int gr = grid_red(dof);
     const int gg = (int)std::min<int64_t>(GRAM_MAX_BLOCKS, std::max<int64_t>(1, dof / (4 * VEC_BLOCK)));
     const int64_t gchunk = (dof + gg - 1) / gg;
+    LaunchPlan plan;
+    if ((rc = prepare_apply<T>(h, 1, plan)) != LM_OK) return rc;
+    T* soa = (T*)h->vec_soa;
     // Gram matrix of the basis, G[i][j] = V[i].V[j], filled one column per new basis vector
     std::vector<double> G((size_t)(kmax + 1) * (kmax + 1), 0.0);
     const int ldg = kmax + 1;
-    auto gram_launch = [&](int m) {   // column m: V[j].V[m], j <= m  -> pinned h_gram slot (m & 1)
-        gram_column_kernel<T><<<dim3(gg, m + 1), VEC_BLOCK, 0, st>>>(V, dof, m, gchunk, h->d_gram_part, h->d_ticket, h->d_gram);
-        h->n_aux++;
-        return cudaMemcpyAsync(h->h_gram + (size_t)(m & 1) * (kmax + 2), h->d_gram, (size_t)(m + 1) * sizeof(double), cudaMemcpyDeviceToHost, st);
-    };
-    auto gram_store = [&](int m) {
-        const double* col = h->h_gram + (size_t)(m & 1) * (kmax + 2);
-        for (int j = 0; j <= m; ++j) G[(size_t)j * ldg + m] = G[(size_t)m * ldg + j] = col[j];
+    auto gram_store = [&](int m) { for (int j = 0; j <= m; ++j) G[(size_t)j * ldg + m] = G[(size_t)m * ldg + j] = hg[(size_t)m * ld + j]; };
+    // new basis vector V[*newest + 1] = x / sqrt(*sumsq) (+ its packed copy for the next apply), its Gram column, *newest += 1
+    auto new_vector = [&](const T* x, const double* sumsq, cudaStream_t s2) {
+        lanczos_scale_pack_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(x, h->N, h->npad, nc, sumsq, h->d_newest, V, soa);
+        gram_column_kernel<T><<<dim3(gg, kmax + 1), VEC_BLOCK, 0, s2>>>(V, dof, h->d_newest, gchunk, h->d_gram_part, h->d_ticket, h->h_gram, ld);
+        lanczos_advance_kernel<<<1, 1, 0, s2>>>(h->d_newest);
     };
 
     // v_1 = z / |z|
-    sumsq_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise, dof, h->d_block, h->d_ticket, h->d_scal + 0);
-    scale_by_inv_norm_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise, dof, h->d_scal + 0, V);
-    h->n_aux += 2;
-    LM_CUDA(h, cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(double), cudaMemcpyDeviceToHost, st));
-    LM_CUDA(h, gram_launch(0));
+    LM_CUDA(h, cudaMemsetAsync(h->d_newest, 0xff, sizeof(int), st));            // *newest = -1
+    sumsq_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise, dof, h->d_block, h->d_ticket, h->d_scal + 0, h->h_ab + 1);
+    new_vector(noise, h->d_scal + 0, st);
+    h->n_aux += 4;
+    LM_CUDA(h, cudaGetLastError());
     LM_CUDA(h, cudaStreamSynchronize(st));
     gram_store(0);
-    const double znorm = std::sqrt(h->h_scal[0]);
+    const double znorm = std::sqrt(ab[1]);
     h->last_iters = 0;
     if (!(znorm > 0.0)) {            // zero noise: M^{1/2} 0 = 0
         if (!accumulate) {
@@ -400,35 +427,58 @@ int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_
         return LM_OK;
     }
 
-    // Iteration k on the device: w = M v_k; w -= beta_{k-1} v_{k-1}; alpha_k; w -= alpha_k v_k; beta_k^2;
-    // v_{k+1} = w / beta_k; Gram column k.  Everything the device needs stays on the device; the host only
-    // READS (alpha_k, beta_k^2, Gram column) for the stopping test, from the pinned slot of parity k & 1.
-    auto enqueue = [&](int k) -> int {
-        T* vk = V + (size_t)(k - 1) * dof;
-        RhsIn<T> in{};
-        RhsOut<T> out{};
-        in.f[0] = vk;
-        in.t[0] = h->angular ? vk + n3 : nullptr;
-        out.lin[0] = w;
-        out.ang[0] = h->angular ? w + n3 : nullptr;
+    // Iteration k on the device, with m = k - 1 = *newest:  w = M v_k;  w -= beta_{k-1} v_{k-1};  alpha_k;
+    // w -= alpha_k v_k;  beta_k^2;  v_{k+1} = w / beta_k (+ packed for the next apply);  Gram column k.
+    // Everything the device needs stays on the device; the host only READS (alpha_k, beta_k^2, Gram column)
+    // from mapped pinned memory for the stopping test.  The launch sequence and its arguments are the
+    // same for every k, so it is captured once as a CUDA graph.
+    RhsOut<T> out{};
+    out.lin[0] = w;
+    out.ang[0] = h->angular ? w + n3 : nullptr;
+    auto body = [&](cudaStream_t s2, bool timed) -> int {
         int rc2;
-        if ((rc2 = apply_device<T>(h, 1, in, out, st)) != LM_OK) return rc2;          // w = M v_k
-        lanczos_alpha_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(w, vk, k > 1 ? vk - dof : nullptr, h->d_scal + 2, dof, h->d_block, h->d_ticket,
-                                                          h->d_scal + 1);           // w -= beta_{k-1} v_{k-1}; alpha_k
-        lanczos_beta_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(w, vk, h->d_scal + 1, dof, h->d_block, h->d_ticket, h->d_scal + 2);  // w -= alpha v; beta^2
-        LM_CUDA(h, cudaMemcpyAsync(h->h_scal + 2 + 2 * (k & 1), h->d_scal + 1, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        scale_by_inv_norm_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(w, dof, h->d_scal + 2, vk + dof);    // v_{k+1} = w / beta_k
-        h->n_aux += 3;
-        if (k < kmax) LM_CUDA(h, gram_launch(k));                                                  // V[k] = v_{k+1} against V[0..k]
-        LM_CUDA(h, cudaEventRecord(h->lz_ev[k & 1], st));
+        if ((rc2 = launch_pair<T>(h, 1, plan, out, s2, timed)) != LM_OK) return rc2;                       // w = M v_k
+        lanczos_alpha_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(w, V, h->d_newest, h->d_scal + 2, dof, h->d_block, h->d_ticket, h->d_scal + 1);
+        lanczos_beta_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(w, V, h->d_newest, h->d_scal + 1, dof, h->d_block, h->d_ticket, h->d_scal + 2, h->h_ab);
+        new_vector(w, h->d_scal + 2, s2);
+        LM_CUDA(h, cudaGetLastError());
         return LM_OK;
     };
     // One iteration of look-ahead when an apply is short: iteration k+1 is enqueued BEFORE the host waits
-    // for iteration k's scalars, so the device never idles on the host round trip (~70 us per iteration:
-    // launches + copy + synchronise).  The price is one wasted apply at convergence, so it is used only
-    // where an apply costs less than the round trips it saves (~25 iterations x 50 us).
+    // for iteration k's scalars, so the device never idles on the host round trip.  The price is one
+    // wasted apply at convergence, so it is used only where an apply costs less than the round trips it
+    // saves (~25 iterations x 50 us); the same regime is launch-bound, so there the body runs as a graph.
     const double apply_cost = (double)h->N * (double)h->N * (h->angular ? 2.3 : 1.0) * (h->precision == LM_F64 ? 2.5 : 1.0);
     const bool lookahead = apply_cost < 2.0e9;
+    const bool use_graph = lookahead && !h->profiling && std::getenv("LM_NO_GRAPH") == nullptr;
+    if (use_graph) {
+        const lm_solver::GraphKey key = {h->V, h->w, h->vec_soa, h->partial, h->pos_soa, kmax, plan.variant, plan.j_splits, h->precision};
+        if (!h->lz_graph || std::memcmp(&key, &h->lz_key, sizeof key) != 0) {
+            if (h->lz_graph) { LM_CUDA(h, cudaGraphExecDestroy(h->lz_graph)); h->lz_graph = nullptr; }
+            cudaGraph_t graph = nullptr;
+            LM_CUDA(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+            const int rc_body = body(h->cap_stream, false);
+            const cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
+            if (rc_body != LM_OK) { if (graph) cudaGraphDestroy(graph); return rc_body; }
+            LM_CUDA(h, ce);
+            const cudaError_t ci = cudaGraphInstantiate(&h->lz_graph, graph, 0);
+            cudaGraphDestroy(graph);
+            LM_CUDA(h, ci);
+            h->lz_key = key;
+        }
+    }
+    auto enqueue = [&](int k) -> int {
+        if (use_graph) {
+            LM_CUDA(h, cudaGraphLaunch(h->lz_graph, st));
+        } else {
+            const int rc2 = body(st, h->profiling);
+            if (rc2 != LM_OK) return rc2;
+        }
+        count_apply(h, plan);
+        h->n_aux += 5;
+        LM_CUDA(h, cudaEventRecord(h->lz_ev[k & 1], st));
+        return LM_OK;
+    };
 
     std::vector<double> alphas, betas, c_prev, c_cur;
     bool converged = false;
@@ -439,7 +489,7 @@ int lanczos_device(lm_solver* h, const T* noise, double tol, T* lin_out, T* ang_
     for (k = 1; k <= kmax; ++k) {
         if (lookahead && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
         LM_CUDA(h, cudaEventSynchronize(h->lz_ev[k & 1]));
-        const double alpha = h->h_scal[2 + 2 * (k & 1)], beta = std::sqrt(std::max(h->h_scal[3 + 2 * (k & 1)], 0.0));
+        const double alpha = ab[2 * k], beta = std::sqrt(std::max((double)ab[2 * k + 1], 0.0));
         if (!std::isfinite(alpha) || !std::isfinite(beta)) {
             cudaStreamSynchronize(st);
             return fail(h, LM_E_CUDA, "Lanczos: non-finite alpha/beta (non-finite input?)");
@@ -670,10 +720,12 @@ int lm_destroy(lm_solver* h)
     cudaFree(h->d_block);
     cudaFree(h->d_ticket);
     cudaFree(h->d_coef);
-    cudaFree(h->d_gram);
     cudaFree(h->d_gram_part);
+    cudaFree(h->d_newest);
     if (h->h_gram) cudaFreeHost(h->h_gram);
-    if (h->h_scal) cudaFreeHost(h->h_scal);
+    if (h->h_ab) cudaFreeHost(h->h_ab);
+    if (h->lz_graph) cudaGraphExecDestroy(h->lz_graph);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     for (void* p : h->st) cudaFree(p);
     for (void* p : h->bd) cudaFree(p);
     for (auto e : h->lz_ev) if (e) cudaEventDestroy(e);

@@ -77,7 +77,8 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-__device__ __forceinline__ void block_reduce_to_scalar(double v, double* block_partials, unsigned int* ticket, double* result)
+__device__ __forceinline__ void block_reduce_to_scalar(double v, double* block_partials, unsigned int* ticket, double* result,
+                                                       double* host_mirror = nullptr)
 {
     __shared__ double warp_part[VEC_BLOCK / 32];
     __shared__ bool is_last;
@@ -99,39 +100,66 @@ __device__ __forceinline__ void block_reduce_to_scalar(double v, double* block_p
         double s = 0.0;
         for (unsigned int b = threadIdx.x; b < gridDim.x; b += 32) s += ((volatile double*)block_partials)[b];
         s = warp_sum(s);
-        if (threadIdx.x == 0) { *result = s; *ticket = 0u; }
+        if (threadIdx.x == 0) {
+            *result = s;
+            if (host_mirror) *host_mirror = s;
+            *ticket = 0u;
+        }
     }
 }
 
 // result = sum_i x_i^2          (|z|^2 of the noise vector)
 template <typename T>
 __global__ void __launch_bounds__(VEC_BLOCK) sumsq_kernel(const T* __restrict__ x, int64_t n, double* block_partials, unsigned int* ticket,
-                                                          double* result)
+                                                          double* result, double* host_mirror)
 {
     double s = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * VEC_BLOCK) {
         const double v = (double)x[i];
         s = fma(v, v, s);
     }
-    block_reduce_to_scalar(s, block_partials, ticket, result);
+    block_reduce_to_scalar(s, block_partials, ticket, result, host_mirror);
 }
 
-// v_out = x / sqrt(*sumsq)     (v_1 = z/|z| and v_{k+1} = w/beta_k)
+// The kernels of one Lanczos iteration read the index m of the NEWEST basis vector V[m] from device
+// memory (`newest`), so that every iteration is the same sequence of launches with the same arguments:
+// the driver captures it once in a CUDA graph and replays it (the loop is launch-bound at small N).
+// Scalars the host needs for the stopping test are written straight into mapped pinned host memory.
+
+// V[*newest + 1] = x / sqrt(*sumsq)  (v_1 = z/|z| with *newest = -1; v_{k+1} = w/beta_k), and the same
+// vector packed as the pair kernel's structure-of-arrays right-hand side (a2) for the next apply:
+// soa[c][i], c < nc, ghosts zero.  x and V hold [3N linear | 3N angular].
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) scale_by_inv_norm_kernel(const T* __restrict__ x, int64_t n, const double* sumsq, T* __restrict__ v_out)
+__global__ void __launch_bounds__(VEC_BLOCK) lanczos_scale_pack_kernel(const T* __restrict__ x, int64_t N, int64_t npad, int nc,
+                                                                       const double* sumsq, const int* __restrict__ newest,
+                                                                       T* __restrict__ V, T* __restrict__ soa)
 {
+    const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
+    if (i >= npad) return;
     const double nrm = sqrt(*sumsq);
     const double inv = nrm > 0.0 ? 1.0 / nrm : 0.0;
-    for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * VEC_BLOCK)
-        v_out[i] = (T)((double)x[i] * inv);
+    const int64_t n3 = 3 * N, dof = (int64_t)nc * N;
+    T* v_out = V + (size_t)(*newest + 1) * dof;
+    for (int c = 0; c < nc; ++c) {
+        T val = T(0);
+        if (i < N) {
+            const int64_t idx = (c < 3 ? 0 : n3) + 3 * i + (c % 3);
+            val = (T)((double)x[idx] * inv);
+            v_out[idx] = val;
+        }
+        soa[(size_t)c * npad + i] = val;
+    }
 }
 
-// w -= sqrt(*beta_prev_sq) * v_prev  (skipped when v_prev == null);  *alpha = w . v
+// v = V[*newest]:  w -= sqrt(*beta_prev_sq) * V[*newest - 1]  (skipped for *newest == 0);  *alpha = w . v
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) lanczos_alpha_kernel(T* __restrict__ w, const T* __restrict__ v, const T* __restrict__ v_prev,
+__global__ void __launch_bounds__(VEC_BLOCK) lanczos_alpha_kernel(T* __restrict__ w, const T* __restrict__ V, const int* __restrict__ newest,
                                                                   const double* beta_prev_sq, int64_t n, double* block_partials,
                                                                   unsigned int* ticket, double* alpha)
 {
+    const int m = *newest;
+    const T* v = V + (size_t)m * n;
+    const T* v_prev = m > 0 ? v - n : nullptr;
     const double bp = v_prev ? sqrt(*beta_prev_sq) : 0.0;
     double s = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * VEC_BLOCK) {
@@ -146,11 +174,14 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_alpha_kernel(T* __restrict_
     block_reduce_to_scalar(s, block_partials, ticket, alpha);
 }
 
-// w -= *alpha * v;  *beta_sq = |w|^2
+// w -= *alpha * V[*newest];  *beta_sq = |w|^2;  host_ab[2(m+1)] = alpha, host_ab[2(m+1)+1] = beta^2 (iteration k = m+1)
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__ w, const T* __restrict__ v, const double* alpha, int64_t n,
-                                                                 double* block_partials, unsigned int* ticket, double* beta_sq)
+__global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__ w, const T* __restrict__ V, const int* __restrict__ newest,
+                                                                 const double* alpha, int64_t n, double* block_partials, unsigned int* ticket,
+                                                                 double* beta_sq, double* host_ab)
 {
+    const int m = *newest;
+    const T* v = V + (size_t)m * n;
     const double a = *alpha;
     double s = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * VEC_BLOCK) {
@@ -158,27 +189,31 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__
         w[i] = wi;
         s = fma((double)wi, (double)wi, s);
     }
-    block_reduce_to_scalar(s, block_partials, ticket, beta_sq);
+    block_reduce_to_scalar(s, block_partials, ticket, beta_sq, host_ab + 2 * (m + 1) + 1);
+    if (blockIdx.x == 0 && threadIdx.x == 0) host_ab[2 * (m + 1)] = a;
 }
 
-// Gram column for the stopping test (a9): g[j] = V[j] . V[k], j = 0..k.  Lanczos without
+// Gram column for the stopping test (a9): with c = *newest + 1 the column of the vector just written,
+// g[j] = V[j] . V[c], j = 0..c, stored to host_gram[c * ld + j].  Lanczos without
 // re-orthogonalisation loses orthogonality of V, so |y_k - y_{k-1}| = |z| |V_k delta| is evaluated as
 // sqrt(delta^T G delta) with the true Gram matrix G = V^T V instead of assuming G = I.
-// Grid (chunks, k+1): block (b, j) forms the part of V[j] . V[k] over the index range [b*chunk, (b+1)*chunk);
-// the last block to finish (ticket) adds the partials [j][b] in index order: deterministic.
+// Grid (chunks, max columns): block (b, j) forms the part of V[j] . V[c] over [b*chunk, (b+1)*chunk) and
+// exits at once for j > c; the last block to finish (ticket) adds the partials [j][b] in index order.
 constexpr int GRAM_MAX_BLOCKS = 128;
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) gram_column_kernel(const T* __restrict__ V, int64_t dof, int k, int64_t chunk, double* partials,
-                                                                unsigned int* ticket, double* g)
+__global__ void __launch_bounds__(VEC_BLOCK) gram_column_kernel(const T* __restrict__ V, int64_t dof, const int* __restrict__ newest, int64_t chunk, double* partials,
+                                                                unsigned int* ticket, double* host_gram, int ld)
 {
     __shared__ double warp_part[VEC_BLOCK / 32];
     __shared__ bool is_last;
+    const int c = *newest + 1;
     const int j = blockIdx.y;
+    if (j > c) return;
     const int64_t lo_i = (int64_t)blockIdx.x * chunk, hi_i = min(lo_i + chunk, dof);
-    const T* vk = V + (size_t)k * dof;
+    const T* vc = V + (size_t)c * dof;
     const T* vj = V + (size_t)j * dof;
     double s = 0.0;
-    for (int64_t i = lo_i + threadIdx.x; i < hi_i; i += VEC_BLOCK) s = fma((double)vj[i], (double)vk[i], s);
+    for (int64_t i = lo_i + threadIdx.x; i < hi_i; i += VEC_BLOCK) s = fma((double)vj[i], (double)vc[i], s);
     s = warp_sum(s);
     if ((threadIdx.x & 31) == 0) warp_part[threadIdx.x >> 5] = s;
     __syncthreads();
@@ -188,19 +223,23 @@ __global__ void __launch_bounds__(VEC_BLOCK) gram_column_kernel(const T* __restr
         for (int w = 0; w < VEC_BLOCK / 32; ++w) t += warp_part[w];
         partials[(size_t)j * gridDim.x + blockIdx.x] = t;
         __threadfence();
-        is_last = (atomicAdd(ticket, 1u) == gridDim.x * gridDim.y - 1);
+        is_last = (atomicAdd(ticket, 1u) == gridDim.x * (unsigned int)(c + 1) - 1);
     }
     __syncthreads();
     if (is_last) {
         __threadfence();
-        for (int jj = threadIdx.x; jj <= k; jj += VEC_BLOCK) {
+        for (int jj = threadIdx.x; jj <= c; jj += VEC_BLOCK) {
             double t = 0.0;
             for (unsigned int b = 0; b < gridDim.x; ++b) t += ((volatile double*)partials)[(size_t)jj * gridDim.x + b];
-            g[jj] = t;
+            host_gram[(size_t)c * ld + jj] = t;
         }
         if (threadIdx.x == 0) *ticket = 0u;
     }
 }
+
+// *newest += 1, as its own launch after the Gram column: blocks of that kernel that exit early may be
+// scheduled after its last active block has finished, so the index must not move while it runs.
+__global__ void lanczos_advance_kernel(int* newest) { *newest += 1; }
 
 // a10: y = scale * sum_{m<k} coef[m] V[m]  split into the linear (first 3N) and angular (last 3N)
 // outputs; accumulate != 0 adds to what is already there (lm_hydrodynamic_velocities).
