@@ -16,6 +16,11 @@ bd_step            X^{n+1} = X^n + dt (3/2 M^n F^n - 1/2 M^{n-1} F^{n-1}) + sqrt
                    F^n = steric forces at X^n + external forces; torques are external (PAPER.md:226:
                    "F represents a combined vector of forces and torques").
 
+thermal_drift_rfd  eq. (11), one realisation (no average):
+                   (1/delta) [ M(X + delta W/2) W - M(X - delta W/2) W ],  W of length 3N acting as forces
+                   (the mobility depends on positions only); rows = linear (and angular) velocities.
+                   For open boundaries its mean over W is the divergence of M, which is zero.
+
 Pins: tests/test_oracle_bd.py.  No function here is "parity unpinned".
 """
 from __future__ import annotations
@@ -91,3 +96,14 @@ def bd_step(pos, v_prev, dt: float, kT: float, a: float = 1.0, eta: float = 1.0,
             info["iterations"] = k
         new = new + noise_prefactor(kT, dt) * np.asarray(y).reshape(-1)[: 3 * N].reshape(N, 3)
     return new, U, info
+
+
+def thermal_drift_rfd(pos, W, delta: float, a: float = 1.0, eta: float = 1.0, angular: bool = False):
+    """One random-finite-difference sample of the thermal drift, eq. (11).  Returns (lin (N,3), ang (N,3) or None)."""
+    x = np.asarray(pos, dtype=np.float64).reshape(-1, 3)
+    w = np.asarray(W, dtype=np.float64).reshape(-1, 3)
+    Up, Op = rpy.mdot(x + 0.5 * delta * w, w, None, a=a, eta=eta, angular=angular)
+    Um, Om = rpy.mdot(x - 0.5 * delta * w, w, None, a=a, eta=eta, angular=angular)
+    lin = (Up - Um) / delta
+    ang = (Op - Om) / delta if angular else None
+    return lin, ang

@@ -13,6 +13,10 @@ B6  noise prefactor: one isolated sphere performs free diffusion with D = k_B T 
 B7  two equal spheres under equal forces: one Euler step moves them by dt times the closed-form
     sedimentation velocity (textbook RPY)
 B8  Lanczos and dense noise modes agree within the gates of S4
+B9  eq. (11): the RFD sample equals the directional derivative sum_k W_k dM/dX_k W built coordinate by
+    coordinate from central differences of the DENSE matrix (a different route: pins 1/delta and the
+    +-delta/2 arguments), to O(delta^2); and its mean over many W vanishes for open boundaries
+     within the statistical error
 """
 import math
 
@@ -148,3 +152,36 @@ def test_b8_noise_modes_agree_and_steric_pushes_overlaps_apart():
     x2 = np.array([[0.0, 0.0, 0.0], [1.0, 0.0, 0.0], [30.0, 0.0, 0.0]])
     new, _, _ = bd.bd_step(x2, None, 1e-3, 0.0, U0=4.0, b=0.1)
     assert np.linalg.norm(new[1] - new[0]) > 1.0
+
+
+def test_b9_rfd_is_the_directional_derivative_and_averages_to_zero():
+    from oracle import rpy
+    rng = np.random.default_rng(9)
+    N = 5
+    x = rng.random((N, 3)) * 4.0                       # overlapping and non-overlapping pairs
+    W = rng.standard_normal((N, 3))
+    delta = 1e-4
+    lin, ang = bd.thermal_drift_rfd(x, W, delta, angular=True)
+    # sum_k W_k dM/dX_k, coordinate by coordinate, from the dense 6N x 6N matrix
+    h = 1e-6
+    dM = np.zeros((6 * N, 6 * N))
+    for p in range(N):
+        for c in range(3):
+            xp, xm = x.copy(), x.copy()
+            xp[p, c] += h
+            xm[p, c] -= h
+            dM += W[p, c] * (rpy.dense(xp, angular=True) - rpy.dense(xm, angular=True)) / (2 * h)
+    ref = dM @ np.concatenate([W.reshape(-1), np.zeros(3 * N)])
+    np.testing.assert_allclose(lin.reshape(-1), ref[: 3 * N], rtol=2e-5, atol=1e-9)
+    np.testing.assert_allclose(ang.reshape(-1), ref[3 * N:], rtol=2e-5, atol=1e-9)
+    # mean over realisations -> div M = 0; a single sample is O(|dM|) ~ 1e-2
+    S = 4000
+    acc = np.zeros((N, 3))
+    sq = np.zeros((N, 3))
+    for _ in range(S):
+        l, _ = bd.thermal_drift_rfd(x, rng.standard_normal((N, 3)), 1e-3)
+        acc += l
+        sq += l * l
+    mean, sem = acc / S, np.sqrt(sq / S) / math.sqrt(S)
+    assert np.sqrt(sq / S).max() > 1e-3                 # the samples themselves are not small
+    assert np.all(np.abs(mean) <= 5 * sem)
