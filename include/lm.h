@@ -13,8 +13,8 @@
  *   sqrtMdotW()           -> (linear, angular)        lm_sqrt_mdot_w
  *   mf + dwf + drift (the sum the example forms)      lm_hydrodynamic_velocities PAPER.md:78 (eq. 9), 137-138
  *   eq. (13) steric force, eq. (14) AB time step       lm_steric_forces, lm_bd_step
- *   divM()                                            not exported: identically zero for open
- *                                                     boundaries
+ *   divM()                                            lm_thermal_drift (zero for open boundaries,
+ *                                                     PAPER.md:87, 151), lm_thermal_drift_rfd (eq. 11)
  *
  * What is computed.  U = M.[F;T] with M the 6N x 6N grand mobility of eq. (7)
  * whose blocks are the free-space Rotne-Prager-Yamakawa pair tensors, summed over
@@ -140,6 +140,20 @@ int lm_bd_step(lm_solver* h, void* pos, const void* ext_forces, const void* ext_
 int lm_bd_step_host(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise,
                     double dt, double kT, double U0, double b, double tol, void* stream);
 int lm_bd_reset(lm_solver* h);                        /* forget the Adams-Bashforth history */
+
+/* ---- Thermal drift  d/dX . M  (the paper's divM) ----
+ * lm_thermal_drift: the library default for open boundaries -- the divergence of the free-space mobility
+ * is identically zero ("the default implementation simply sets the thermal drift to
+ * zero"): writes zeros to lin_out (3N) and ang_out (3N, iff include_angular).
+ * lm_thermal_drift_rfd: ONE realisation of the random finite difference of eq. (11),
+ *   (1/delta) [ M(X + delta W/2) W - M(X - delta W/2) W ],
+ * at the positions X of the last lm_set_positions (which stay set), W = noise: 3N values ~ N(0,1)
+ * acting as forces (the mobility depends on positions only); rows: linear (lin_out) and,
+ * with include_angular, angular (ang_out) velocities.  Its average over realisations estimates d/dX . M,
+ * zero here; it is exported because eq. (11) is part of the paper's generic machinery and because it
+ * costs exactly two M.F applies.  delta <= 0 -> LM_E_INVALID.  Asynchronous on `stream`. */
+int lm_thermal_drift(lm_solver* h, void* lin_out, void* ang_out, void* stream);
+int lm_thermal_drift_rfd(lm_solver* h, const void* noise, double delta, void* lin_out, void* ang_out, void* stream);
 
 /* Lanczos controls and introspection.  Diagnostics through the environment (read at call time):
  * LM_DEBUG_LANCZOS=1 prints alpha_k, beta_k and the relative step of every iteration on stderr;

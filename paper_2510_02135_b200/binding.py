@@ -40,6 +40,8 @@ SIGNATURES = {
     "lm_bd_step": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_double, c_double, c_double, c_void_p]),
     "lm_bd_step_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_double, c_double, c_double, c_void_p]),
     "lm_bd_reset": (c_int, [c_void_p]),
+    "lm_thermal_drift": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
+    "lm_thermal_drift_rfd": (c_int, [c_void_p, c_void_p, c_double, c_void_p, c_void_p, c_void_p]),
     "lm_set_max_iter": (c_int, [c_void_p, c_int]),
     "lm_last_iterations": (c_int, [c_void_p]),
     "lm_last_error": (c_char_p, [c_void_p]),
@@ -243,6 +245,17 @@ class Solver:
 
     def bd_reset(self):
         self._check(lib().lm_bd_reset(self._h))
+
+    # -- thermal drift (the paper's divM)
+    def thermal_drift(self, lin_out, ang_out=None, stream=None):
+        for x in (lin_out, ang_out):
+            self._expect(x, 3 * self.N, False)
+        self._check(lib().lm_thermal_drift(self._h, _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+
+    def thermal_drift_rfd(self, noise, delta, lin_out, ang_out=None, stream=None):
+        for x in (noise, lin_out, ang_out):
+            self._expect(x, 3 * self.N, False)
+        self._check(lib().lm_thermal_drift_rfd(self._h, _ptr(noise), float(delta), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
 
     # -- controls / introspection
     def set_max_iter(self, n):

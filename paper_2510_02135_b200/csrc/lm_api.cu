@@ -115,6 +115,10 @@ struct lm_solver {
     void* bd[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     size_t bd_bytes[7] = {0, 0, 0, 0, 0, 0, 0};
     bool bd_have_prev = false;
+    bool steric_attr_set = false;
+    // random finite difference (lm_thermal_drift_rfd): displaced packed positions, U(X-) linear / angular
+    void* rfd[3] = {nullptr, nullptr, nullptr};
+    size_t rfd_bytes[3] = {0, 0, 0};
 
     // staging for the _host entry points
     void* st[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // pos, f, t, noise, lin, ang
@@ -536,10 +540,9 @@ template <typename T> int set_positions_t(lm_solver* h, const void* pos, cudaStr
 template <typename T>
 int steric_device(lm_solver* h, double U0, double b, const T* ext, T* out, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!h->steric_attr_set) {
         LM_CUDA(h, cudaFuncSetAttribute((const void*)steric_pair_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, steric_smem_bytes<T>()));
-        attr_set = true;
+        h->steric_attr_set = true;
     }
     const int units = (int)(h->npad / STERIC_SUB);
     const int i_tiles = (int)((h->N + STERIC_TARGETS - 1) / STERIC_TARGETS);
@@ -562,6 +565,32 @@ int steric_device(lm_solver* h, double U0, double b, const T* ext, T* out, cudaS
     steric_pair_kernel<T><<<dim3(i_tiles, splits), STERIC_BLOCK, steric_smem_bytes<T>(), st>>>(p);
     steric_reduce_kernel<T><<<grid_1d(h->N), VEC_BLOCK, 0, st>>>((const T*)h->partial, splits, h->N, h->npad, ext, out);
     h->n_aux += 2;
+    LM_CUDA(h, cudaGetLastError());
+    return LM_OK;
+}
+
+// eq. (11): (1/delta) [ M(X + delta W/2) W - M(X - delta W/2) W ], one realisation
+template <typename T>
+int rfd_device(lm_solver* h, const T* W, double delta, T* lin_out, T* ang_out, cudaStream_t st)
+{
+    const int64_t n3 = 3 * h->N;
+    int rc;
+    if ((rc = ensure(h, &h->rfd[0], &h->rfd_bytes[0], (size_t)3 * h->npad * sizeof(T))) != LM_OK) return rc;
+    if ((rc = ensure(h, &h->rfd[1], &h->rfd_bytes[1], (size_t)n3 * sizeof(T))) != LM_OK) return rc;
+    if (h->angular && (rc = ensure(h, &h->rfd[2], &h->rfd_bytes[2], (size_t)n3 * sizeof(T))) != LM_OK) return rc;
+    void* const home = h->pos_soa;
+    T* outs[2][2] = {{lin_out, ang_out}, {(T*)h->rfd[1], (T*)h->rfd[2]}};
+    for (int side = 0; side < 2; ++side) {
+        shift_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)home, W, h->N, h->npad, (T)((side ? -0.5 : 0.5) * delta), (T*)h->rfd[0]);
+        h->n_aux++;
+        h->pos_soa = h->rfd[0];                       // the apply reads the displaced copy; the handle's positions are untouched
+        rc = apply_batch<T>(h, 1, W, nullptr, outs[side][0], h->angular ? outs[side][1] : nullptr, st);
+        h->pos_soa = home;
+        if (rc != LM_OK) return rc;
+    }
+    rfd_difference_kernel<T><<<grid_1d(n3), VEC_BLOCK, 0, st>>>(lin_out, (const T*)h->rfd[1], n3, (T)(1.0 / delta));
+    if (h->angular) rfd_difference_kernel<T><<<grid_1d(n3), VEC_BLOCK, 0, st>>>(ang_out, (const T*)h->rfd[2], n3, (T)(1.0 / delta));
+    h->n_aux += h->angular ? 2 : 1;
     LM_CUDA(h, cudaGetLastError());
     return LM_OK;
 }
@@ -728,6 +757,7 @@ int lm_destroy(lm_solver* h)
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     for (void* p : h->st) cudaFree(p);
     for (void* p : h->bd) cudaFree(p);
+    for (void* p : h->rfd) cudaFree(p);
     for (auto e : h->lz_ev) if (e) cudaEventDestroy(e);
     for (auto& pr : h->pending) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
     for (auto e : h->event_pool) cudaEventDestroy(e);
@@ -930,6 +960,29 @@ int lm_bd_step_host(lm_solver* h, void* pos, const void* ext_forces, const void*
     LM_CUDA(h, cudaMemcpyAsync(pos, dp, bytes, cudaMemcpyDeviceToHost, st));
     LM_CUDA(h, cudaStreamSynchronize(st));
     return rc;
+}
+
+// ---------------------------------------------------------------- thermal drift
+int lm_thermal_drift(lm_solver* h, void* lin_out, void* ang_out, void* stream)
+{
+    int rc = check_io(h, nullptr, nullptr, lin_out, ang_out, false);
+    if (rc != LM_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)3 * h->N * esize(h);
+    LM_CUDA(h, cudaMemsetAsync(lin_out, 0, bytes, st));
+    if (h->angular) LM_CUDA(h, cudaMemsetAsync(ang_out, 0, bytes, st));
+    return LM_OK;
+}
+
+int lm_thermal_drift_rfd(lm_solver* h, const void* noise, double delta, void* lin_out, void* ang_out, void* stream)
+{
+    int rc = check_io(h, noise, nullptr, lin_out, ang_out, false);
+    if (rc != LM_OK) return rc;
+    if (!noise) return fail(h, LM_E_NULL, "noise is NULL");
+    if (!(delta > 0.0) || !std::isfinite(delta)) return fail(h, LM_E_INVALID, "delta must be > 0");
+    cudaStream_t st = (cudaStream_t)stream;
+    return h->precision == LM_F32 ? rfd_device<float>(h, (const float*)noise, delta, (float*)lin_out, (float*)ang_out, st)
+                                  : rfd_device<double>(h, (const double*)noise, delta, (double*)lin_out, (double*)ang_out, st);
 }
 
 // ---------------------------------------------------------------- stats / introspection

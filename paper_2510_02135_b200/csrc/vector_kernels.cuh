@@ -67,6 +67,30 @@ __global__ void __launch_bounds__(VEC_BLOCK) reduce_partials_kernel(const T* __r
     else       out.ang[q][3 * i + (k - 3)] = s;
 }
 
+// eq. (11) PAPER.md:151-155 (random finite difference): packed positions displaced along W,
+// out[c][i] = soa[c][i] + s W[3i+c]  (s = +-delta/2); ghosts stay where they are.
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) shift_positions_kernel(const T* __restrict__ soa, const T* __restrict__ W, int64_t N, int64_t npad, T s,
+                                                                    T* __restrict__ out)
+{
+    const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
+    if (i >= npad) return;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        T v = soa[(size_t)c * npad + i];
+        if (i < N) v += s * W[3 * i + c];
+        out[(size_t)c * npad + i] = v;
+    }
+}
+
+// up = (up - um) * inv_delta   (the difference quotient of eq. (11))
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) rfd_difference_kernel(T* __restrict__ up, const T* __restrict__ um, int64_t n, T inv_delta)
+{
+    const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
+    if (i < n) up[i] = (up[i] - um[i]) * inv_delta;
+}
+
 // ---------------------------------------------------------------- Lanczos vector operations (a7)
 // Reductions: warp shuffles -> one fp64 partial per block -> the last block to finish (ticket)
 // adds the block partials in index order, so the result is deterministic for a given grid.

@@ -228,3 +228,41 @@ def test_bd_reset_host_variant_and_errors(lm, torch):
         s.steric_forces(U0, -1.0, None, out)
     assert e.value.code in (lm.LM_E_INVALID, lm.LM_E_NOPOS)
     s.close()
+
+
+@pytest.mark.parametrize("prec,angular,delta", [("f64", False, 1e-3), ("f64", True, 1e-3), ("f32", False, 0.05), ("f32", True, 0.05)])
+def test_thermal_drift_rfd_matches_oracle_and_default_is_zero(lm, torch, prec, angular, delta):
+    """eq. (11): the difference quotient divides the M.F rounding error by delta, so the gate is the M.F
+    gate times |M W| / (delta |RFD|)."""
+    from oracle import rpy
+    c = case(900, 15.0, 31, prec, angular)
+    N = 900
+    W = c["noise"][: 3 * N]
+    s = lm.Solver(prec, N, 1.0, 1.0, angular)
+    s.set_positions(dev(torch, c["pos"]))
+    lin = torch.empty(3 * N, dtype=s.torch_dtype, device="cuda")
+    ang = torch.empty(3 * N, dtype=s.torch_dtype, device="cuda") if angular else None
+    s.thermal_drift_rfd(dev(torch, W), delta, lin, ang)
+    torch.cuda.synchronize()
+    lo, ao = bd.thermal_drift_rfd(c["pos"], W, delta, angular=angular)
+    U, Om = rpy.mdot(c["pos"], W, None, angular=angular)
+    # the displaced positions are rounded to the run precision on the GPU: that alone perturbs M W by ~eps |x| |dM W|
+    eps_x = np.finfo(workloads.np_dtype(prec)).eps * np.abs(c["pos"]).max()
+    gate = 4 * TOL[prec] * np.linalg.norm(U) / (delta * np.linalg.norm(lo)) + 4 * eps_x / delta
+    assert rel(lin.cpu().numpy(), lo) <= gate
+    if angular:
+        gate_a = 4 * TOL[prec] * np.linalg.norm(Om) / (delta * np.linalg.norm(ao)) + 4 * eps_x / delta
+        assert rel(ang.cpu().numpy(), ao) <= gate_a
+    # the handle's own positions are untouched: M.F afterwards is M.F at X
+    U2 = torch.empty(3 * N, dtype=s.torch_dtype, device="cuda")
+    s.mdot(dev(torch, W), None, U2, ang)
+    torch.cuda.synchronize()
+    assert rel(U2.cpu().numpy(), U) <= TOL[prec]
+    # library default for open boundaries: zero drift (PAPER.md:151)
+    s.thermal_drift(lin, ang)
+    torch.cuda.synchronize()
+    assert float(lin.abs().max()) == 0.0 and (ang is None or float(ang.abs().max()) == 0.0)
+    with pytest.raises(lm.LmError) as e:
+        s.thermal_drift_rfd(dev(torch, W), 0.0, lin, ang)
+    assert e.value.code == lm.LM_E_INVALID
+    s.close()
