@@ -55,14 +55,14 @@ template <typename T, int NRHS, bool ANG, int SUB, int MINB> Variant<T> make_sma
 template <typename T> std::vector<Variant<T>> build_variants();
 template <> std::vector<Variant<float>> build_variants<float>()
 {
-    return {make_large<float, 1, false, 4, 32, 2>(), make_large<float, 2, false, 4, 32, 1>(), make_large<float, 4, false, 2, 32, 2>(),
+    return {make_large<float, 1, false, 4, 32, 2>(), make_large<float, 2, false, 4, 32, 1>(), make_large<float, 4, false, 4, 32, 1>(),
             make_large<float, 1, true, 2, 32, 2>(),  make_large<float, 2, true, 2, 32, 1>(),
             make_small<float, 1, false, 32, 8>(), make_small<float, 2, false, 32, 8>(), make_small<float, 4, false, 32, 6>(),
             make_small<float, 1, true, 32, 8>(),  make_small<float, 2, true, 32, 6>()};
 }
 template <> std::vector<Variant<double>> build_variants<double>()
 {
-    return {make_large<double, 1, false, 2, 32, 2>(), make_large<double, 2, false, 2, 32, 1>(), make_large<double, 4, false, 2, 32, 1>(),
+    return {make_large<double, 1, false, 4, 32, 1>(), make_large<double, 2, false, 2, 32, 1>(), make_large<double, 4, false, 2, 32, 1>(),
             make_large<double, 1, true, 2, 32, 1>(),  make_large<double, 2, true, 2, 32, 1>(),
             make_small<double, 1, false, 32, 8>(), make_small<double, 2, false, 32, 6>(), make_small<double, 4, false, 32, 4>(),
             make_small<double, 1, true, 32, 6>(),  make_small<double, 2, true, 32, 4>()};
