@@ -96,6 +96,16 @@ int lm_mdot_batch(lm_solver* h, int nrhs, const void* forces, const void* torque
 int lm_sqrt_mdot_w(lm_solver* h, const void* noise, double tol, void* lin_out, void* ang_out,
                    int* iters_out, void* stream);
 
+/* nvec independent noise vectors sharing one position set: y_q = M^{1/2} W_q, q < nvec.  The Lanczos
+ * recurrences run in lockstep in groups of 4 / 2 / 1 vectors (angular: 2 / 1) so that ONE multi-right-
+ * hand-side pair-kernel launch per iteration serves a whole group (the pair geometry is evaluated once
+ * per pair, as in lm_mdot_batch); each vector has its own alpha, beta, Gram matrix and stopping test
+ * and stops contributing to the result at its own step.  noise: [nvec][dof]; lin_out / ang_out:
+ * [nvec][3N]; iters_out: HOST int[nvec] or NULL.  Each y_q equals what lm_sqrt_mdot_w returns for W_q up
+ * to the summation order of the pair kernel.  LM_E_NOCONV if any vector reached max_iter. */
+int lm_sqrt_mdot_w_batch(lm_solver* h, int nvec, const void* noise, double tol, void* lin_out, void* ang_out,
+                         int* iters_out, void* stream);
+
 /* out = M.[F;T] + noise_prefactor * M^{1/2} W  (+ 0 thermal drift): the right-hand
  * side of eq. (9) for dt = 1 with noise_prefactor = sqrt(2 k_B T / dt) supplied by the caller
  * (PAPER.md:116-118).  noise == NULL: deterministic part only (tol ignored). */

@@ -30,6 +30,7 @@ SIGNATURES = {
     "lm_mdot": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "lm_mdot_batch": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "lm_sqrt_mdot_w": (c_int, [c_void_p, c_void_p, c_double, c_void_p, c_void_p, POINTER(c_int), c_void_p]),
+    "lm_sqrt_mdot_w_batch": (c_int, [c_void_p, c_int, c_void_p, c_double, c_void_p, c_void_p, POINTER(c_int), c_void_p]),
     "lm_hydrodynamic_velocities": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_void_p, c_void_p, c_void_p]),
     "lm_set_positions_host": (c_int, [c_void_p, c_void_p, c_void_p]),
     "lm_mdot_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
@@ -192,6 +193,15 @@ class Solver:
         self._check(lib().lm_sqrt_mdot_w(self._h, _ptr(noise), float(tol), _ptr(lin_out), _ptr(ang_out), ctypes.byref(iters),
                                          _stream_ptr(stream)), allow=(LM_E_NOCONV,) if allow_noconv else ())
         return iters.value
+
+    def sqrt_mdot_w_batch(self, nvec, noise, tol, lin_out, ang_out=None, stream=None, allow_noconv=False):
+        self._expect(noise, nvec * (6 if self.angular else 3) * self.N, False)
+        for x in (lin_out, ang_out):
+            self._expect(x, nvec * 3 * self.N, False)
+        iters = (c_int * int(nvec))()
+        self._check(lib().lm_sqrt_mdot_w_batch(self._h, int(nvec), _ptr(noise), float(tol), _ptr(lin_out), _ptr(ang_out), iters,
+                                               _stream_ptr(stream)), allow=(LM_E_NOCONV,) if allow_noconv else ())
+        return list(iters)
 
     def hydrodynamic_velocities(self, forces, torques, noise, noise_prefactor, tol, lin_out, ang_out=None, stream=None):
         self._check(lib().lm_hydrodynamic_velocities(self._h, _ptr(forces), _ptr(torques), _ptr(noise), float(noise_prefactor),

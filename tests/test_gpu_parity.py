@@ -415,3 +415,67 @@ def test_stats_and_launch_config(lm, torch):
     st = s.get_stats()
     assert st["pair_kernel_launches"] == 1 and st["pair_kernel_ms"] > 0
     assert lm.lm_probe_fma_peak(lm.LM_F32, 0.05) > 1e13
+
+
+# ---------------------------------------------------------------- several noise vectors per call
+@pytest.mark.parametrize("prec,angular", [("f64", False), ("f64", True), ("f32", False), ("f32", True)])
+@pytest.mark.parametrize("nvec", [2, 3, 4, 7])
+def test_sqrt_mdot_w_batch_each_vector_matches_oracle(lm, torch, prec, angular, nvec):
+    """Lockstep recurrences on the multi-RHS kernel: every vector must satisfy the single-vector gates (S4)
+    against the fp64 Lanczos oracle and the exact dense root, with its own stopping step; groups 4/2/1
+    (angular 2/1) and a zero vector in the batch."""
+    N, tol = 300, 1e-3
+    case = workloads.random_case(N, 12.0, 40 + nvec, prec, angular, with_noise=True)
+    dof = (6 if angular else 3) * N
+    rng = np.random.default_rng(100 + nvec)
+    W = rng.standard_normal((nvec, dof)).astype(workloads.np_dtype(prec))
+    W[0] = case["noise"]
+    if nvec >= 3:
+        W[2] = 0.0                                         # M^{1/2} 0 = 0, zero iterations
+    s = lm.Solver(prec, N, 1.0, 1.0, angular)
+    s.set_positions(dev(torch, case["pos"]))
+    lin = torch.empty(nvec * 3 * N, dtype=s.torch_dtype, device="cuda")
+    ang = torch.empty(nvec * 3 * N, dtype=s.torch_dtype, device="cuda") if angular else None
+    iters = s.sqrt_mdot_w_batch(nvec, dev(torch, W).reshape(-1), tol, lin, ang)
+    torch.cuda.synchronize()
+    lin = lin.cpu().numpy().reshape(nvec, 3 * N)
+    ang = ang.cpu().numpy().reshape(nvec, 3 * N) if angular else None
+    for q in range(nvec):
+        y = lin[q] if not angular else np.concatenate([lin[q], ang[q]])
+        if nvec >= 3 and q == 2:
+            assert iters[q] == 0 and np.all(y == 0.0)
+            continue
+        yo, ko, conv = rpy.lanczos_sqrt_mdot_w(case["pos"], W[q], tol, angular=angular)
+        exact = rpy.dense_sqrt_mdot_w(case["pos"], W[q], angular=angular)
+        assert conv
+        assert abs(iters[q] - ko) <= (0 if prec == "f64" else max(1, ko // 4)), (q, iters[q], ko)
+        assert rel(y, yo) <= (1e-6 if prec == "f64" else 10 * tol), (q, rel(y, yo))
+        assert rel(y, exact) <= 10 * tol, (q, rel(y, exact))
+    # the single-vector call gives the same answer for vector 0 (up to the pair kernel's summation order)
+    y1, it1, _ = gpu_sqrt(lm, torch, prec, case["pos"], W[0], tol, angular)
+    y0 = lin[0] if not angular else np.concatenate([lin[0], ang[0]])
+    assert abs(it1 - iters[0]) <= (0 if prec == "f64" else 1)
+    assert rel(y0, y1) <= (1e-10 if prec == "f64" else 5 * tol)
+    s.close()
+
+
+def test_sqrt_mdot_w_batch_noconv_and_errors(lm, torch):
+    case = workloads.random_case(200, 8.0, 50, "f64", False, with_noise=True)
+    N = 200
+    s = lm.Solver("f64", N, 1.0, 1.0, False)
+    s.set_positions(dev(torch, case["pos"]))
+    W = np.random.default_rng(5).standard_normal((2, 3 * N))
+    lin = torch.empty(2 * 3 * N, dtype=torch.float64, device="cuda")
+    s.set_max_iter(3)
+    with pytest.raises(lm.LmError) as e:
+        s.sqrt_mdot_w_batch(2, dev(torch, W).reshape(-1), 1e-12, lin)
+    assert e.value.code == lm.LM_E_NOCONV
+    its = s.sqrt_mdot_w_batch(2, dev(torch, W).reshape(-1), 1e-12, lin, allow_noconv=True)
+    assert its == [3, 3]
+    for q in range(2):                                        # the last iterate IS written: 3 plain Lanczos steps
+        yo, ko, _ = rpy.lanczos_sqrt_mdot_w(case["pos"], W[q], 1e-12, max_iter=3)
+        assert ko == 3 and rel(lin.cpu().numpy().reshape(2, -1)[q], yo) <= 1e-11
+    with pytest.raises(lm.LmError) as e:
+        s.sqrt_mdot_w_batch(0, dev(torch, W).reshape(-1)[:0], 1e-3, lin[:0])
+    assert e.value.code in (lm.LM_E_INVALID, lm.LM_E_NULL)
+    s.close()
