@@ -186,6 +186,9 @@ def main():
     ap.add_argument("--N", type=int, default=None, help="override N (measurement sweeps only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "sharded"],
+                    help="N > 1 ranks: independent replicas (default, weak scaling) or ONE problem row-sharded over the ranks "
+                         "(lm_dist_init: all-gather of the row blocks inside every apply, strong scaling)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -216,7 +219,9 @@ def main():
 
     from paper_2510_02135_b200 import multi
     cfg = workloads.CONFIGS[args.config]
-    data = workloads.generate(args.config, args.N, seed=multi.replica_seed(cfg.seed, rank))   # independent replicas
+    sharded = args.parallelism == "sharded" and world > 1
+    # replicas: every rank its own problem (seed + 1000 rank); sharded: the same problem on every rank
+    data = workloads.generate(args.config, args.N, seed=cfg.seed if sharded else multi.replica_seed(cfg.seed, rank))
     N = data["N"]
     f64 = cfg.precision == "f64"
     tdt = torch.float64 if f64 else torch.float32
@@ -224,6 +229,8 @@ def main():
     stream = torch.cuda.current_stream()
 
     solver = lm.Solver(cfg.precision, N, cfg.eta, cfg.a, cfg.angular)
+    if sharded:
+        multi.init_sharded(solver)
 
     # ---- device-resident inputs (value) and pinned host inputs (e2e)
     def pinned(x):
@@ -339,7 +346,8 @@ def main():
     if clocks and clocks.get("sm_max_mhz"):
         sm_max_mhz = float(clocks["sm_max_mhz"])
     peak = sms * nominal_lanes(f64) * sm_max_mhz * 1e6 / 1e12                 # T lane-ops/s at max clock
-    achieved = instr * float(N) * float(N) / (pair_ms_avg * 1e-3) / 1e12
+    pairs_per_launch = stats["pairs"] / max(1, launches_pair)                 # rank 0's share when row-sharded
+    achieved = instr * pairs_per_launch / (pair_ms_avg * 1e-3) / 1e12
     probe = lm.lm_probe_fma_peak(lm.LM_F64 if f64 else lm.LM_F32, 0.3) / 1e12
     roofline = {
         "bound": "alu", "kernel": f"rpy_pair_kernel<{cfg.precision}, nrhs={nrhs_launch}, angular={int(cfg.angular)}>",
@@ -347,21 +355,21 @@ def main():
         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if args.N is None else None,
         "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_c%d_pair_kernel_ncu_full.md)" % args.config,
         "peak_source": f"derived: {sms} SMs x {nominal_lanes(f64)} lanes x {sm_max_mhz:.0f} MHz (clocks.max.sm); MEASURED_PEAKS.json has no ALU entry",
-        "lane_ops_per_pair": instr, "flops_per_pair": flops, "pairs_per_launch": float(N) * float(N),
+        "lane_ops_per_pair": instr, "flops_per_pair": flops, "pairs_per_launch": pairs_per_launch,
         "launch_ms_avg": pair_ms_avg, "launches_timed": launches_pair,
-        "flop_frac": flops * float(N) * float(N) / (pair_ms_avg * 1e-3) / 1e12 / (2 * peak),
+        "flop_frac": flops * pairs_per_launch / (pair_ms_avg * 1e-3) / 1e12 / (2 * peak),
         "measured_fma_peak": probe, "frac_of_measured_fma_peak": achieved / probe,
-        "kernel_gpairs_per_s": float(N) * float(N) / (pair_ms_avg * 1e-3) / 1e9,
+        "kernel_gpairs_per_s": pairs_per_launch / (pair_ms_avg * 1e-3) / 1e9,
     }
     if clocks and clocks.get("sm_mhz"):
         roofline["frac_at_observed_clock"] = achieved / (sms * nominal_lanes(f64) * clocks["sm_mhz"] * 1e6 / 1e12)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
         "dtype": cfg.precision, "data": "synthetic",
         "config": config_dict(cfg, N, {"l2": "256 MiB device memset between steps, outside the event brackets",
-                                       "parallelism": "replicas only" if world > 1 else "1 GPU",
+                                       "parallelism": ("row-sharded, all-gather per apply" if sharded else "replicas only") if world > 1 else "1 GPU",
                                        "pair_launches_per_step": launches_pair / args.steps, "lanczos_iterations": iters,
                                        "launch": solver.pair_launch_config(nrhs_launch)}),
         "ms_per_mdot": pair_ms_avg,

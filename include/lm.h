@@ -165,6 +165,30 @@ int lm_bd_reset(lm_solver* h);                        /* forget the Adams-Bashfo
 int lm_thermal_drift(lm_solver* h, void* lin_out, void* ang_out, void* stream);
 int lm_thermal_drift_rfd(lm_solver* h, const void* noise, double delta, void* lin_out, void* ang_out, void* stream);
 
+/* ---- Row-sharded applies across GPUs (one process per GPU) ----
+ * The target rows of M.[F;T] are independent, so G ranks can each compute a block of rows against ALL
+ * sources.  SPMD with replicated inputs and outputs: every rank creates a handle for the same N, calls
+ * the same functions in the same order with the same positions / forces / noise, computes only its row
+ * block  [r B, min((r+1) B, N)),  B = ceil(N / G)  (lm_dist_row_block), and one grouped ncclAllGather
+ * per pair-kernel launch (over NVLink / NVSwitch) completes every output on every rank.  All entry points
+ * (lm_mdot*, lm_sqrt_mdot_w*, lm_hydrodynamic_velocities, lm_thermal_drift_rfd, lm_bd_step) then work
+ * unchanged; the O(N) vector kernels and lm_steric_forces are replicated.  Ranks must run the same GPU
+ * model: the Lanczos stopping decision is taken per rank from bit-identical scalars.
+ *   lm_dist_unique_id : 128-byte NCCL unique id (host buffer); call on ONE rank and broadcast it to the
+ *                       others by any means (torch.distributed, MPI, a file).
+ *   lm_dist_init      : collective; creates this handle's communicator (current CUDA device) and fixes
+ *                       its row block.  nranks = 1 is allowed.  NCCL is loaded at run time (the libnccl
+ *                       already in the process, else the system one); LM_E_CUDA if it cannot be.
+ *   lm_dist_row_block : host-only helper, the row block of `rank` (needs no GPU).
+ *   lm_mdot_rows      : WITHOUT a communicator: compute only rows [row_begin, row_begin + row_count) of
+ *                       lm_mdot and write them at their places in the full-length outputs (the other
+ *                       entries are left untouched) -- the building block for a caller's own sharding. */
+int lm_dist_row_block(int64_t N, int nranks, int rank, int64_t* row_begin, int64_t* row_end);
+int lm_dist_unique_id(void* out128);
+int lm_dist_init(lm_solver* h, int nranks, int rank, const void* unique_id128);
+int lm_mdot_rows(lm_solver* h, int64_t row_begin, int64_t row_count, const void* forces, const void* torques,
+                 void* lin_out, void* ang_out, void* stream);
+
 /* Lanczos controls and introspection.  Diagnostics through the environment (read at call time):
  * LM_DEBUG_LANCZOS=1 prints alpha_k, beta_k and the relative step of every iteration on stderr;
  * LM_NO_GRAPH=1 launches the iteration's kernels one by one instead of replaying the captured CUDA graph. */

@@ -43,6 +43,10 @@ SIGNATURES = {
     "lm_bd_reset": (c_int, [c_void_p]),
     "lm_thermal_drift": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "lm_thermal_drift_rfd": (c_int, [c_void_p, c_void_p, c_double, c_void_p, c_void_p, c_void_p]),
+    "lm_dist_row_block": (c_int, [c_int64, c_int, c_int, POINTER(c_int64), POINTER(c_int64)]),
+    "lm_dist_unique_id": (c_int, [c_void_p]),
+    "lm_dist_init": (c_int, [c_void_p, c_int, c_int, c_void_p]),
+    "lm_mdot_rows": (c_int, [c_void_p, c_int64, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "lm_set_max_iter": (c_int, [c_void_p, c_int]),
     "lm_last_iterations": (c_int, [c_void_p]),
     "lm_last_error": (c_char_p, [c_void_p]),
@@ -90,6 +94,23 @@ def lm_host_tridiag_sqrt_e1(alpha, beta) -> np.ndarray:
     if rc != LM_OK:
         raise LmError(rc, "lm_host_tridiag_sqrt_e1")
     return out
+
+
+def lm_dist_row_block(N: int, nranks: int, rank: int):
+    """(row_begin, row_end) of `rank`'s block of target rows -- host only, needs no GPU."""
+    b, e = c_int64(0), c_int64(0)
+    rc = lib().lm_dist_row_block(int(N), int(nranks), int(rank), ctypes.byref(b), ctypes.byref(e))
+    if rc != LM_OK:
+        raise LmError(rc, "lm_dist_row_block: need N > 0 and 0 <= rank < nranks")
+    return b.value, e.value
+
+
+def lm_dist_unique_id() -> bytes:
+    buf = ctypes.create_string_buffer(128)
+    rc = lib().lm_dist_unique_id(buf)
+    if rc != LM_OK:
+        raise LmError(rc, "lm_dist_unique_id: NCCL unavailable")
+    return buf.raw
 
 
 def lm_probe_fma_peak(precision: int, seconds: float = 0.2) -> float:
@@ -255,6 +276,17 @@ class Solver:
 
     def bd_reset(self):
         self._check(lib().lm_bd_reset(self._h))
+
+    # -- row-sharded applies
+    def dist_init(self, nranks: int, rank: int, unique_id: bytes):
+        assert len(unique_id) == 128
+        self._check(lib().lm_dist_init(self._h, int(nranks), int(rank), ctypes.create_string_buffer(unique_id, 128)))
+
+    def mdot_rows(self, row_begin, row_count, forces, torques, lin_out, ang_out=None, stream=None):
+        for x in (forces, torques, lin_out, ang_out):
+            self._expect(x, 3 * self.N, False)
+        self._check(lib().lm_mdot_rows(self._h, int(row_begin), int(row_count), _ptr(forces), _ptr(torques), _ptr(lin_out), _ptr(ang_out),
+                                       _stream_ptr(stream)))
 
     # -- thermal drift (the paper's divM)
     def thermal_drift(self, lin_out, ang_out=None, stream=None):

@@ -4,6 +4,7 @@
 // arithmetic is the k x k tridiagonal problem of the Lanczos stopping test (tridiag_host.h).
 // There is no CPU fallback: without a CUDA device every compute call returns LM_E_CUDA.
 #include <cuda_runtime.h>
+#include <dlfcn.h>
 
 #include <algorithm>
 #include <cmath>
@@ -75,6 +76,47 @@ struct LaunchPlan {
 
 }  // namespace lm
 
+// ---------------------------------------------------------------- NCCL, loaded at run time (row-sharded applies only)
+// The library does not link NCCL: a single-GPU user never needs it.  lm_dist_* resolve the few entry
+// points below from the libnccl already in the process (PyTorch's) or, failing that, the system one.
+namespace lm {
+struct NcclApi {
+    struct UniqueId { char internal[128]; };
+    typedef void* Comm;
+    int (*GetUniqueId)(UniqueId*) = nullptr;
+    int (*CommInitRank)(Comm*, int, UniqueId, int) = nullptr;
+    int (*CommDestroy)(Comm) = nullptr;
+    int (*AllGather)(const void*, void*, size_t, int, Comm, cudaStream_t) = nullptr;
+    int (*GroupStart)() = nullptr;
+    int (*GroupEnd)() = nullptr;
+    const char* (*GetErrorString)(int) = nullptr;
+    bool ok = false;
+    std::string why;
+};
+constexpr int NCCL_FLOAT32 = 7, NCCL_FLOAT64 = 8;   // ncclDataType_t values (nccl.h)
+
+inline NcclApi& nccl_api()
+{
+    static NcclApi api;
+    static bool tried = false;
+    if (tried) return api;
+    tried = true;
+    void* lib = dlopen("libnccl.so.2", RTLD_NOW | RTLD_NOLOAD);
+    if (!lib) lib = dlopen("libnccl.so.2", RTLD_NOW | RTLD_GLOBAL);
+    if (!lib) { api.why = std::string("cannot load libnccl.so.2: ") + dlerror(); return api; }
+    auto sym = [&](const char* name) { void* p = dlsym(lib, name); if (!p) api.why = std::string("libnccl.so.2 lacks ") + name; return p; };
+    api.GetUniqueId = (int (*)(NcclApi::UniqueId*))sym("ncclGetUniqueId");
+    api.CommInitRank = (int (*)(NcclApi::Comm*, int, NcclApi::UniqueId, int))sym("ncclCommInitRank");
+    api.CommDestroy = (int (*)(NcclApi::Comm))sym("ncclCommDestroy");
+    api.AllGather = (int (*)(const void*, void*, size_t, int, NcclApi::Comm, cudaStream_t))sym("ncclAllGather");
+    api.GroupStart = (int (*)())sym("ncclGroupStart");
+    api.GroupEnd = (int (*)())sym("ncclGroupEnd");
+    api.GetErrorString = (const char* (*)(int))sym("ncclGetErrorString");
+    api.ok = api.GetUniqueId && api.CommInitRank && api.CommDestroy && api.AllGather && api.GroupStart && api.GroupEnd && api.GetErrorString;
+    return api;
+}
+}  // namespace lm
+
 using namespace lm;
 
 // ---------------------------------------------------------------- handle
@@ -119,6 +161,14 @@ struct lm_solver {
     // random finite difference (lm_thermal_drift_rfd): displaced packed positions, U(X-) linear / angular
     void* rfd[3] = {nullptr, nullptr, nullptr};
     size_t rfd_bytes[3] = {0, 0, 0};
+
+    // row-sharded applies over NCCL (lm_dist_init): rank r computes target rows [r B, min((r+1) B, N)), B = rows_per_rank
+    int dist_ranks = 0, dist_rank = 0;        // dist_ranks == 0: not distributed
+    int64_t rows_per_rank = 0;
+    void* nccl_comm = nullptr;
+    void* gath[2 * MAX_RHS] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // all-gather buffers, 3 B ranks each
+    size_t gath_bytes[2 * MAX_RHS] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int64_t row_begin = 0, row_end = 0;       // the target rows every apply computes ([0, N) unless sharded / lm_mdot_rows)
 
     // staging for the _host entry points
     void* st[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // pos, f, t, noise, lin, ang
@@ -225,7 +275,8 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
         const auto& v = vs[vi];
         if (v.nrhs != nrhs || v.ang != h->angular) continue;
         const int targets = v.block * v.tpt;
-        const int i_tiles = (int)((h->N + targets - 1) / targets);
+        const int64_t rows = std::max<int64_t>(h->row_end - h->row_begin, 0);          // target rows of this rank / call
+        const int i_tiles = (int)((rows + targets - 1) / targets);
         const int units = (int)(h->npad / v.sub);
         const int64_t slots = (int64_t)h->sm_count * v.ctas_per_sm;
         const int max_splits = std::min(units, 256);
@@ -242,7 +293,7 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
             double cost = (double)full * wave(v.ctas_per_sm) + wave(rem_per_sm);
             // cost is in pairs evaluated back to back on one SM (~1e4 per microsecond): the reduce pass
             // adds a ~3 us launch plus writing and re-reading s partial vectors
-            if (s > 1) cost += 3.0e4 + 0.1 * (double)s * (double)h->N;
+            if (s > 1) cost += 3.0e4 + 0.1 * (double)s * (double)rows;
             if (cost < best_cost) {
                 best_cost = cost;
                 best.variant = vi;
@@ -286,17 +337,37 @@ template <typename T> int prepare_apply(lm_solver* h, int nrhs, LaunchPlan& plan
     return LM_OK;
 }
 
-// launch_pair: the pair kernel on the packed right-hand side already in h->vec_soa, then the split-j reduce
+// launch_pair: the pair kernel on the packed right-hand side already in h->vec_soa, then the split-j reduce.
+// Only the target rows [h->row_begin, h->row_end) are computed.  With a communicator (lm_dist_init) those are
+// this rank's block: the kernel writes into all-gather buffers of 3 B ranks elements, ONE grouped
+// ncclAllGather (in place: rank r's segment starts at 3 B r) completes every output on every rank, and the
+// first 3N elements are copied to the caller's buffers.
 template <typename T> int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>& out, cudaStream_t st, bool timed)
 {
     const int nc = h->angular ? 6 : 3;
     const auto& v = variants<T>(h)[plan.variant];
+    const bool dist = h->dist_ranks > 0;
+    RhsOut<T> kout = out;
+    const size_t seg = (size_t)3 * h->rows_per_rank;                       // elements each rank contributes
+    if (dist) {
+        const size_t bytes = seg * h->dist_ranks * sizeof(T);
+        for (int q = 0; q < nrhs; ++q) {
+            for (int part = 0; part < (h->angular ? 2 : 1); ++part) {
+                const int rc = ensure(h, &h->gath[2 * q + part], &h->gath_bytes[2 * q + part], bytes);
+                if (rc != LM_OK) return rc;
+            }
+            kout.lin[q] = (T*)h->gath[2 * q];
+            kout.ang[q] = h->angular ? (T*)h->gath[2 * q + 1] : nullptr;
+        }
+    }
     PairParams<T> p;
     p.pos = (const T*)h->pos_soa;
     p.vec = (const T*)h->vec_soa;
-    p.out = out;
+    p.out = kout;
     p.partial = (T*)h->partial;
     p.N = h->N;
+    p.i_begin = h->row_begin;
+    p.i_end = h->row_end;
     p.npad = h->npad;
     p.n_units = plan.n_units;
     p.c = make_consts<T>(h->eta, h->a);
@@ -307,21 +378,40 @@ template <typename T> int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& 
         e1 = get_event(h);
         LM_CUDA(h, cudaEventRecord(e0, st));
     }
-    v.kernel<<<dim3(plan.i_tiles, plan.j_splits), v.block, v.smem, st>>>(p);
+    if (plan.i_tiles > 0) v.kernel<<<dim3(plan.i_tiles, plan.j_splits), v.block, v.smem, st>>>(p);
     if (timed) {
         LM_CUDA(h, cudaEventRecord(e1, st));
         h->pending.emplace_back(e0, e1);
     }
-    if (plan.j_splits > 1)
-        reduce_partials_kernel<T><<<dim3(grid_1d(h->N), nrhs * nc), VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc, h->N, h->npad, out);
+    if (plan.i_tiles > 0 && plan.j_splits > 1)
+        reduce_partials_kernel<T><<<dim3(grid_1d(h->row_end - h->row_begin), nrhs * nc), VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc,
+                                                                                                         h->row_begin, h->row_end, h->npad, kout);
     LM_CUDA(h, cudaGetLastError());
+    if (dist) {
+        NcclApi& nccl = nccl_api();
+        const int dtype = sizeof(T) == 4 ? NCCL_FLOAT32 : NCCL_FLOAT64;
+        int nrc = nccl.GroupStart();
+        for (int q = 0; q < nrhs && nrc == 0; ++q)
+            for (int part = 0; part < (h->angular ? 2 : 1) && nrc == 0; ++part) {
+                T* buf = (T*)h->gath[2 * q + part];
+                nrc = nccl.AllGather(buf + seg * h->dist_rank, buf, seg, dtype, (NcclApi::Comm)h->nccl_comm, st);
+            }
+        const int nrc_end = nccl.GroupEnd();
+        if (nrc == 0) nrc = nrc_end;
+        if (nrc != 0) return fail(h, LM_E_CUDA, std::string("ncclAllGather failed: ") + nccl.GetErrorString(nrc));
+        const size_t out_bytes = (size_t)3 * h->N * sizeof(T);
+        for (int q = 0; q < nrhs; ++q) {
+            LM_CUDA(h, cudaMemcpyAsync(out.lin[q], h->gath[2 * q], out_bytes, cudaMemcpyDeviceToDevice, st));
+            if (h->angular) LM_CUDA(h, cudaMemcpyAsync(out.ang[q], h->gath[2 * q + 1], out_bytes, cudaMemcpyDeviceToDevice, st));
+        }
+    }
     return LM_OK;
 }
 
 void count_apply(lm_solver* h, const LaunchPlan& plan)
 {
     h->n_pair++;
-    h->pairs += (double)h->N * (double)h->N;
+    h->pairs += (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N;
     if (plan.j_splits > 1) h->n_aux++;
 }
 
@@ -474,7 +564,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     // saves (~25 iterations x 50 us); the same regime is launch-bound, so there the body runs as a graph.
     const double apply_cost = (double)h->N * (double)h->N * (h->angular ? 2.3 : 1.0) * (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nv);
     const bool lookahead = apply_cost < 2.0e9;
-    const bool use_graph = lookahead && !h->profiling && std::getenv("LM_NO_GRAPH") == nullptr;
+    const bool use_graph = lookahead && !h->profiling && h->dist_ranks == 0 && std::getenv("LM_NO_GRAPH") == nullptr;
     if (use_graph && remaining > 0) {
         const lm_solver::GraphKey key = {h->V, h->w, h->vec_soa, h->partial, h->pos_soa, kmax, plan.variant, plan.j_splits, h->precision * 8 + nv};
         if (!h->lz_graph || std::memcmp(&key, &h->lz_key, sizeof key) != 0) {
@@ -776,6 +866,8 @@ int lm_create(lm_solver** out, int precision, int64_t N, double eta, double a, i
     h->a = a;
     h->angular = include_angular ? 1 : 0;
     h->npad = (N + NPAD_QUANTUM - 1) / NPAD_QUANTUM * NPAD_QUANTUM;
+    h->row_begin = 0;
+    h->row_end = N;
     auto bail = [&](int code) { lm_destroy(h); return code; };
     if (cudaGetDevice(&h->device) != cudaSuccess) return bail(LM_E_CUDA);
     if (cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess) return bail(LM_E_CUDA);
@@ -807,6 +899,8 @@ int lm_destroy(lm_solver* h)
     for (void* p : h->st) cudaFree(p);
     for (void* p : h->bd) cudaFree(p);
     for (void* p : h->rfd) cudaFree(p);
+    for (void* p : h->gath) cudaFree(p);
+    if (h->nccl_comm && nccl_api().ok) nccl_api().CommDestroy((NcclApi::Comm)h->nccl_comm);
     for (auto e : h->lz_ev) if (e) cudaEventDestroy(e);
     for (auto& pr : h->pending) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
     for (auto e : h->event_pool) cudaEventDestroy(e);
@@ -1064,6 +1158,66 @@ int lm_thermal_drift_rfd(lm_solver* h, const void* noise, double delta, void* li
     cudaStream_t st = (cudaStream_t)stream;
     return h->precision == LM_F32 ? rfd_device<float>(h, (const float*)noise, delta, (float*)lin_out, (float*)ang_out, st)
                                   : rfd_device<double>(h, (const double*)noise, delta, (double*)lin_out, (double*)ang_out, st);
+}
+
+// ---------------------------------------------------------------- row-sharded applies
+int lm_dist_row_block(int64_t N, int nranks, int rank, int64_t* row_begin, int64_t* row_end)
+{
+    if (N <= 0 || nranks < 1 || rank < 0 || rank >= nranks) return LM_E_INVALID;
+    const int64_t B = (N + nranks - 1) / nranks;
+    if (row_begin) *row_begin = std::min<int64_t>(N, (int64_t)rank * B);
+    if (row_end) *row_end = std::min<int64_t>(N, (int64_t)(rank + 1) * B);
+    return LM_OK;
+}
+
+int lm_dist_unique_id(void* out128)
+{
+    if (!out128) return LM_E_NULL;
+    NcclApi& nccl = nccl_api();
+    if (!nccl.ok) return LM_E_CUDA;
+    NcclApi::UniqueId id;
+    if (nccl.GetUniqueId(&id) != 0) return LM_E_CUDA;
+    std::memcpy(out128, id.internal, sizeof id.internal);
+    return LM_OK;
+}
+
+int lm_dist_init(lm_solver* h, int nranks, int rank, const void* unique_id128)
+{
+    if (!h) return LM_E_NULL;
+    h->err.clear();
+    if (!unique_id128) return fail(h, LM_E_NULL, "unique id is NULL");
+    if (h->dist_ranks > 0) return fail(h, LM_E_INVALID, "lm_dist_init was already called on this handle");
+    int64_t b = 0, e = 0;
+    if (lm_dist_row_block(h->N, nranks, rank, &b, &e) != LM_OK) return fail(h, LM_E_INVALID, "need 0 <= rank < nranks");
+    NcclApi& nccl = nccl_api();
+    if (!nccl.ok) return fail(h, LM_E_CUDA, "NCCL unavailable: " + nccl.why);
+    NcclApi::UniqueId id;
+    std::memcpy(id.internal, unique_id128, sizeof id.internal);
+    NcclApi::Comm comm = nullptr;
+    const int nrc = nccl.CommInitRank(&comm, nranks, id, rank);
+    if (nrc != 0) return fail(h, LM_E_CUDA, std::string("ncclCommInitRank failed: ") + nccl.GetErrorString(nrc));
+    h->nccl_comm = comm;
+    h->dist_ranks = nranks;
+    h->dist_rank = rank;
+    h->rows_per_rank = (h->N + nranks - 1) / nranks;
+    h->row_begin = b;
+    h->row_end = e;
+    return LM_OK;
+}
+
+int lm_mdot_rows(lm_solver* h, int64_t row_begin, int64_t row_count, const void* forces, const void* torques, void* lin_out, void* ang_out,
+                 void* stream)
+{
+    if (!h) return LM_E_NULL;
+    h->err.clear();
+    if (h->dist_ranks > 0) return fail(h, LM_E_INVALID, "lm_mdot_rows is for handles without a communicator (lm_dist_init shards by itself)");
+    if (row_begin < 0 || row_count < 0 || row_begin + row_count > h->N) return fail(h, LM_E_INVALID, "row range outside [0, N)");
+    h->row_begin = row_begin;
+    h->row_end = row_begin + row_count;
+    const int rc = lm_mdot_batch(h, 1, forces, torques, lin_out, ang_out, stream);
+    h->row_begin = 0;
+    h->row_end = h->N;
+    return rc;
 }
 
 // ---------------------------------------------------------------- stats / introspection

@@ -133,6 +133,8 @@ template <typename T> struct PairParams {
     RhsOut<T> out;              // j_splits == 1: per right-hand side, 3N interleaved each
     T* __restrict__ partial;    // j_splits  > 1: [j_splits][nrhs*NC][npad]
     int64_t N;
+    int64_t i_begin, i_end;     // target rows handled by this launch: [i_begin, i_end) (whole problem: [0, N));
+                                // i-tile b covers i_begin + b * TARGETS ...  (row-sharded applies)
     int64_t npad;               // multiple of NPAD_QUANTUM (hence of every SUB in use)
     int n_units;                // npad / SUB: the sources are dealt to the gridDim.y j-splits in units of
                                 // SUB, as evenly as possible (split y gets units [y U / S, (y+1) U / S))
@@ -290,7 +292,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
     constexpr unsigned int NWARPS = BLOCK / 32;
 
     const int tid = threadIdx.x;
-    const int64_t i0 = (int64_t)blockIdx.x * Tr::TARGETS;
+    const int64_t i0 = p.i_begin + (int64_t)blockIdx.x * Tr::TARGETS;
     // this CTA's source range [j_begin, j_begin + j_count): a whole number of SUB-source units
     const int u_begin = (int)((int64_t)blockIdx.y * p.n_units / gridDim.y);
     const int u_end = (int)((int64_t)(blockIdx.y + 1) * p.n_units / gridDim.y);
@@ -418,7 +420,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
         for (int half = 0; half < 2; ++half) {
             const int64_t i = i0 + (2 * q + half) * BLOCK + tid;
             if (gridDim.y == 1) {
-                if (i < p.N) {
+                if (i < p.i_end) {
 #pragma unroll
                     for (int r = 0; r < NRHS; ++r) {
                         T* ul = p.out.lin[r] + 3 * i;

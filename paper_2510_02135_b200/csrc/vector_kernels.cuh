@@ -45,11 +45,11 @@ __global__ void __launch_bounds__(VEC_BLOCK) pack_rhs_kernel(RhsIn<T> in, int nr
 // One thread per (right-hand side, component, particle): consecutive threads read consecutive
 // addresses of one partial array; the loads of the splits are independent and unrolled.
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) reduce_partials_kernel(const T* __restrict__ partial, int splits, int nrhs, int nc, int64_t N,
-                                                                    int64_t npad, RhsOut<T> out)
+__global__ void __launch_bounds__(VEC_BLOCK) reduce_partials_kernel(const T* __restrict__ partial, int splits, int nrhs, int nc, int64_t i_begin,
+                                                                    int64_t i_end, int64_t npad, RhsOut<T> out)
 {
-    const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
-    if (i >= N) return;
+    const int64_t i = i_begin + (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;   // target rows [i_begin, i_end)
+    if (i >= i_end) return;
     const int qk = blockIdx.y, q = qk / nc, k = qk % nc;
     const size_t stride = (size_t)nrhs * nc * npad;
     const T* p = partial + (size_t)qk * npad + i;

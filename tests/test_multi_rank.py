@@ -46,3 +46,62 @@ def test_single_process_passthrough_and_seeds():
     from paper_2510_02135_b200 import multi
     assert multi.aggregate_over_ranks(3.5, 7.0) == (3.5, 7.0)
     assert multi.replica_seed(2, 0) == 2 and multi.replica_seed(2, 3) == 3002
+
+
+# ---------------------------------------------------------------- row-sharded applies: host logic (no GPU)
+def test_row_blocks_tile_the_rows():
+    sys.path.insert(0, ROOT)
+    import paper_2510_02135_b200 as lm
+    for N in (1, 2, 7, 64, 1000, 1024, 131072, 1048576 + 3):
+        for G in (1, 2, 3, 4, 8, 16):
+            B = -(-N // G)
+            prev_end = 0
+            for r in range(G):
+                b, e = lm.lm_dist_row_block(N, G, r)
+                assert b == prev_end and b <= e <= N and e - b <= B     # contiguous, in order, at most B rows
+                assert b == min(N, r * B)                                # rank r's all-gather segment starts at 3 B r
+                prev_end = e
+            assert prev_end == N                                         # every row exactly once
+    with pytest.raises(lm.LmError):
+        lm.lm_dist_row_block(10, 2, 2)
+    with pytest.raises(lm.LmError):
+        lm.lm_dist_row_block(0, 2, 0)
+
+
+def _block_worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+    import paper_2510_02135_b200 as lm
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    N = 1001
+    b, e = lm.lm_dist_row_block(N, world, rank)
+    mine = torch.tensor([b, e], dtype=torch.int64)
+    allb = [torch.zeros(2, dtype=torch.int64) for _ in range(world)]
+    dist.all_gather(allb, mine)
+    # what the library's in-place all-gather does, on the host: rank r fills rows [b, e) of a 3 B G buffer
+    B = -(-N // world)
+    seg = torch.full((3 * B,), -1.0, dtype=torch.float64)
+    seg[: 3 * (e - b)] = torch.arange(3 * b, 3 * e, dtype=torch.float64)
+    parts = [torch.zeros(3 * B, dtype=torch.float64) for _ in range(world)]
+    dist.all_gather(parts, seg)
+    full = torch.cat(parts)[: 3 * N]
+    out.put((rank, [t.tolist() for t in allb], bool(torch.equal(full, torch.arange(3 * N, dtype=torch.float64)))))
+    dist.destroy_process_group()
+
+
+def test_row_blocks_across_two_gloo_ranks():
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = 31500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_block_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(out.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    for rank, blocks, ok in res:
+        assert blocks == [[0, 501], [501, 1001]] and ok
