@@ -171,9 +171,9 @@ int lm_thermal_drift_rfd(lm_solver* h, const void* noise, double delta, void* li
  * the same functions in the same order with the same positions / forces / noise, computes only its row
  * block  [r B, min((r+1) B, N)),  B = ceil(N / G)  (lm_dist_row_block), and one grouped ncclAllGather
  * per pair-kernel launch (over NVLink / NVSwitch) completes every output on every rank.  All entry points
- * (lm_mdot*, lm_sqrt_mdot_w*, lm_hydrodynamic_velocities, lm_thermal_drift_rfd, lm_bd_step) then work
- * unchanged; the O(N) vector kernels and lm_steric_forces are replicated.  Ranks must run the same GPU
- * model: the Lanczos stopping decision is taken per rank from bit-identical scalars.
+ * (lm_mdot*, lm_sqrt_mdot_w*, lm_hydrodynamic_velocities, lm_thermal_drift_rfd, lm_steric_forces,
+ * lm_bd_step) then work unchanged; only the O(N) vector kernels are replicated.  Ranks must run the
+ * same GPU model: the Lanczos stopping decision is taken per rank from bit-identical scalars.
  *   lm_dist_unique_id : 128-byte NCCL unique id (host buffer); call on ONE rank and broadcast it to the
  *                       others by any means (torch.distributed, MPI, a file).
  *   lm_dist_init      : collective; creates this handle's communicator (current CUDA device) and fixes

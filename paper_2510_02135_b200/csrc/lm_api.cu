@@ -684,27 +684,44 @@ int steric_device(lm_solver* h, double U0, double b, const T* ext, T* out, cudaS
         h->steric_attr_set = true;
     }
     const int units = (int)(h->npad / STERIC_SUB);
-    const int i_tiles = (int)((h->N + STERIC_TARGETS - 1) / STERIC_TARGETS);
+    const int64_t rows = std::max<int64_t>(h->row_end - h->row_begin, 0);      // this rank's target rows (all rows unless sharded)
+    const int i_tiles = (int)((rows + STERIC_TARGETS - 1) / STERIC_TARGETS);
     // about four resident sets of CTAs (2 per SM): the work per CTA depends on how many groups are within the cut-off
-    const int splits = (int)std::max<int64_t>(1, std::min<int64_t>(units, ((int64_t)8 * h->sm_count + i_tiles - 1) / i_tiles));
+    const int splits = (int)std::max<int64_t>(1, std::min<int64_t>(units, ((int64_t)8 * h->sm_count + std::max(i_tiles, 1) - 1) / std::max(i_tiles, 1)));
     int rc = ensure(h, &h->partial, &h->partial_bytes, (size_t)splits * 3 * h->npad * sizeof(T));
     if (rc != LM_OK) return rc;
+    const bool dist = h->dist_ranks > 0;
+    const size_t seg = (size_t)3 * h->rows_per_rank;
+    T* kout = out;
+    if (dist) {
+        if ((rc = ensure(h, &h->gath[0], &h->gath_bytes[0], seg * h->dist_ranks * sizeof(T))) != LM_OK) return rc;
+        kout = (T*)h->gath[0];
+    }
     const double K = sizeof(T) == 4 ? 20.0 : 40.0;           // exp(-K) below the type's epsilon
     StericParams<T> p;
     p.pos = (const T*)h->pos_soa;
     p.partial = (T*)h->partial;
     p.N = h->N;
     p.npad = h->npad;
+    p.i_begin = h->row_begin;
     p.n_units = units;
     p.tiny = make_consts<T>(h->eta, h->a).tiny;
     p.d = (T)(2.0 * h->a);
     p.rc2 = (T)((2.0 * h->a + K * b) * (2.0 * h->a + K * b));
     p.m0 = (T)(U0 / b);
     p.inv_b = (T)(sizeof(T) == 4 ? 1.4426950408889634 / b : 1.0 / b);
-    steric_pair_kernel<T><<<dim3(i_tiles, splits), STERIC_BLOCK, steric_smem_bytes<T>(), st>>>(p);
-    steric_reduce_kernel<T><<<grid_1d(h->N), VEC_BLOCK, 0, st>>>((const T*)h->partial, splits, h->N, h->npad, ext, out);
-    h->n_aux += 2;
+    if (i_tiles > 0) {
+        steric_pair_kernel<T><<<dim3(i_tiles, splits), STERIC_BLOCK, steric_smem_bytes<T>(), st>>>(p);
+        steric_reduce_kernel<T><<<grid_1d(rows), VEC_BLOCK, 0, st>>>((const T*)h->partial, splits, h->row_begin, h->row_end, h->npad, ext, kout);
+        h->n_aux += 2;
+    }
     LM_CUDA(h, cudaGetLastError());
+    if (dist) {                                              // row blocks -> every rank (as in launch_pair)
+        NcclApi& nccl = nccl_api();
+        const int nrc = nccl.AllGather(kout + seg * h->dist_rank, kout, seg, sizeof(T) == 4 ? NCCL_FLOAT32 : NCCL_FLOAT64, (NcclApi::Comm)h->nccl_comm, st);
+        if (nrc != 0) return fail(h, LM_E_CUDA, std::string("ncclAllGather failed: ") + nccl.GetErrorString(nrc));
+        LM_CUDA(h, cudaMemcpyAsync(out, kout, (size_t)3 * h->N * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    }
     return LM_OK;
 }
 

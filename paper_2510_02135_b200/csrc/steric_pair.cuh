@@ -21,6 +21,7 @@ template <typename T> struct StericParams {
     const T* __restrict__ pos;   // [3][npad]  x | y | z
     T* __restrict__ partial;     // [j_splits][3][npad]
     int64_t N, npad;
+    int64_t i_begin;             // first target row of this launch (row-sharded runs; 0 otherwise)
     int n_units;                 // npad / STERIC_SUB
     T tiny;                      // floor of r^2 (as in the RPY kernel)
     T d;                         // contact distance 2a
@@ -50,7 +51,7 @@ __global__ void __launch_bounds__(STERIC_BLOCK, 2) steric_pair_kernel(const Ster
     unsigned int* done = reinterpret_cast<unsigned int*>(full + STAGES);
 
     const int tid = threadIdx.x;
-    const int64_t i0 = (int64_t)blockIdx.x * STERIC_TARGETS;
+    const int64_t i0 = p.i_begin + (int64_t)blockIdx.x * STERIC_TARGETS;
     const int u_begin = (int)((int64_t)blockIdx.y * p.n_units / gridDim.y);
     const int u_end = (int)((int64_t)(blockIdx.y + 1) * p.n_units / gridDim.y);
     const int64_t j_begin = (int64_t)u_begin * SUB;
@@ -145,11 +146,11 @@ __global__ void __launch_bounds__(STERIC_BLOCK, 2) steric_pair_kernel(const Ster
 
 // F[3i+k] = ext[3i+k] + sum over splits of partial  (fixed order: deterministic)
 template <typename T>
-__global__ void __launch_bounds__(256) steric_reduce_kernel(const T* __restrict__ partial, int splits, int64_t N, int64_t npad,
+__global__ void __launch_bounds__(256) steric_reduce_kernel(const T* __restrict__ partial, int splits, int64_t i_begin, int64_t i_end, int64_t npad,
                                                             const T* __restrict__ ext, T* __restrict__ out)
 {
-    const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
-    if (i >= N) return;
+    const int64_t i = i_begin + (int64_t)blockIdx.x * 256 + threadIdx.x;   // target rows [i_begin, i_end)
+    if (i >= i_end) return;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         T s = ext ? ext[3 * i + k] : T(0);
