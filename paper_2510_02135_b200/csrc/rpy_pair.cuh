@@ -15,19 +15,22 @@
 //     instruction, which is what the sm_100 register file can feed at the FMA pipe's rate;
 //   * sources are staged as structure-of-arrays tiles by 1-D TMA bulk copies
 //     (cp.async.bulk.shared::cluster.global, SASS UBLKCP) completing on an mbarrier,
-//     double buffered -- no thread issues a global load in the main loop;
+//     double buffered -- no thread issues a global load in the main loop; a stage is released
+//     without a CTA barrier: every warp counts itself out, the last one out issues the refill;
 //   * fp32 arithmetic is packed two targets per instruction (FFMA2 / FMUL2 / FADD2, the
 //     sm_100 f32x2 forms);  1/r from MUFU.RSQ (fp32) or MUFU.RSQ64H + one cubically convergent
 //     correction (fp64);
-//   * overlap (r < 2a) / far-field select without divergence and without paying for it where
-//     no pair overlaps: sources are walked in chunks of SUB; a chunk is first evaluated with the
-//     FAR-FIELD formulas only while a predicate collects (r^2 < 4a^2) over all its pairs; one
-//     warp vote per chunk decides whether the chunk is accepted or re-evaluated with the
-//     GENERAL body (both branches + per-lane FSEL).  Dense regions lock the warp onto the
-//     general body, so the worst case costs what the plain select kernel costs;
+//   * overlap (r < 2a) / far-field select without divergence, nothing evaluated twice, and the
+//     near formulas paid for only where pairs overlap: sources are walked in groups of GS (2 or 4);
+//     the geometry (d, r^2) of the whole group x all the thread's packed pairs comes first while a
+//     running minimum collects min r^2; ONE warp vote per group then picks the FAR-FIELD body (no
+//     near formulas, no selects) or the GENERAL body (both branches + per-lane FSEL) BEFORE
+//     anything is accumulated;
 //   * r = 0 is made safe by a tiny additive floor inside the r^2 FMA chain (no extra instruction);
-//   * two-level accumulation: the per-chunk packed accumulator is flushed into a per-thread
-//     total at every chunk end (keeps the fp32 summation error ~ eps*(sqrt(SUB)+sqrt(N/SUB))).
+//   * two-level accumulation: the per-tile packed accumulator is flushed into a per-thread total
+//     at every tile end (keeps the fp32 summation error ~ eps*(sqrt(TJ)+sqrt(N/TJ)));
+//   * the sources are dealt to the gridDim.y j-splits in units of SUB, the targets handled are the
+//     rows [i_begin, i_end) (the whole problem, or one rank's block of a row-sharded apply).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
