@@ -179,9 +179,12 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 //   FAR == true : far-field formulas only (the caller has checked that no pair of the group overlaps).
 //   FAR == false: both branches, selected per lane.
 // (nx, ny, nz) = -x_i of the two targets; (xj, yj, zj), V[] = the source, warp-uniform scalars.
-template <typename T> struct PairGeom { P2<T> dx, dy, dz, r2; };
+template <typename T> struct PairGeom { P2<T> dx, dy, dz, r2, invr; };
 
-template <typename T>
+// EARLY_RSQRT: issue the MUFU before the vote, so that its latency overlaps the vote and the branch;
+// pays off where the apply body is long (angular, 4 right-hand sides: measured +2 %), costs ~1 % in
+// register pressure on the short translational bodies, which therefore take 1/r after the vote.
+template <typename T, bool EARLY_RSQRT>
 __device__ __forceinline__ PairGeom<T> pair_geom(const PairConsts<T>& c, P2<T> nx, P2<T> ny, P2<T> nz, T xj, T yj, T zj,
                                                  typename NearOf<T>::type& near)
 {
@@ -191,16 +194,17 @@ __device__ __forceinline__ PairGeom<T> pair_geom(const PairConsts<T>& c, P2<T> n
     g.dz = add2(nz, zj);
     g.r2 = fma2(g.dz, g.dz, fma2(g.dy, g.dy, fma2(g.dx, g.dx, splat(c.tiny))));
     near_update(near, lo(g.r2), hi(g.r2));
+    if constexpr (EARLY_RSQRT) g.invr = rsqrt2(g.r2);
     return g;
 }
 
-template <typename T, int NRHS, bool ANG, bool FAR>
+template <typename T, int NRHS, bool ANG, bool FAR, bool EARLY_RSQRT>
 __device__ __forceinline__ void pair_apply(const PairConsts<T>& c, const PairGeom<T>& gm, const T (&V)[NRHS * (ANG ? 6 : 3)],
                                            P2<T> (&acc)[NRHS * (ANG ? 6 : 3)])
 {
     constexpr int NC = ANG ? 6 : 3;
     const P2<T> dx = gm.dx, dy = gm.dy, dz = gm.dz, r2 = gm.r2;
-    const P2<T> invr = rsqrt2(r2);
+    const P2<T> invr = EARLY_RSQRT ? gm.invr : rsqrt2(r2);
     const P2<T> u = mul2(invr, invr);
     const P2<T> w3 = mul2(invr, u);
     P2<T> w5, f, g, r;
@@ -287,6 +291,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
     using Tr = PairKernelTraits<T, NRHS, ANG, TPT, BLOCK, TJ, STAGES, SUB>;
     constexpr int NC = Tr::NC, NV = Tr::NV, NP = Tr::NP, ARRAYS = Tr::ARRAYS;
     constexpr int VN = Vec16<T>::N, GS = Tr::GS;
+    constexpr bool EARLY = ANG || NRHS >= 4;
     using V16 = typename Vec16<T>::type;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     T* tiles = reinterpret_cast<T*>(smem_raw);
@@ -380,7 +385,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
                 for (int e = 0; e < GS; ++e)
 #pragma unroll
                     for (int q = 0; q < NP; ++q)
-                        gm[e][q] = pair_geom<T>(p.c, nx[q], ny[q], nz[q], vget(X, e0 + e), vget(Y, e0 + e), vget(Z, e0 + e), near);
+                        gm[e][q] = pair_geom<T, EARLY>(p.c, nx[q], ny[q], nz[q], vget(X, e0 + e), vget(Y, e0 + e), vget(Z, e0 + e), near);
                 const bool hit = __any_sync(0xffffffffu, near_test(near, p.c.four_a2));
                 auto body = [&](auto far_tag) {
                     constexpr bool FAR = decltype(far_tag)::value;
@@ -390,7 +395,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 #pragma unroll
                         for (int k = 0; k < NV; ++k) Vs[k] = vget(Vv[k], e0 + e);
 #pragma unroll
-                        for (int q = 0; q < NP; ++q) pair_apply<T, NRHS, ANG, FAR>(p.c, gm[e][q], Vs, acc[q]);
+                        for (int q = 0; q < NP; ++q) pair_apply<T, NRHS, ANG, FAR, EARLY>(p.c, gm[e][q], Vs, acc[q]);
                     }
                 };
                 if (!hit) body(std::true_type{});
