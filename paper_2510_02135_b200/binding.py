@@ -137,7 +137,10 @@ def _ptr(x):
 def _stream_ptr(stream):
     if stream is None:
         import torch
-        return c_void_p(torch.cuda.current_stream().cuda_stream)
+        try:                               # the raw handle of torch's current stream, without building a Stream object
+            return c_void_p(torch._C._cuda_getCurrentRawStream(torch.cuda.current_device()))
+        except AttributeError:
+            return c_void_p(torch.cuda.current_stream().cuda_stream)
     if isinstance(stream, int):
         return c_void_p(stream)
     return c_void_p(stream.cuda_stream)

@@ -178,6 +178,18 @@ struct lm_solver {
     std::vector<Variant<float>> vf;
     std::vector<Variant<double>> vd;
 
+    // launch plans are pure functions of (nrhs, row range): cached, the chooser's search is off the per-call path
+    struct PlanSlot { bool valid = false; int64_t rb = 0, re = 0; lm::LaunchPlan plan; } plan_cache[lm::MAX_RHS + 1];
+
+    // small-N applies (pack + pair kernel + reduce) replayed as a CUDA graph when called again with the same buffers
+    struct ApplyKey {
+        const void *f[lm::MAX_RHS], *t[lm::MAX_RHS], *lin[lm::MAX_RHS], *ang[lm::MAX_RHS];
+        const void *pos, *vec, *partial;
+        int64_t rb, re;
+        int nrhs, variant, splits, pad;
+    };
+    struct ApplySlot { bool have_last = false; ApplyKey last, graph_key; cudaGraphExec_t exec = nullptr; } apply_graph[lm::MAX_RHS + 1];
+
     // stats
     int64_t n_pair = 0, n_aux = 0;
     double pairs = 0.0, pair_ms = 0.0;
@@ -268,6 +280,10 @@ template <typename T> int init_variants(lm_solver* h)
 // (its sources + a fixed prologue/epilogue) x its targets; CTAs resident on one SM share it.
 template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
 {
+    if (nrhs >= 0 && nrhs <= MAX_RHS) {
+        const auto& slot = h->plan_cache[nrhs];
+        if (slot.valid && slot.rb == h->row_begin && slot.re == h->row_end) return slot.plan;
+    }
     const auto& vs = variants<T>(h);
     LaunchPlan best;
     double best_cost = 1e300;
@@ -302,6 +318,13 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
                 best.n_units = units;
             }
         }
+    }
+    if (nrhs >= 0 && nrhs <= MAX_RHS) {
+        auto& slot = h->plan_cache[nrhs];
+        slot.valid = true;
+        slot.rb = h->row_begin;
+        slot.re = h->row_end;
+        slot.plan = best;
     }
     return best;
 }
@@ -415,15 +438,62 @@ void count_apply(lm_solver* h, const LaunchPlan& plan)
     if (plan.j_splits > 1) h->n_aux++;
 }
 
+int ensure_capture_stream(lm_solver* h)
+{
+    if (!h->cap_stream) LM_CUDA(h, cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+    return LM_OK;
+}
+
 template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& in, const RhsOut<T>& out, cudaStream_t st)
 {
     const int nc = h->angular ? 6 : 3;
     LaunchPlan plan;
     int rc = prepare_apply<T>(h, nrhs, plan);
     if (rc != LM_OK) return rc;
-    pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>(in, nrhs, nc, h->N, h->npad, (T*)h->vec_soa);
+    auto direct = [&](cudaStream_t s2, bool timed) -> int {
+        pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(in, nrhs, nc, h->N, h->npad, (T*)h->vec_soa);
+        return launch_pair<T>(h, nrhs, plan, out, s2, timed);
+    };
+    // A short apply is bound by the host's three launches (~11 us measured against ~3 us of kernels each): when
+    // the SAME call (same buffers, same plan) comes twice in a row -- a time-stepping loop -- it is captured
+    // once and replayed as a CUDA graph from then on; any other call is launched directly.
+    const double cost = (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N * (h->angular ? 2.3 : 1.0) *
+                        (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nrhs);
+    if (cost < 2.0e9 && !h->profiling && h->dist_ranks == 0 && std::getenv("LM_NO_GRAPH") == nullptr) {
+        lm_solver::ApplyKey key;
+        std::memset(&key, 0, sizeof key);
+        for (int q = 0; q < nrhs; ++q) { key.f[q] = in.f[q]; key.t[q] = in.t[q]; key.lin[q] = out.lin[q]; key.ang[q] = out.ang[q]; }
+        key.pos = h->pos_soa; key.vec = h->vec_soa; key.partial = h->partial;
+        key.rb = h->row_begin; key.re = h->row_end;
+        key.nrhs = nrhs; key.variant = plan.variant; key.splits = plan.j_splits;
+        auto& slot = h->apply_graph[nrhs];
+        bool replay = slot.exec && std::memcmp(&key, &slot.graph_key, sizeof key) == 0;
+        if (!replay && slot.have_last && std::memcmp(&key, &slot.last, sizeof key) == 0) {
+            if ((rc = ensure_capture_stream(h)) != LM_OK) return rc;
+            if (slot.exec) { LM_CUDA(h, cudaGraphExecDestroy(slot.exec)); slot.exec = nullptr; }
+            cudaGraph_t graph = nullptr;
+            LM_CUDA(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+            const int rc_body = direct(h->cap_stream, false);
+            const cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
+            if (rc_body != LM_OK) { if (graph) cudaGraphDestroy(graph); return rc_body; }
+            LM_CUDA(h, ce);
+            const cudaError_t ci = cudaGraphInstantiate(&slot.exec, graph, 0);
+            cudaGraphDestroy(graph);
+            LM_CUDA(h, ci);
+            slot.graph_key = key;
+            replay = true;
+        }
+        slot.last = key;
+        slot.have_last = true;
+        if (replay) {
+            LM_CUDA(h, cudaGraphLaunch(slot.exec, st));
+            h->n_aux++;
+            count_apply(h, plan);
+            return LM_OK;
+        }
+    }
+    if ((rc = direct(st, h->profiling)) != LM_OK) return rc;
     h->n_aux++;
-    if ((rc = launch_pair<T>(h, nrhs, plan, out, st, h->profiling)) != LM_OK) return rc;
     count_apply(h, plan);
     return LM_OK;
 }
@@ -474,8 +544,8 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
         LM_CUDA(h, cudaMalloc((void**)&h->d_newest, sizeof(int)));
         LM_CUDA(h, cudaMemsetAsync(h->d_ticket, 0, sizeof(unsigned int), st));
         for (auto& e : h->lz_ev) LM_CUDA(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-        LM_CUDA(h, cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
     }
+    if ((rc = ensure_capture_stream(h)) != LM_OK) return rc;
     if (h->coef_cap < (size_t)(kmax + 2)) {
         if (h->d_coef) { LM_CUDA(h, cudaFree(h->d_coef)); LM_CUDA(h, cudaFree(h->d_gram_part)); LM_CUDA(h, cudaFreeHost(h->h_gram)); LM_CUDA(h, cudaFreeHost(h->h_ab)); }
         h->d_coef = nullptr;
@@ -912,6 +982,7 @@ int lm_destroy(lm_solver* h)
     if (h->h_gram) cudaFreeHost(h->h_gram);
     if (h->h_ab) cudaFreeHost(h->h_ab);
     if (h->lz_graph) cudaGraphExecDestroy(h->lz_graph);
+    for (auto& g : h->apply_graph) if (g.exec) cudaGraphExecDestroy(g.exec);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     for (void* p : h->st) cudaFree(p);
     for (void* p : h->bd) cudaFree(p);
