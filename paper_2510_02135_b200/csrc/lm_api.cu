@@ -459,7 +459,7 @@ template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& i
     // once and replayed as a CUDA graph from then on; any other call is launched directly.
     const double cost = (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N * (h->angular ? 2.3 : 1.0) *
                         (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nrhs);
-    if (cost < 2.0e9 && !h->profiling && h->dist_ranks == 0 && std::getenv("LM_NO_GRAPH") == nullptr) {
+    if (cost < 2.0e8 && !h->profiling && h->dist_ranks == 0 && std::getenv("LM_NO_GRAPH") == nullptr) {      // N <~ 14000 fp32
         lm_solver::ApplyKey key;
         std::memset(&key, 0, sizeof key);
         for (int q = 0; q < nrhs; ++q) { key.f[q] = in.f[q]; key.t[q] = in.t[q]; key.lin[q] = out.lin[q]; key.ang[q] = out.ang[q]; }
