@@ -479,3 +479,37 @@ def test_sqrt_mdot_w_batch_noconv_and_errors(lm, torch):
         s.sqrt_mdot_w_batch(0, dev(torch, W).reshape(-1)[:0], 1e-3, lin[:0])
     assert e.value.code in (lm.LM_E_INVALID, lm.LM_E_NULL)
     s.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_repeated_small_applies_replay_a_graph_on_current_data(lm, torch, prec):
+    """Short applies called again with the same buffers are replayed as a CUDA graph: the
+    replay must read the buffers' CURRENT contents (forces changed in place, positions re-set), and calls with
+    other buffers, other right-hand-side counts or a row range must not be served by a stale graph."""
+    N = 700
+    c = workloads.random_case(N, 15.0, 77, prec, False)
+    s = lm.Solver(prec, N)
+    X, F = dev(torch, c["pos"]).reshape(-1), dev(torch, c["forces"]).reshape(-1).clone()
+    U = torch.empty(3 * N, dtype=s.torch_dtype, device="cuda")
+    s.set_positions(X)
+    pos, f = np.asarray(c["pos"], np.float64), np.asarray(c["forces"], np.float64)
+    for it in range(5):                                   # direct, capture, replay, replay, replay
+        s.mdot(F, None, U)
+        torch.cuda.synchronize()
+        assert rel(U.cpu().numpy(), rpy.mdot(pos, f)[0]) <= TOL[prec], it
+        F.mul_(-1.5)                                      # same buffer, new contents
+        f = f * -1.5
+    X2 = (X * 1.25).contiguous()
+    s.set_positions(X2)                                   # same packed buffer inside the handle, new contents
+    s.mdot(F, None, U)
+    torch.cuda.synchronize()
+    assert rel(U.cpu().numpy(), rpy.mdot(X2.cpu().numpy().reshape(N, 3), f)[0]) <= TOL[prec]
+    U2 = torch.empty_like(U)                              # another output buffer: not the captured call
+    s.mdot(F, None, U2)
+    s.mdot_rows(100, 50, F, None, U2)                     # a row range in between
+    s.mdot(F, None, U)
+    s.mdot(F, None, U)
+    torch.cuda.synchronize()
+    ref = rpy.mdot(X2.cpu().numpy().reshape(N, 3), f)[0]
+    assert rel(U2.cpu().numpy(), ref) <= TOL[prec] and rel(U.cpu().numpy(), ref) <= TOL[prec]
+    s.close()
