@@ -1,4 +1,7 @@
-// lm_api.cu -- C ABI of liblm (include/lm.h): handle, launch configuration, Lanczos driver.
+// lm_api.cu -- C ABI of liblm (include/lm.h).  One translation unit: the device kernels (rpy_pair.cuh,
+// steric_pair.cuh, vector_kernels.cuh), then the host side in include order: lm_handle.cuh (state, launch
+// chooser), lm_apply.cuh (one M.F apply), lm_lanczos.cuh (M^{1/2} W driver), lm_bd.cuh (eqs. 11, 13, 14),
+// and below the typed front ends and the extern "C" entry points.
 //
 // Everything numerical runs in the kernels of rpy_pair.cuh / vector_kernels.cuh; the only host
 // arithmetic is the k x k tridiagonal problem of the Lanczos stopping test (tridiag_host.h).
@@ -21,843 +24,12 @@
 #include "tridiag_host.h"
 #include "vector_kernels.cuh"
 
-namespace lm {
-
-// ---------------------------------------------------------------- pair-kernel variants
-// LARGE: 256 threads x TPT targets (TPT/2 packed pairs per thread), tiles of up to 512 sources.
-// SMALL: 64 x 2, tiles of up to 64 sources (fills 148 SMs when N is small, SURVEY.md sec. 7 "Small N").
-// SUB = sources per overlap-vote chunk = the unit in which sources are dealt to the j-splits;
-// npad is a multiple of NPAD_QUANTUM, which every SUB divides.
-constexpr int NPAD_QUANTUM = 32;
-constexpr int L_BLOCK = 256, L_TJ = 512, L_STAGES = 2;
-constexpr int S_BLOCK = 64, S_TPT = 2, S_TJ = 64, S_STAGES = 2;
-constexpr int64_t MAX_SOURCES_PER_CTA = 262144;   // bounds the top level of the two-level fp32 summation
-
-template <typename T> struct Variant {
-    void (*kernel)(const PairParams<T>);
-    int nrhs, ang, block, tpt, tj, sub, smem;
-    int ctas_per_sm;      // filled at first use (occupancy API)
-    double efficiency;    // relative per-pair throughput used by the launch chooser
-};
-
-template <typename T, int NRHS, bool ANG, int TPT, int SUB, int MINB> Variant<T> make_large()
-{
-    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB>;
-    static_assert(NPAD_QUANTUM % SUB == 0, "every SUB divides NPAD_QUANTUM");
-    return {rpy_pair_kernel<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB, MINB>, NRHS, ANG, L_BLOCK, TPT, L_TJ, SUB, Tr::SMEM_BYTES, 0, 1.0};
-}
-template <typename T, int NRHS, bool ANG, int SUB, int MINB> Variant<T> make_small()
-{
-    using Tr = PairKernelTraits<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB>;
-    static_assert(NPAD_QUANTUM % SUB == 0, "every SUB divides NPAD_QUANTUM");
-    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB, MINB>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, SUB, Tr::SMEM_BYTES, 0, 0.8};
-}
-
-template <typename T> std::vector<Variant<T>> build_variants();
-template <> std::vector<Variant<float>> build_variants<float>()
-{
-    return {make_large<float, 1, false, 4, 32, 2>(), make_large<float, 2, false, 4, 32, 1>(), make_large<float, 4, false, 4, 32, 1>(),
-            make_large<float, 1, true, 2, 32, 2>(),  make_large<float, 2, true, 2, 32, 1>(),
-            make_small<float, 1, false, 32, 8>(), make_small<float, 2, false, 32, 8>(), make_small<float, 4, false, 32, 6>(),
-            make_small<float, 1, true, 32, 8>(),  make_small<float, 2, true, 32, 6>()};
-}
-template <> std::vector<Variant<double>> build_variants<double>()
-{
-    return {make_large<double, 1, false, 4, 32, 1>(), make_large<double, 2, false, 2, 32, 1>(), make_large<double, 4, false, 2, 32, 1>(),
-            make_large<double, 1, true, 2, 32, 1>(),  make_large<double, 2, true, 2, 32, 1>(),
-            make_small<double, 1, false, 32, 8>(), make_small<double, 2, false, 32, 6>(), make_small<double, 4, false, 32, 4>(),
-            make_small<double, 1, true, 32, 6>(),  make_small<double, 2, true, 32, 4>()};
-}
-
-struct LaunchPlan {
-    int variant = -1;
-    int i_tiles = 0, j_splits = 0, n_units = 0;
-};
-
-}  // namespace lm
-
-// ---------------------------------------------------------------- NCCL, loaded at run time (row-sharded applies only)
-// The library does not link NCCL: a single-GPU user never needs it.  lm_dist_* resolve the few entry
-// points below from the libnccl already in the process (PyTorch's) or, failing that, the system one.
-namespace lm {
-struct NcclApi {
-    struct UniqueId { char internal[128]; };
-    typedef void* Comm;
-    int (*GetUniqueId)(UniqueId*) = nullptr;
-    int (*CommInitRank)(Comm*, int, UniqueId, int) = nullptr;
-    int (*CommDestroy)(Comm) = nullptr;
-    int (*AllGather)(const void*, void*, size_t, int, Comm, cudaStream_t) = nullptr;
-    int (*GroupStart)() = nullptr;
-    int (*GroupEnd)() = nullptr;
-    const char* (*GetErrorString)(int) = nullptr;
-    bool ok = false;
-    std::string why;
-};
-constexpr int NCCL_FLOAT32 = 7, NCCL_FLOAT64 = 8;   // ncclDataType_t values (nccl.h)
-
-inline NcclApi& nccl_api()
-{
-    static NcclApi api;
-    static bool tried = false;
-    if (tried) return api;
-    tried = true;
-    void* lib = dlopen("libnccl.so.2", RTLD_NOW | RTLD_NOLOAD);
-    if (!lib) lib = dlopen("libnccl.so.2", RTLD_NOW | RTLD_GLOBAL);
-    if (!lib) { api.why = std::string("cannot load libnccl.so.2: ") + dlerror(); return api; }
-    auto sym = [&](const char* name) { void* p = dlsym(lib, name); if (!p) api.why = std::string("libnccl.so.2 lacks ") + name; return p; };
-    api.GetUniqueId = (int (*)(NcclApi::UniqueId*))sym("ncclGetUniqueId");
-    api.CommInitRank = (int (*)(NcclApi::Comm*, int, NcclApi::UniqueId, int))sym("ncclCommInitRank");
-    api.CommDestroy = (int (*)(NcclApi::Comm))sym("ncclCommDestroy");
-    api.AllGather = (int (*)(const void*, void*, size_t, int, NcclApi::Comm, cudaStream_t))sym("ncclAllGather");
-    api.GroupStart = (int (*)())sym("ncclGroupStart");
-    api.GroupEnd = (int (*)())sym("ncclGroupEnd");
-    api.GetErrorString = (const char* (*)(int))sym("ncclGetErrorString");
-    api.ok = api.GetUniqueId && api.CommInitRank && api.CommDestroy && api.AllGather && api.GroupStart && api.GroupEnd && api.GetErrorString;
-    return api;
-}
-}  // namespace lm
-
-using namespace lm;
-
-// ---------------------------------------------------------------- handle
-struct lm_solver {
-    int precision = LM_F32;
-    int64_t N = 0, npad = 0;
-    double eta = 1.0, a = 1.0;
-    int angular = 0;
-    int max_iter = 100;
-    int device = 0, sm_count = 0;
-    bool have_pos = false;
-    std::string err;
-    int last_iters = -1;
-
-    void* pos_soa = nullptr;
-    void* vec_soa = nullptr;   size_t vec_soa_bytes = 0;
-    void* partial = nullptr;   size_t partial_bytes = 0;
-
-    // Lanczos workspace
-    void* V = nullptr;         size_t V_bytes = 0;
-    void* w = nullptr;         size_t w_bytes = 0;
-    double* d_scal = nullptr;  // [0] |z|^2  [1] alpha  [2] beta^2
-    double* d_block = nullptr; // block partials of the reductions
-    unsigned int* d_ticket = nullptr;
-    int* d_newest = nullptr;   // index of the newest basis vector (read by the iteration's kernels)
-    double* d_coef = nullptr;  size_t coef_cap = 0;   // coef_cap also sizes the buffers below
-    double* d_gram_part = nullptr;
-    // mapped pinned host memory the kernels write the stopping-test scalars into
-    double* h_ab = nullptr;    // [1] |z|^2; [2k], [2k+1]: alpha_k, beta_k^2
-    double* h_gram = nullptr;  // column c at [c * (max_iter + 2) + j] = V[j].V[c], j <= c
-    cudaEvent_t lz_ev[2] = {nullptr, nullptr};   // iteration k's scalars have landed (parity k & 1)
-    // one Lanczos iteration captured as a CUDA graph (small N: the loop is launch-bound)
-    cudaStream_t cap_stream = nullptr;
-    cudaGraphExec_t lz_graph = nullptr;
-    struct GraphKey { const void *V, *w, *vec, *partial, *pos; int kmax, variant, splits, prec; } lz_key = {nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0};
-
-    // Brownian-dynamics step (lm_bd_step): F, v_n, v_{n-1}, noise velocity, angular scratch x2, position staging
-    void* bd[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    size_t bd_bytes[7] = {0, 0, 0, 0, 0, 0, 0};
-    bool bd_have_prev = false;
-    bool steric_attr_set = false;
-    // random finite difference (lm_thermal_drift_rfd): displaced packed positions, U(X-) linear / angular
-    void* rfd[3] = {nullptr, nullptr, nullptr};
-    size_t rfd_bytes[3] = {0, 0, 0};
-
-    // row-sharded applies over NCCL (lm_dist_init): rank r computes target rows [r B, min((r+1) B, N)), B = rows_per_rank
-    int dist_ranks = 0, dist_rank = 0;        // dist_ranks == 0: not distributed
-    int64_t rows_per_rank = 0;
-    void* nccl_comm = nullptr;
-    void* gath[2 * MAX_RHS] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // all-gather buffers, 3 B ranks each
-    size_t gath_bytes[2 * MAX_RHS] = {0, 0, 0, 0, 0, 0, 0, 0};
-    int64_t row_begin = 0, row_end = 0;       // the target rows every apply computes ([0, N) unless sharded / lm_mdot_rows)
-
-    // staging for the _host entry points
-    void* st[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // pos, f, t, noise, lin, ang
-    size_t st_bytes[6] = {0, 0, 0, 0, 0, 0};
-
-    // variants (typed; only the handle's precision is populated)
-    std::vector<Variant<float>> vf;
-    std::vector<Variant<double>> vd;
-
-    // launch plans are pure functions of (nrhs, row range): cached, the chooser's search is off the per-call path
-    struct PlanSlot { bool valid = false; int64_t rb = 0, re = 0; lm::LaunchPlan plan; } plan_cache[lm::MAX_RHS + 1];
-
-    // small-N applies (pack + pair kernel + reduce) replayed as a CUDA graph when called again with the same buffers
-    struct ApplyKey {
-        const void *f[lm::MAX_RHS], *t[lm::MAX_RHS], *lin[lm::MAX_RHS], *ang[lm::MAX_RHS];
-        const void *pos, *vec, *partial;
-        int64_t rb, re;
-        int nrhs, variant, splits, pad;
-    };
-    struct ApplySlot { bool have_last = false; ApplyKey last, graph_key; cudaGraphExec_t exec = nullptr; } apply_graph[lm::MAX_RHS + 1];
-
-    // stats
-    int64_t n_pair = 0, n_aux = 0;
-    double pairs = 0.0, pair_ms = 0.0;
-    bool profiling = false;
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> pending;
-    std::vector<cudaEvent_t> event_pool;
-};
+#include "lm_handle.cuh"
+#include "lm_apply.cuh"
+#include "lm_lanczos.cuh"
+#include "lm_bd.cuh"
 
 namespace {
-
-int fail(lm_solver* h, int code, const std::string& msg)
-{
-    if (h) h->err = msg;
-    return code;
-}
-
-#define LM_CUDA(h, expr)                                                                              \
-    do {                                                                                              \
-        cudaError_t e__ = (expr);                                                                     \
-        if (e__ != cudaSuccess) {                                                                     \
-            char buf__[512];                                                                          \
-            std::snprintf(buf__, sizeof buf__, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
-            return fail(h, LM_E_CUDA, buf__);                                                         \
-        }                                                                                             \
-    } while (0)
-
-size_t esize(const lm_solver* h) { return h->precision == LM_F32 ? 4 : 8; }
-int64_t dof_of(const lm_solver* h) { return (h->angular ? 6 : 3) * h->N; }
-
-int ensure(lm_solver* h, void** ptr, size_t* cap, size_t bytes)
-{
-    if (*cap >= bytes && *ptr) return LM_OK;
-    if (*ptr) LM_CUDA(h, cudaFree(*ptr));
-    *ptr = nullptr;
-    *cap = 0;
-    LM_CUDA(h, cudaMalloc(ptr, bytes));
-    *cap = bytes;
-    return LM_OK;
-}
-
-template <typename T> PairConsts<T> make_consts(double eta, double a)
-{
-    const double pi = 3.14159265358979323846264338327950288;
-    PairConsts<T> c;
-    const double c4 = 4.0 / (3.0 * a);                 // (1/(6 pi eta a)) / C1: translational self mobility
-    const double c8 = 1.0 / (a * a * a);               // (1/(8 pi eta a^3)) / C1: rotational self mobility
-    // floor of r^2: r = 0 becomes r = a 2^-40 (fp32) / a 2^-100 (fp64): a relative perturbation of the
-    // self term far below the type's epsilon, while 1/r^3 stays finite (1/r^5 may overflow to +inf in
-    // fp32; it only feeds the far branch, which the select discards for r < 2a)
-    c.tiny = (T)std::max(a * a * std::ldexp(1.0, sizeof(T) == 4 ? -80 : -200), sizeof(T) == 4 ? 4.8e-38 : 1e-300);
-    c.four_a2 = (T)(4.0 * a * a);
-    c.c2 = (T)(2.0 * a * a / 3.0);
-    c.nc3 = (T)(-2.0 * a * a);
-    c.c4 = (T)c4;
-    c.nc5 = (T)(-c4 * 9.0 / (32.0 * a));
-    c.c6 = (T)(c4 * 3.0 / (32.0 * a));
-    c.c8 = (T)c8;
-    c.k1 = (T)(-c8 * 27.0 / (32.0 * a));
-    c.k2 = (T)(c8 * 5.0 / (64.0 * a * a * a));
-    c.k3 = (T)(c8 * 9.0 / (32.0 * a));
-    c.k4 = (T)(-c8 * 3.0 / (64.0 * a * a * a));
-    c.k5 = (T)(1.0 / (2.0 * a * a * a));
-    c.k6 = (T)(-3.0 / (16.0 * a * a * a * a));
-    c.C1 = (T)(1.0 / (8.0 * pi * eta));                // Oseen prefactor, applied once per target
-    return c;
-}
-
-template <typename T> std::vector<Variant<T>>& variants(lm_solver* h);
-template <> std::vector<Variant<float>>& variants<float>(lm_solver* h) { return h->vf; }
-template <> std::vector<Variant<double>>& variants<double>(lm_solver* h) { return h->vd; }
-
-template <typename T> int init_variants(lm_solver* h)
-{
-    auto& vs = variants<T>(h);
-    vs = build_variants<T>();
-    for (auto& v : vs) {
-        LM_CUDA(h, cudaFuncSetAttribute((const void*)v.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem));
-        int nb = 0;
-        LM_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)v.kernel, v.block, v.smem));
-        v.ctas_per_sm = std::max(nb, 1);
-    }
-    return LM_OK;
-}
-
-// Pick the variant and the number of j-splits.  Sources are dealt to the splits in units of SUB, as
-// evenly as possible, so the grid can be sized to a whole number of resident sets (148 SMs x
-// resident CTAs per SM) whatever N is.  Cost model: CTAs run in waves of `slots`; a CTA costs
-// (its sources + a fixed prologue/epilogue) x its targets; CTAs resident on one SM share it.
-template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
-{
-    if (nrhs >= 0 && nrhs <= MAX_RHS) {
-        const auto& slot = h->plan_cache[nrhs];
-        if (slot.valid && slot.rb == h->row_begin && slot.re == h->row_end) return slot.plan;
-    }
-    const auto& vs = variants<T>(h);
-    LaunchPlan best;
-    double best_cost = 1e300;
-    for (int vi = 0; vi < (int)vs.size(); ++vi) {
-        const auto& v = vs[vi];
-        if (v.nrhs != nrhs || v.ang != h->angular) continue;
-        const int targets = v.block * v.tpt;
-        const int64_t rows = std::max<int64_t>(h->row_end - h->row_begin, 0);          // target rows of this rank / call
-        const int i_tiles = (int)((rows + targets - 1) / targets);
-        const int units = (int)(h->npad / v.sub);
-        const int64_t slots = (int64_t)h->sm_count * v.ctas_per_sm;
-        const int max_splits = std::min(units, 256);
-        const int min_splits = (int)std::min<int64_t>(max_splits, (h->npad + MAX_SOURCES_PER_CTA - 1) / MAX_SOURCES_PER_CTA);
-        for (int s = min_splits; s <= max_splits; ++s) {
-            const int64_t src = (int64_t)((units + s - 1) / s) * v.sub;            // sources of the largest split
-            const int64_t ctas = (int64_t)i_tiles * s;
-            const int64_t full = ctas / slots, rem = ctas % slots;
-            const int64_t rem_per_sm = (rem + h->sm_count - 1) / h->sm_count;      // CTAs sharing an SM in the last wave
-            // prologue, pipeline fill and epilogue of a CTA ~ 0.1 tile (fitted to plan sweeps on B200)
-            const double per_cta = ((double)src + 0.1 * v.tj) * targets / v.efficiency;
-            // few resident warps hide less latency: w warps per SM sub-partition cost a factor (1 + 0.3 / w)
-            auto wave = [&](int64_t resident) { return resident ? per_cta * resident * (1.0 + 0.3 * 128.0 / ((double)resident * v.block)) : 0.0; };
-            double cost = (double)full * wave(v.ctas_per_sm) + wave(rem_per_sm);
-            // cost is in pairs evaluated back to back on one SM (~1e4 per microsecond): the reduce pass
-            // adds a ~3 us launch plus writing and re-reading s partial vectors
-            if (s > 1) cost += 3.0e4 + 0.1 * (double)s * (double)rows;
-            if (cost < best_cost) {
-                best_cost = cost;
-                best.variant = vi;
-                best.i_tiles = i_tiles;
-                best.j_splits = s;
-                best.n_units = units;
-            }
-        }
-    }
-    if (nrhs >= 0 && nrhs <= MAX_RHS) {
-        auto& slot = h->plan_cache[nrhs];
-        slot.valid = true;
-        slot.rb = h->row_begin;
-        slot.re = h->row_end;
-        slot.plan = best;
-    }
-    return best;
-}
-
-cudaEvent_t get_event(lm_solver* h)
-{
-    if (!h->event_pool.empty()) {
-        cudaEvent_t e = h->event_pool.back();
-        h->event_pool.pop_back();
-        return e;
-    }
-    cudaEvent_t e = nullptr;
-    cudaEventCreate(&e);
-    return e;
-}
-
-int grid_1d(int64_t n) { return (int)std::max<int64_t>(1, (n + VEC_BLOCK - 1) / VEC_BLOCK); }
-int grid_red(int64_t n) { return (int)std::min<int64_t>(RED_MAX_BLOCKS, std::max<int64_t>(1, (n + VEC_BLOCK - 1) / VEC_BLOCK)); }
-
-// ---------------------------------------------------------------- device apply: out = M . rhs  (nrhs <= MAX_RHS)
-// prepare_apply: choose the launch plan and size the packed right-hand side and the partials (no launches)
-template <typename T> int prepare_apply(lm_solver* h, int nrhs, LaunchPlan& plan)
-{
-    const int nc = h->angular ? 6 : 3;
-    plan = choose_plan<T>(h, nrhs);
-    if (plan.variant < 0) return fail(h, LM_E_INVALID, "no pair-kernel variant for this nrhs");
-    int rc = ensure(h, &h->vec_soa, &h->vec_soa_bytes, (size_t)nrhs * nc * h->npad * sizeof(T));
-    if (rc != LM_OK) return rc;
-    if (plan.j_splits > 1) {
-        rc = ensure(h, &h->partial, &h->partial_bytes, (size_t)plan.j_splits * nrhs * nc * h->npad * sizeof(T));
-        if (rc != LM_OK) return rc;
-    }
-    return LM_OK;
-}
-
-// launch_pair: the pair kernel on the packed right-hand side already in h->vec_soa, then the split-j reduce.
-// Only the target rows [h->row_begin, h->row_end) are computed.  With a communicator (lm_dist_init) those are
-// this rank's block: the kernel writes into all-gather buffers of 3 B ranks elements, ONE grouped
-// ncclAllGather (in place: rank r's segment starts at 3 B r) completes every output on every rank, and the
-// first 3N elements are copied to the caller's buffers.
-template <typename T> int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>& out, cudaStream_t st, bool timed)
-{
-    const int nc = h->angular ? 6 : 3;
-    const auto& v = variants<T>(h)[plan.variant];
-    const bool dist = h->dist_ranks > 0;
-    RhsOut<T> kout = out;
-    const size_t seg = (size_t)3 * h->rows_per_rank;                       // elements each rank contributes
-    if (dist) {
-        const size_t bytes = seg * h->dist_ranks * sizeof(T);
-        for (int q = 0; q < nrhs; ++q) {
-            for (int part = 0; part < (h->angular ? 2 : 1); ++part) {
-                const int rc = ensure(h, &h->gath[2 * q + part], &h->gath_bytes[2 * q + part], bytes);
-                if (rc != LM_OK) return rc;
-            }
-            kout.lin[q] = (T*)h->gath[2 * q];
-            kout.ang[q] = h->angular ? (T*)h->gath[2 * q + 1] : nullptr;
-        }
-    }
-    PairParams<T> p;
-    p.pos = (const T*)h->pos_soa;
-    p.vec = (const T*)h->vec_soa;
-    p.out = kout;
-    p.partial = (T*)h->partial;
-    p.N = h->N;
-    p.i_begin = h->row_begin;
-    p.i_end = h->row_end;
-    p.npad = h->npad;
-    p.n_units = plan.n_units;
-    p.c = make_consts<T>(h->eta, h->a);
-
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (timed) {
-        e0 = get_event(h);
-        e1 = get_event(h);
-        LM_CUDA(h, cudaEventRecord(e0, st));
-    }
-    if (plan.i_tiles > 0) v.kernel<<<dim3(plan.i_tiles, plan.j_splits), v.block, v.smem, st>>>(p);
-    if (timed) {
-        LM_CUDA(h, cudaEventRecord(e1, st));
-        h->pending.emplace_back(e0, e1);
-    }
-    if (plan.i_tiles > 0 && plan.j_splits > 1)
-        reduce_partials_kernel<T><<<dim3(grid_1d(h->row_end - h->row_begin), nrhs * nc), VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc,
-                                                                                                         h->row_begin, h->row_end, h->npad, kout);
-    LM_CUDA(h, cudaGetLastError());
-    if (dist) {
-        NcclApi& nccl = nccl_api();
-        const int dtype = sizeof(T) == 4 ? NCCL_FLOAT32 : NCCL_FLOAT64;
-        int nrc = nccl.GroupStart();
-        for (int q = 0; q < nrhs && nrc == 0; ++q)
-            for (int part = 0; part < (h->angular ? 2 : 1) && nrc == 0; ++part) {
-                T* buf = (T*)h->gath[2 * q + part];
-                nrc = nccl.AllGather(buf + seg * h->dist_rank, buf, seg, dtype, (NcclApi::Comm)h->nccl_comm, st);
-            }
-        const int nrc_end = nccl.GroupEnd();
-        if (nrc == 0) nrc = nrc_end;
-        if (nrc != 0) return fail(h, LM_E_CUDA, std::string("ncclAllGather failed: ") + nccl.GetErrorString(nrc));
-        const size_t out_bytes = (size_t)3 * h->N * sizeof(T);
-        for (int q = 0; q < nrhs; ++q) {
-            LM_CUDA(h, cudaMemcpyAsync(out.lin[q], h->gath[2 * q], out_bytes, cudaMemcpyDeviceToDevice, st));
-            if (h->angular) LM_CUDA(h, cudaMemcpyAsync(out.ang[q], h->gath[2 * q + 1], out_bytes, cudaMemcpyDeviceToDevice, st));
-        }
-    }
-    return LM_OK;
-}
-
-void count_apply(lm_solver* h, const LaunchPlan& plan)
-{
-    h->n_pair++;
-    h->pairs += (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N;
-    if (plan.j_splits > 1) h->n_aux++;
-}
-
-int ensure_capture_stream(lm_solver* h)
-{
-    if (!h->cap_stream) LM_CUDA(h, cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
-    return LM_OK;
-}
-
-template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& in, const RhsOut<T>& out, cudaStream_t st)
-{
-    const int nc = h->angular ? 6 : 3;
-    LaunchPlan plan;
-    int rc = prepare_apply<T>(h, nrhs, plan);
-    if (rc != LM_OK) return rc;
-    auto direct = [&](cudaStream_t s2, bool timed) -> int {
-        pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(in, nrhs, nc, h->N, h->npad, (T*)h->vec_soa);
-        return launch_pair<T>(h, nrhs, plan, out, s2, timed);
-    };
-    // A short apply is bound by the host's three launches (~11 us measured against ~3 us of kernels each): when
-    // the SAME call (same buffers, same plan) comes twice in a row -- a time-stepping loop -- it is captured
-    // once and replayed as a CUDA graph from then on; any other call is launched directly.
-    const double cost = (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N * (h->angular ? 2.3 : 1.0) *
-                        (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nrhs);
-    if (cost < 2.0e8 && !h->profiling && h->dist_ranks == 0 && std::getenv("LM_NO_GRAPH") == nullptr) {      // N <~ 14000 fp32
-        lm_solver::ApplyKey key;
-        std::memset(&key, 0, sizeof key);
-        for (int q = 0; q < nrhs; ++q) { key.f[q] = in.f[q]; key.t[q] = in.t[q]; key.lin[q] = out.lin[q]; key.ang[q] = out.ang[q]; }
-        key.pos = h->pos_soa; key.vec = h->vec_soa; key.partial = h->partial;
-        key.rb = h->row_begin; key.re = h->row_end;
-        key.nrhs = nrhs; key.variant = plan.variant; key.splits = plan.j_splits;
-        auto& slot = h->apply_graph[nrhs];
-        bool replay = slot.exec && std::memcmp(&key, &slot.graph_key, sizeof key) == 0;
-        if (!replay && slot.have_last && std::memcmp(&key, &slot.last, sizeof key) == 0) {
-            if ((rc = ensure_capture_stream(h)) != LM_OK) return rc;
-            if (slot.exec) { LM_CUDA(h, cudaGraphExecDestroy(slot.exec)); slot.exec = nullptr; }
-            cudaGraph_t graph = nullptr;
-            LM_CUDA(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
-            const int rc_body = direct(h->cap_stream, false);
-            const cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
-            if (rc_body != LM_OK) { if (graph) cudaGraphDestroy(graph); return rc_body; }
-            LM_CUDA(h, ce);
-            const cudaError_t ci = cudaGraphInstantiate(&slot.exec, graph, 0);
-            cudaGraphDestroy(graph);
-            LM_CUDA(h, ci);
-            slot.graph_key = key;
-            replay = true;
-        }
-        slot.last = key;
-        slot.have_last = true;
-        if (replay) {
-            LM_CUDA(h, cudaGraphLaunch(slot.exec, st));
-            h->n_aux++;
-            count_apply(h, plan);
-            return LM_OK;
-        }
-    }
-    if ((rc = direct(st, h->profiling)) != LM_OK) return rc;
-    h->n_aux++;
-    count_apply(h, plan);
-    return LM_OK;
-}
-
-// any nrhs: chunks of 4, 2, 1 right-hand sides per launch
-template <typename T>
-int apply_batch(lm_solver* h, int nrhs, const T* forces, const T* torques, T* lin_out, T* ang_out, cudaStream_t st)
-{
-    const int64_t n3 = 3 * h->N;
-    int q = 0;
-    while (q < nrhs) {
-        int chunk = nrhs - q >= 4 ? 4 : (nrhs - q >= 2 ? 2 : 1);
-        if (h->angular && chunk > 2) chunk = 2;     // angular variants exist for 1 and 2 right-hand sides
-        RhsIn<T> in{};
-        RhsOut<T> out{};
-        for (int r = 0; r < chunk; ++r) {
-            in.f[r] = forces ? forces + (q + r) * n3 : nullptr;
-            in.t[r] = torques ? torques + (q + r) * n3 : nullptr;
-            out.lin[r] = lin_out + (q + r) * n3;
-            out.ang[r] = ang_out ? ang_out + (q + r) * n3 : nullptr;
-        }
-        const int rc = apply_device<T>(h, chunk, in, out, st);
-        if (rc != LM_OK) return rc;
-        q += chunk;
-    }
-    return LM_OK;
-}
-
-// ---------------------------------------------------------------- Lanczos driver (a7-a10)
-// nv <= MAX_RHS (angular: 2) independent Lanczos recurrences advanced in lockstep: one multi-right-hand-side
-// pair-kernel launch per iteration serves all of them, every other kernel runs
-// once per vector.  nv = 1 is lm_sqrt_mdot_w.  noise / outputs: [nv][dof] / [nv][3N].  iters_out: nv ints.
-template <typename T>
-int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out, T* ang_out, double scale, int accumulate, int* iters_out,
-                   cudaStream_t st)
-{
-    const int64_t dof = dof_of(h), n3 = 3 * h->N;
-    const int nc = h->angular ? 6 : 3;
-    const int kmax = h->max_iter;
-    const int ld = kmax + 2;
-    int rc;
-    if ((rc = ensure(h, &h->V, &h->V_bytes, (size_t)nv * (kmax + 1) * dof * sizeof(T))) != LM_OK) return rc;
-    if ((rc = ensure(h, &h->w, &h->w_bytes, (size_t)nv * dof * sizeof(T))) != LM_OK) return rc;
-    if (!h->d_scal) {
-        LM_CUDA(h, cudaMalloc((void**)&h->d_scal, MAX_RHS * 4 * sizeof(double)));
-        LM_CUDA(h, cudaMalloc((void**)&h->d_block, RED_MAX_BLOCKS * sizeof(double)));
-        LM_CUDA(h, cudaMalloc((void**)&h->d_ticket, sizeof(unsigned int)));
-        LM_CUDA(h, cudaMalloc((void**)&h->d_newest, sizeof(int)));
-        LM_CUDA(h, cudaMemsetAsync(h->d_ticket, 0, sizeof(unsigned int), st));
-        for (auto& e : h->lz_ev) LM_CUDA(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-    }
-    if ((rc = ensure_capture_stream(h)) != LM_OK) return rc;
-    if (h->coef_cap < (size_t)(kmax + 2)) {
-        if (h->d_coef) { LM_CUDA(h, cudaFree(h->d_coef)); LM_CUDA(h, cudaFree(h->d_gram_part)); LM_CUDA(h, cudaFreeHost(h->h_gram)); LM_CUDA(h, cudaFreeHost(h->h_ab)); }
-        h->d_coef = nullptr;
-        h->coef_cap = 0;
-        LM_CUDA(h, cudaMalloc((void**)&h->d_coef, (size_t)MAX_RHS * (kmax + 2) * sizeof(double)));
-        LM_CUDA(h, cudaMalloc((void**)&h->d_gram_part, (size_t)(kmax + 2) * GRAM_MAX_BLOCKS * sizeof(double)));
-        LM_CUDA(h, cudaHostAlloc((void**)&h->h_gram, (size_t)MAX_RHS * ld * ld * sizeof(double), cudaHostAllocMapped));
-        LM_CUDA(h, cudaHostAlloc((void**)&h->h_ab, (size_t)MAX_RHS * 2 * ld * sizeof(double), cudaHostAllocMapped));
-        h->coef_cap = (size_t)(kmax + 2);
-    }
-    // per-vector views
-    auto Vq = [&](int q) { return (T*)h->V + (size_t)q * (kmax + 1) * dof; };
-    auto wq = [&](int q) { return (T*)h->w + (size_t)q * dof; };
-    auto scal = [&](int q) { return h->d_scal + 4 * q; };                       // [0] |z|^2  [1] alpha  [2] beta^2
-    auto ab = [&](int q) { return (volatile const double*)(h->h_ab + (size_t)q * 2 * ld); };
-    auto hg = [&](int q) { return (volatile const double*)(h->h_gram + (size_t)q * ld * ld); };
-    const int gr = grid_red(dof);
-    const int gg = (int)std::min<int64_t>(GRAM_MAX_BLOCKS, std::max<int64_t>(1, dof / (4 * VEC_BLOCK)));
-    const int64_t gchunk = (dof + gg - 1) / gg;
-    LaunchPlan plan;
-    if ((rc = prepare_apply<T>(h, nv, plan)) != LM_OK) return rc;
-    auto soa = [&](int q) { return (T*)h->vec_soa + (size_t)q * nc * h->npad; };
-    // Gram matrices of the bases, G[q][i][j] = V_q[i].V_q[j], filled one column per new basis vector
-    const int ldg = kmax + 1;
-    std::vector<std::vector<double>> G(nv, std::vector<double>((size_t)ldg * ldg, 0.0));
-    auto gram_store = [&](int q, int m) {
-        for (int j = 0; j <= m; ++j) G[q][(size_t)j * ldg + m] = G[q][(size_t)m * ldg + j] = hg(q)[(size_t)m * ld + j];
-    };
-    // new basis vectors V_q[*newest + 1] = x_q / sqrt(sumsq_q) (+ packed copies for the next apply), their Gram
-    // columns, then *newest += 1 (once: the recurrences move in lockstep)
-    auto new_vectors = [&](const T* x, int which_scal, cudaStream_t s2) {
-        for (int q = 0; q < nv; ++q) {
-            lanczos_scale_pack_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(x + (size_t)q * dof, h->N, h->npad, nc, scal(q) + which_scal, h->d_newest,
-                                                                              Vq(q), soa(q));
-            gram_column_kernel<T><<<dim3(gg, kmax + 1), VEC_BLOCK, 0, s2>>>(Vq(q), dof, h->d_newest, gchunk, h->d_gram_part, h->d_ticket,
-                                                                             h->h_gram + (size_t)q * ld * ld, ld);
-        }
-        lanczos_advance_kernel<<<1, 1, 0, s2>>>(h->d_newest);
-    };
-
-    // v_1 = z / |z|
-    LM_CUDA(h, cudaMemsetAsync(h->d_newest, 0xff, sizeof(int), st));            // *newest = -1
-    for (int q = 0; q < nv; ++q)
-        sumsq_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise + (size_t)q * dof, dof, h->d_block, h->d_ticket, scal(q), h->h_ab + (size_t)q * 2 * ld + 1);
-    new_vectors(noise, 0, st);
-    h->n_aux += 3 * nv + 1;
-    LM_CUDA(h, cudaGetLastError());
-    LM_CUDA(h, cudaStreamSynchronize(st));
-    std::vector<double> znorm(nv);
-    std::vector<char> done(nv, 0), conv(nv, 0);
-    std::vector<int> kfin(nv, 0);
-    std::vector<std::vector<double>> alphas(nv), betas(nv), c_prev(nv), c_cur(nv), c_fin(nv);
-    int remaining = nv;
-    for (int q = 0; q < nv; ++q) {
-        gram_store(q, 0);
-        znorm[q] = std::sqrt(ab(q)[1]);
-        if (!(znorm[q] > 0.0)) { done[q] = conv[q] = 1; --remaining; }            // zero noise: M^{1/2} 0 = 0
-    }
-    h->last_iters = 0;
-
-    // Iteration k on the device, with m = k - 1 = *newest, for every vector:  w = M v_k;  w -= beta_{k-1} v_{k-1};
-    // alpha_k;  w -= alpha_k v_k;  beta_k^2;  v_{k+1} = w / beta_k (+ packed for the next apply);  Gram column k.
-    // Everything the device needs stays on the device; the host only READS (alpha_k, beta_k^2, Gram column)
-    // from mapped pinned memory for the stopping test.  The launch sequence and its arguments are the
-    // same for every k, so it is captured once as a CUDA graph.
-    RhsOut<T> out{};
-    for (int q = 0; q < nv; ++q) {
-        out.lin[q] = wq(q);
-        out.ang[q] = h->angular ? wq(q) + n3 : nullptr;
-    }
-    auto body = [&](cudaStream_t s2, bool timed) -> int {
-        int rc2;
-        if ((rc2 = launch_pair<T>(h, nv, plan, out, s2, timed)) != LM_OK) return rc2;                      // w_q = M v_k,q
-        for (int q = 0; q < nv; ++q) {
-            lanczos_alpha_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q) + 2, dof, h->d_block, h->d_ticket, scal(q) + 1);
-            lanczos_beta_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q) + 1, dof, h->d_block, h->d_ticket, scal(q) + 2,
-                                                             h->h_ab + (size_t)q * 2 * ld);
-        }
-        new_vectors((const T*)h->w, 2, s2);
-        LM_CUDA(h, cudaGetLastError());
-        return LM_OK;
-    };
-    // One iteration of look-ahead when an apply is short: iteration k+1 is enqueued BEFORE the host waits
-    // for iteration k's scalars, so the device never idles on the host round trip.  The price is one
-    // wasted apply at convergence, so it is used only where an apply costs less than the round trips it
-    // saves (~25 iterations x 50 us); the same regime is launch-bound, so there the body runs as a graph.
-    const double apply_cost = (double)h->N * (double)h->N * (h->angular ? 2.3 : 1.0) * (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nv);
-    const bool lookahead = apply_cost < 2.0e9;
-    const bool use_graph = lookahead && !h->profiling && h->dist_ranks == 0 && std::getenv("LM_NO_GRAPH") == nullptr;
-    if (use_graph && remaining > 0) {
-        const lm_solver::GraphKey key = {h->V, h->w, h->vec_soa, h->partial, h->pos_soa, kmax, plan.variant, plan.j_splits, h->precision * 8 + nv};
-        if (!h->lz_graph || std::memcmp(&key, &h->lz_key, sizeof key) != 0) {
-            if (h->lz_graph) { LM_CUDA(h, cudaGraphExecDestroy(h->lz_graph)); h->lz_graph = nullptr; }
-            cudaGraph_t graph = nullptr;
-            LM_CUDA(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
-            const int rc_body = body(h->cap_stream, false);
-            const cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
-            if (rc_body != LM_OK) { if (graph) cudaGraphDestroy(graph); return rc_body; }
-            LM_CUDA(h, ce);
-            const cudaError_t ci = cudaGraphInstantiate(&h->lz_graph, graph, 0);
-            cudaGraphDestroy(graph);
-            LM_CUDA(h, ci);
-            h->lz_key = key;
-        }
-    }
-    auto enqueue = [&](int k) -> int {
-        if (use_graph) {
-            LM_CUDA(h, cudaGraphLaunch(h->lz_graph, st));
-        } else {
-            const int rc2 = body(st, h->profiling);
-            if (rc2 != LM_OK) return rc2;
-        }
-        count_apply(h, plan);
-        h->n_aux += 4 * nv + 1;
-        LM_CUDA(h, cudaEventRecord(h->lz_ev[k & 1], st));
-        return LM_OK;
-    };
-
-    const bool debug = std::getenv("LM_DEBUG_LANCZOS") != nullptr;   // per-iteration trace on stderr
-    const double breakdown = (h->precision == LM_F32) ? 1e-6 : 1e-14;
-    int k = 0;
-    if (remaining > 0 && (rc = enqueue(1)) != LM_OK) return rc;
-    for (k = 1; k <= kmax && remaining > 0; ++k) {
-        if (lookahead && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
-        LM_CUDA(h, cudaEventSynchronize(h->lz_ev[k & 1]));
-        for (int q = 0; q < nv; ++q) {
-            if (done[q]) continue;
-            const double alpha = ab(q)[2 * k], beta = std::sqrt(std::max((double)ab(q)[2 * k + 1], 0.0));
-            if (!std::isfinite(alpha) || !std::isfinite(beta)) {
-                cudaStreamSynchronize(st);
-                return fail(h, LM_E_CUDA, "Lanczos: non-finite alpha/beta (non-finite input?)");
-            }
-            alphas[q].push_back(alpha);
-            c_cur[q].assign(k, 0.0);
-            if (!tridiag_sqrt_e1(k, alphas[q].data(), betas[q].data(), c_cur[q].data())) {
-                cudaStreamSynchronize(st);
-                return fail(h, LM_E_NOCONV, "Lanczos: tridiagonal eigensolve did not converge");
-            }
-            bool converged = false;
-            if (k >= 2) {
-                // |y_k - y_{k-1}|^2 / |z|^2 = delta^T G_k delta,  |y_{k-1}|^2 / |z|^2 = c_{k-1}^T G_{k-1} c_{k-1}
-                std::vector<double> delta(c_cur[q]);
-                for (int i = 0; i < k - 1; ++i) delta[i] -= c_prev[q][i];
-                double num = 0.0, den = 0.0;
-                for (int i = 0; i < k; ++i)
-                    for (int j = 0; j < k; ++j) num += delta[i] * G[q][(size_t)i * ldg + j] * delta[j];
-                for (int i = 0; i < k - 1; ++i)
-                    for (int j = 0; j < k - 1; ++j) den += c_prev[q][i] * G[q][(size_t)i * ldg + j] * c_prev[q][j];
-                if (std::sqrt(std::max(num, 0.0)) <= tol * std::sqrt(std::max(den, 0.0))) converged = true;
-                if (debug)
-                    std::fprintf(stderr, "[lm lanczos] vec=%d k=%d alpha=%.9e beta=%.9e step=%.3e\n", q, k, alpha, beta, std::sqrt(std::max(num, 0.0) / den));
-            }
-            if (beta <= breakdown * std::fabs(alpha)) converged = true;   // invariant subspace: iterate is exact
-            if (converged || k == kmax) {
-                done[q] = 1;
-                conv[q] = converged;
-                kfin[q] = k;
-                c_fin[q] = c_cur[q];
-                --remaining;
-                continue;
-            }
-            gram_store(q, k);
-            betas[q].push_back(beta);
-            c_prev[q] = c_cur[q];
-        }
-        if (!lookahead && remaining > 0 && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
-    }
-    // results: y_q = scale |z_q| V_q c_q  (a10)
-    bool all_converged = true;
-    std::vector<double> coef((size_t)nv * (kmax + 2), 0.0);
-    for (int q = 0; q < nv; ++q) {
-        all_converged = all_converged && conv[q];
-        for (int i = 0; i < kfin[q]; ++i) coef[(size_t)q * (kmax + 2) + i] = c_fin[q][i];
-        if (iters_out) iters_out[q] = kfin[q];
-        h->last_iters = std::max(h->last_iters, kfin[q]);
-    }
-    LM_CUDA(h, cudaMemcpyAsync(h->d_coef, coef.data(), coef.size() * sizeof(double), cudaMemcpyHostToDevice, st));
-    for (int q = 0; q < nv; ++q) {
-        T* lo = lin_out + (size_t)q * n3;
-        T* ao = h->angular ? ang_out + (size_t)q * n3 : nullptr;
-        if (kfin[q] == 0) {               // zero noise vector
-            if (!accumulate) {
-                LM_CUDA(h, cudaMemsetAsync(lo, 0, (size_t)n3 * sizeof(T), st));
-                if (h->angular) LM_CUDA(h, cudaMemsetAsync(ao, 0, (size_t)n3 * sizeof(T), st));
-            }
-            continue;
-        }
-        lanczos_combine_kernel<T><<<grid_1d(dof), VEC_BLOCK, 0, st>>>(Vq(q), dof, kfin[q], h->d_coef + (size_t)q * (kmax + 2), scale * znorm[q], accumulate,
-                                                                       n3, lo, ao);
-        h->n_aux++;
-    }
-    LM_CUDA(h, cudaGetLastError());
-    LM_CUDA(h, cudaStreamSynchronize(st));      // coef (pageable) must outlive the copy; drains a look-ahead iteration
-    if (!all_converged) return fail(h, LM_E_NOCONV, "Lanczos: max_iter reached before the tolerance was met (last iterate written)");
-    return LM_OK;
-}
-
-// ---------------------------------------------------------------- steric forces and the BD step
-template <typename T> int set_positions_t(lm_solver* h, const void* pos, cudaStream_t st);
-
-template <typename T>
-int steric_device(lm_solver* h, double U0, double b, const T* ext, T* out, cudaStream_t st)
-{
-    if (!h->steric_attr_set) {
-        LM_CUDA(h, cudaFuncSetAttribute((const void*)steric_pair_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, steric_smem_bytes<T>()));
-        h->steric_attr_set = true;
-    }
-    const int units = (int)(h->npad / STERIC_SUB);
-    const int64_t rows = std::max<int64_t>(h->row_end - h->row_begin, 0);      // this rank's target rows (all rows unless sharded)
-    const int i_tiles = (int)((rows + STERIC_TARGETS - 1) / STERIC_TARGETS);
-    // about four resident sets of CTAs (2 per SM): the work per CTA depends on how many groups are within the cut-off
-    const int splits = (int)std::max<int64_t>(1, std::min<int64_t>(units, ((int64_t)8 * h->sm_count + std::max(i_tiles, 1) - 1) / std::max(i_tiles, 1)));
-    int rc = ensure(h, &h->partial, &h->partial_bytes, (size_t)splits * 3 * h->npad * sizeof(T));
-    if (rc != LM_OK) return rc;
-    const bool dist = h->dist_ranks > 0;
-    const size_t seg = (size_t)3 * h->rows_per_rank;
-    T* kout = out;
-    if (dist) {
-        if ((rc = ensure(h, &h->gath[0], &h->gath_bytes[0], seg * h->dist_ranks * sizeof(T))) != LM_OK) return rc;
-        kout = (T*)h->gath[0];
-    }
-    const double K = sizeof(T) == 4 ? 20.0 : 40.0;           // exp(-K) below the type's epsilon
-    StericParams<T> p;
-    p.pos = (const T*)h->pos_soa;
-    p.partial = (T*)h->partial;
-    p.N = h->N;
-    p.npad = h->npad;
-    p.i_begin = h->row_begin;
-    p.n_units = units;
-    p.tiny = make_consts<T>(h->eta, h->a).tiny;
-    p.d = (T)(2.0 * h->a);
-    p.rc2 = (T)((2.0 * h->a + K * b) * (2.0 * h->a + K * b));
-    p.m0 = (T)(U0 / b);
-    p.inv_b = (T)(sizeof(T) == 4 ? 1.4426950408889634 / b : 1.0 / b);
-    if (i_tiles > 0) {
-        steric_pair_kernel<T><<<dim3(i_tiles, splits), STERIC_BLOCK, steric_smem_bytes<T>(), st>>>(p);
-        steric_reduce_kernel<T><<<grid_1d(rows), VEC_BLOCK, 0, st>>>((const T*)h->partial, splits, h->row_begin, h->row_end, h->npad, ext, kout);
-        h->n_aux += 2;
-    }
-    LM_CUDA(h, cudaGetLastError());
-    if (dist) {                                              // row blocks -> every rank (as in launch_pair)
-        NcclApi& nccl = nccl_api();
-        const int nrc = nccl.AllGather(kout + seg * h->dist_rank, kout, seg, sizeof(T) == 4 ? NCCL_FLOAT32 : NCCL_FLOAT64, (NcclApi::Comm)h->nccl_comm, st);
-        if (nrc != 0) return fail(h, LM_E_CUDA, std::string("ncclAllGather failed: ") + nccl.GetErrorString(nrc));
-        LM_CUDA(h, cudaMemcpyAsync(out, kout, (size_t)3 * h->N * sizeof(T), cudaMemcpyDeviceToDevice, st));
-    }
-    return LM_OK;
-}
-
-// eq. (11): (1/delta) [ M(X + delta W/2) W - M(X - delta W/2) W ], one realisation
-template <typename T>
-int rfd_device(lm_solver* h, const T* W, double delta, T* lin_out, T* ang_out, cudaStream_t st)
-{
-    const int64_t n3 = 3 * h->N;
-    int rc;
-    if ((rc = ensure(h, &h->rfd[0], &h->rfd_bytes[0], (size_t)3 * h->npad * sizeof(T))) != LM_OK) return rc;
-    if ((rc = ensure(h, &h->rfd[1], &h->rfd_bytes[1], (size_t)n3 * sizeof(T))) != LM_OK) return rc;
-    if (h->angular && (rc = ensure(h, &h->rfd[2], &h->rfd_bytes[2], (size_t)n3 * sizeof(T))) != LM_OK) return rc;
-    void* const home = h->pos_soa;
-    T* outs[2][2] = {{lin_out, ang_out}, {(T*)h->rfd[1], (T*)h->rfd[2]}};
-    for (int side = 0; side < 2; ++side) {
-        shift_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)home, W, h->N, h->npad, (T)((side ? -0.5 : 0.5) * delta), (T*)h->rfd[0]);
-        h->n_aux++;
-        h->pos_soa = h->rfd[0];                       // the apply reads the displaced copy; the handle's positions are untouched
-        rc = apply_batch<T>(h, 1, W, nullptr, outs[side][0], h->angular ? outs[side][1] : nullptr, st);
-        h->pos_soa = home;
-        if (rc != LM_OK) return rc;
-    }
-    rfd_difference_kernel<T><<<grid_1d(n3), VEC_BLOCK, 0, st>>>(lin_out, (const T*)h->rfd[1], n3, (T)(1.0 / delta));
-    if (h->angular) rfd_difference_kernel<T><<<grid_1d(n3), VEC_BLOCK, 0, st>>>(ang_out, (const T*)h->rfd[2], n3, (T)(1.0 / delta));
-    h->n_aux += h->angular ? 2 : 1;
-    LM_CUDA(h, cudaGetLastError());
-    return LM_OK;
-}
-
-template <typename T>
-int bd_step_device(lm_solver* h, T* pos, const T* ext_f, const T* ext_t, const T* noise, double dt, double kT, double U0, double b, double tol,
-                   cudaStream_t st)
-{
-    const int64_t n3 = 3 * h->N;
-    const size_t bytes = (size_t)n3 * sizeof(T);
-    int rc;
-    for (int k = 0; k < 6; ++k)
-        if ((rc = ensure(h, &h->bd[k], &h->bd_bytes[k], bytes)) != LM_OK) return rc;
-    T *F = (T*)h->bd[0], *vn = (T*)h->bd[1], *vprev = (T*)h->bd[2], *y = (T*)h->bd[3], *ang = (T*)h->bd[4], *yang = (T*)h->bd[5];
-    if ((rc = set_positions_t<T>(h, pos, st)) != LM_OK) return rc;
-    // F^n = steric(X^n) + external;  v_n = M^n [F^n; T]
-    const bool have_force = U0 != 0.0 || ext_f;
-    if (U0 != 0.0) {
-        if ((rc = steric_device<T>(h, U0, b, ext_f, F, st)) != LM_OK) return rc;
-    }
-    const T* Fin = U0 != 0.0 ? F : ext_f;
-    if (have_force || ext_t) {
-        if ((rc = apply_batch<T>(h, 1, Fin, ext_t, vn, h->angular ? ang : nullptr, st)) != LM_OK) return rc;
-    } else {
-        LM_CUDA(h, cudaMemsetAsync(vn, 0, bytes, st));
-    }
-    int rc_noise = LM_OK;
-    const bool noisy = noise && kT > 0.0;
-    if (noisy) {
-        rc_noise = lanczos_device<T>(h, 1, noise, tol, y, h->angular ? yang : nullptr, 1.0, 0, nullptr, st);
-        if (rc_noise != LM_OK && rc_noise != LM_E_NOCONV) return rc_noise;
-    }
-    const double cn = h->bd_have_prev ? 1.5 : 1.0, cp = h->bd_have_prev ? 0.5 : 0.0;
-    bd_update_kernel<T><<<grid_1d(n3), VEC_BLOCK, 0, st>>>(pos, vn, vprev, noisy ? y : nullptr, n3, (T)(dt * cn), (T)(dt * cp),
-                                                           (T)std::sqrt(2.0 * kT * dt));
-    h->n_aux++;
-    LM_CUDA(h, cudaGetLastError());
-    h->bd_have_prev = true;
-    h->have_pos = false;       // the packed copy now holds X^n, not the caller's X^{n+1}
-    return rc_noise;
-}
 
 // ---------------------------------------------------------------- typed front ends
 template <typename T> int set_positions_t(lm_solver* h, const void* pos, cudaStream_t st)

@@ -1,0 +1,329 @@
+// lm_handle.cuh -- the solver handle of liblm: pair-kernel variants, NCCL loader, state, error helpers and the launch chooser.
+// Included by lm_api.cu only (one translation unit); everything after the handle lives in an anonymous namespace.
+#pragma once
+
+namespace lm {
+
+// ---------------------------------------------------------------- pair-kernel variants
+// LARGE: 256 threads x TPT targets (TPT/2 packed pairs per thread), tiles of up to 512 sources.
+// SMALL: 64 x 2, tiles of up to 64 sources (fills 148 SMs when N is small, SURVEY.md sec. 7 "Small N").
+// SUB = sources per overlap-vote chunk = the unit in which sources are dealt to the j-splits;
+// npad is a multiple of NPAD_QUANTUM, which every SUB divides.
+constexpr int NPAD_QUANTUM = 32;
+constexpr int L_BLOCK = 256, L_TJ = 512, L_STAGES = 2;
+constexpr int S_BLOCK = 64, S_TPT = 2, S_TJ = 64, S_STAGES = 2;
+constexpr int64_t MAX_SOURCES_PER_CTA = 262144;   // bounds the top level of the two-level fp32 summation
+
+template <typename T> struct Variant {
+    void (*kernel)(const PairParams<T>);
+    int nrhs, ang, block, tpt, tj, sub, smem;
+    int ctas_per_sm;      // filled at first use (occupancy API)
+    double efficiency;    // relative per-pair throughput used by the launch chooser
+};
+
+template <typename T, int NRHS, bool ANG, int TPT, int SUB, int MINB> Variant<T> make_large()
+{
+    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB>;
+    static_assert(NPAD_QUANTUM % SUB == 0, "every SUB divides NPAD_QUANTUM");
+    return {rpy_pair_kernel<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB, MINB>, NRHS, ANG, L_BLOCK, TPT, L_TJ, SUB, Tr::SMEM_BYTES, 0, 1.0};
+}
+template <typename T, int NRHS, bool ANG, int SUB, int MINB> Variant<T> make_small()
+{
+    using Tr = PairKernelTraits<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB>;
+    static_assert(NPAD_QUANTUM % SUB == 0, "every SUB divides NPAD_QUANTUM");
+    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB, MINB>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, SUB, Tr::SMEM_BYTES, 0, 0.8};
+}
+
+template <typename T> std::vector<Variant<T>> build_variants();
+template <> std::vector<Variant<float>> build_variants<float>()
+{
+    return {make_large<float, 1, false, 4, 32, 2>(), make_large<float, 2, false, 4, 32, 1>(), make_large<float, 4, false, 4, 32, 1>(),
+            make_large<float, 1, true, 2, 32, 2>(),  make_large<float, 2, true, 2, 32, 1>(),
+            make_small<float, 1, false, 32, 8>(), make_small<float, 2, false, 32, 8>(), make_small<float, 4, false, 32, 6>(),
+            make_small<float, 1, true, 32, 8>(),  make_small<float, 2, true, 32, 6>()};
+}
+template <> std::vector<Variant<double>> build_variants<double>()
+{
+    return {make_large<double, 1, false, 4, 32, 1>(), make_large<double, 2, false, 2, 32, 1>(), make_large<double, 4, false, 2, 32, 1>(),
+            make_large<double, 1, true, 2, 32, 1>(),  make_large<double, 2, true, 2, 32, 1>(),
+            make_small<double, 1, false, 32, 8>(), make_small<double, 2, false, 32, 6>(), make_small<double, 4, false, 32, 4>(),
+            make_small<double, 1, true, 32, 6>(),  make_small<double, 2, true, 32, 4>()};
+}
+
+struct LaunchPlan {
+    int variant = -1;
+    int i_tiles = 0, j_splits = 0, n_units = 0;
+};
+
+}  // namespace lm
+
+// ---------------------------------------------------------------- NCCL, loaded at run time (row-sharded applies only)
+// The library does not link NCCL: a single-GPU user never needs it.  lm_dist_* resolve the few entry
+// points below from the libnccl already in the process (PyTorch's) or, failing that, the system one.
+namespace lm {
+struct NcclApi {
+    struct UniqueId { char internal[128]; };
+    typedef void* Comm;
+    int (*GetUniqueId)(UniqueId*) = nullptr;
+    int (*CommInitRank)(Comm*, int, UniqueId, int) = nullptr;
+    int (*CommDestroy)(Comm) = nullptr;
+    int (*AllGather)(const void*, void*, size_t, int, Comm, cudaStream_t) = nullptr;
+    int (*GroupStart)() = nullptr;
+    int (*GroupEnd)() = nullptr;
+    const char* (*GetErrorString)(int) = nullptr;
+    bool ok = false;
+    std::string why;
+};
+constexpr int NCCL_FLOAT32 = 7, NCCL_FLOAT64 = 8;   // ncclDataType_t values (nccl.h)
+
+inline NcclApi& nccl_api()
+{
+    static NcclApi api;
+    static bool tried = false;
+    if (tried) return api;
+    tried = true;
+    void* lib = dlopen("libnccl.so.2", RTLD_NOW | RTLD_NOLOAD);
+    if (!lib) lib = dlopen("libnccl.so.2", RTLD_NOW | RTLD_GLOBAL);
+    if (!lib) { api.why = std::string("cannot load libnccl.so.2: ") + dlerror(); return api; }
+    auto sym = [&](const char* name) { void* p = dlsym(lib, name); if (!p) api.why = std::string("libnccl.so.2 lacks ") + name; return p; };
+    api.GetUniqueId = (int (*)(NcclApi::UniqueId*))sym("ncclGetUniqueId");
+    api.CommInitRank = (int (*)(NcclApi::Comm*, int, NcclApi::UniqueId, int))sym("ncclCommInitRank");
+    api.CommDestroy = (int (*)(NcclApi::Comm))sym("ncclCommDestroy");
+    api.AllGather = (int (*)(const void*, void*, size_t, int, NcclApi::Comm, cudaStream_t))sym("ncclAllGather");
+    api.GroupStart = (int (*)())sym("ncclGroupStart");
+    api.GroupEnd = (int (*)())sym("ncclGroupEnd");
+    api.GetErrorString = (const char* (*)(int))sym("ncclGetErrorString");
+    api.ok = api.GetUniqueId && api.CommInitRank && api.CommDestroy && api.AllGather && api.GroupStart && api.GroupEnd && api.GetErrorString;
+    return api;
+}
+}  // namespace lm
+
+using namespace lm;
+
+// ---------------------------------------------------------------- handle
+struct lm_solver {
+    int precision = LM_F32;
+    int64_t N = 0, npad = 0;
+    double eta = 1.0, a = 1.0;
+    int angular = 0;
+    int max_iter = 100;
+    int device = 0, sm_count = 0;
+    bool have_pos = false;
+    std::string err;
+    int last_iters = -1;
+
+    void* pos_soa = nullptr;
+    void* vec_soa = nullptr;   size_t vec_soa_bytes = 0;
+    void* partial = nullptr;   size_t partial_bytes = 0;
+
+    // Lanczos workspace
+    void* V = nullptr;         size_t V_bytes = 0;
+    void* w = nullptr;         size_t w_bytes = 0;
+    double* d_scal = nullptr;  // [0] |z|^2  [1] alpha  [2] beta^2
+    double* d_block = nullptr; // block partials of the reductions
+    unsigned int* d_ticket = nullptr;
+    int* d_newest = nullptr;   // index of the newest basis vector (read by the iteration's kernels)
+    double* d_coef = nullptr;  size_t coef_cap = 0;   // coef_cap also sizes the buffers below
+    double* d_gram_part = nullptr;
+    // mapped pinned host memory the kernels write the stopping-test scalars into
+    double* h_ab = nullptr;    // [1] |z|^2; [2k], [2k+1]: alpha_k, beta_k^2
+    double* h_gram = nullptr;  // column c at [c * (max_iter + 2) + j] = V[j].V[c], j <= c
+    cudaEvent_t lz_ev[2] = {nullptr, nullptr};   // iteration k's scalars have landed (parity k & 1)
+    // one Lanczos iteration captured as a CUDA graph (small N: the loop is launch-bound)
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t lz_graph = nullptr;
+    struct GraphKey { const void *V, *w, *vec, *partial, *pos; int kmax, variant, splits, prec; } lz_key = {nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0};
+
+    // Brownian-dynamics step (lm_bd_step): F, v_n, v_{n-1}, noise velocity, angular scratch x2, position staging
+    void* bd[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    size_t bd_bytes[7] = {0, 0, 0, 0, 0, 0, 0};
+    bool bd_have_prev = false;
+    bool steric_attr_set = false;
+    // random finite difference (lm_thermal_drift_rfd): displaced packed positions, U(X-) linear / angular
+    void* rfd[3] = {nullptr, nullptr, nullptr};
+    size_t rfd_bytes[3] = {0, 0, 0};
+
+    // row-sharded applies over NCCL (lm_dist_init): rank r computes target rows [r B, min((r+1) B, N)), B = rows_per_rank
+    int dist_ranks = 0, dist_rank = 0;        // dist_ranks == 0: not distributed
+    int64_t rows_per_rank = 0;
+    void* nccl_comm = nullptr;
+    void* gath[2 * MAX_RHS] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // all-gather buffers, 3 B ranks each
+    size_t gath_bytes[2 * MAX_RHS] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int64_t row_begin = 0, row_end = 0;       // the target rows every apply computes ([0, N) unless sharded / lm_mdot_rows)
+
+    // staging for the _host entry points
+    void* st[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // pos, f, t, noise, lin, ang
+    size_t st_bytes[6] = {0, 0, 0, 0, 0, 0};
+
+    // variants (typed; only the handle's precision is populated)
+    std::vector<Variant<float>> vf;
+    std::vector<Variant<double>> vd;
+
+    // launch plans are pure functions of (nrhs, row range): cached, the chooser's search is off the per-call path
+    struct PlanSlot { bool valid = false; int64_t rb = 0, re = 0; lm::LaunchPlan plan; } plan_cache[lm::MAX_RHS + 1];
+
+    // small-N applies (pack + pair kernel + reduce) replayed as a CUDA graph when called again with the same buffers
+    struct ApplyKey {
+        const void *f[lm::MAX_RHS], *t[lm::MAX_RHS], *lin[lm::MAX_RHS], *ang[lm::MAX_RHS];
+        const void *pos, *vec, *partial;
+        int64_t rb, re;
+        int nrhs, variant, splits, pad;
+    };
+    struct ApplySlot { bool have_last = false; ApplyKey last, graph_key; cudaGraphExec_t exec = nullptr; } apply_graph[lm::MAX_RHS + 1];
+
+    // stats
+    int64_t n_pair = 0, n_aux = 0;
+    double pairs = 0.0, pair_ms = 0.0;
+    bool profiling = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> pending;
+    std::vector<cudaEvent_t> event_pool;
+};
+
+namespace {
+
+int fail(lm_solver* h, int code, const std::string& msg)
+{
+    if (h) h->err = msg;
+    return code;
+}
+
+#define LM_CUDA(h, expr)                                                                              \
+    do {                                                                                              \
+        cudaError_t e__ = (expr);                                                                     \
+        if (e__ != cudaSuccess) {                                                                     \
+            char buf__[512];                                                                          \
+            std::snprintf(buf__, sizeof buf__, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+            return fail(h, LM_E_CUDA, buf__);                                                         \
+        }                                                                                             \
+    } while (0)
+
+size_t esize(const lm_solver* h) { return h->precision == LM_F32 ? 4 : 8; }
+int64_t dof_of(const lm_solver* h) { return (h->angular ? 6 : 3) * h->N; }
+
+int ensure(lm_solver* h, void** ptr, size_t* cap, size_t bytes)
+{
+    if (*cap >= bytes && *ptr) return LM_OK;
+    if (*ptr) LM_CUDA(h, cudaFree(*ptr));
+    *ptr = nullptr;
+    *cap = 0;
+    LM_CUDA(h, cudaMalloc(ptr, bytes));
+    *cap = bytes;
+    return LM_OK;
+}
+
+template <typename T> PairConsts<T> make_consts(double eta, double a)
+{
+    const double pi = 3.14159265358979323846264338327950288;
+    PairConsts<T> c;
+    const double c4 = 4.0 / (3.0 * a);                 // (1/(6 pi eta a)) / C1: translational self mobility
+    const double c8 = 1.0 / (a * a * a);               // (1/(8 pi eta a^3)) / C1: rotational self mobility
+    // floor of r^2: r = 0 becomes r = a 2^-40 (fp32) / a 2^-100 (fp64): a relative perturbation of the
+    // self term far below the type's epsilon, while 1/r^3 stays finite (1/r^5 may overflow to +inf in
+    // fp32; it only feeds the far branch, which the select discards for r < 2a)
+    c.tiny = (T)std::max(a * a * std::ldexp(1.0, sizeof(T) == 4 ? -80 : -200), sizeof(T) == 4 ? 4.8e-38 : 1e-300);
+    c.four_a2 = (T)(4.0 * a * a);
+    c.c2 = (T)(2.0 * a * a / 3.0);
+    c.nc3 = (T)(-2.0 * a * a);
+    c.c4 = (T)c4;
+    c.nc5 = (T)(-c4 * 9.0 / (32.0 * a));
+    c.c6 = (T)(c4 * 3.0 / (32.0 * a));
+    c.c8 = (T)c8;
+    c.k1 = (T)(-c8 * 27.0 / (32.0 * a));
+    c.k2 = (T)(c8 * 5.0 / (64.0 * a * a * a));
+    c.k3 = (T)(c8 * 9.0 / (32.0 * a));
+    c.k4 = (T)(-c8 * 3.0 / (64.0 * a * a * a));
+    c.k5 = (T)(1.0 / (2.0 * a * a * a));
+    c.k6 = (T)(-3.0 / (16.0 * a * a * a * a));
+    c.C1 = (T)(1.0 / (8.0 * pi * eta));                // Oseen prefactor, applied once per target
+    return c;
+}
+
+template <typename T> std::vector<Variant<T>>& variants(lm_solver* h);
+template <> std::vector<Variant<float>>& variants<float>(lm_solver* h) { return h->vf; }
+template <> std::vector<Variant<double>>& variants<double>(lm_solver* h) { return h->vd; }
+
+template <typename T> int init_variants(lm_solver* h)
+{
+    auto& vs = variants<T>(h);
+    vs = build_variants<T>();
+    for (auto& v : vs) {
+        LM_CUDA(h, cudaFuncSetAttribute((const void*)v.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem));
+        int nb = 0;
+        LM_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)v.kernel, v.block, v.smem));
+        v.ctas_per_sm = std::max(nb, 1);
+    }
+    return LM_OK;
+}
+
+// Pick the variant and the number of j-splits.  Sources are dealt to the splits in units of SUB, as
+// evenly as possible, so the grid can be sized to a whole number of resident sets (148 SMs x
+// resident CTAs per SM) whatever N is.  Cost model: CTAs run in waves of `slots`; a CTA costs
+// (its sources + a fixed prologue/epilogue) x its targets; CTAs resident on one SM share it.
+template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
+{
+    if (nrhs >= 0 && nrhs <= MAX_RHS) {
+        const auto& slot = h->plan_cache[nrhs];
+        if (slot.valid && slot.rb == h->row_begin && slot.re == h->row_end) return slot.plan;
+    }
+    const auto& vs = variants<T>(h);
+    LaunchPlan best;
+    double best_cost = 1e300;
+    for (int vi = 0; vi < (int)vs.size(); ++vi) {
+        const auto& v = vs[vi];
+        if (v.nrhs != nrhs || v.ang != h->angular) continue;
+        const int targets = v.block * v.tpt;
+        const int64_t rows = std::max<int64_t>(h->row_end - h->row_begin, 0);          // target rows of this rank / call
+        const int i_tiles = (int)((rows + targets - 1) / targets);
+        const int units = (int)(h->npad / v.sub);
+        const int64_t slots = (int64_t)h->sm_count * v.ctas_per_sm;
+        const int max_splits = std::min(units, 256);
+        const int min_splits = (int)std::min<int64_t>(max_splits, (h->npad + MAX_SOURCES_PER_CTA - 1) / MAX_SOURCES_PER_CTA);
+        for (int s = min_splits; s <= max_splits; ++s) {
+            const int64_t src = (int64_t)((units + s - 1) / s) * v.sub;            // sources of the largest split
+            const int64_t ctas = (int64_t)i_tiles * s;
+            const int64_t full = ctas / slots, rem = ctas % slots;
+            const int64_t rem_per_sm = (rem + h->sm_count - 1) / h->sm_count;      // CTAs sharing an SM in the last wave
+            // prologue, pipeline fill and epilogue of a CTA ~ 0.1 tile (fitted to plan sweeps on B200)
+            const double per_cta = ((double)src + 0.1 * v.tj) * targets / v.efficiency;
+            // few resident warps hide less latency: w warps per SM sub-partition cost a factor (1 + 0.3 / w)
+            auto wave = [&](int64_t resident) { return resident ? per_cta * resident * (1.0 + 0.3 * 128.0 / ((double)resident * v.block)) : 0.0; };
+            double cost = (double)full * wave(v.ctas_per_sm) + wave(rem_per_sm);
+            // cost is in pairs evaluated back to back on one SM (~1e4 per microsecond): the reduce pass
+            // adds a ~3 us launch plus writing and re-reading s partial vectors
+            if (s > 1) cost += 3.0e4 + 0.1 * (double)s * (double)rows;
+            if (cost < best_cost) {
+                best_cost = cost;
+                best.variant = vi;
+                best.i_tiles = i_tiles;
+                best.j_splits = s;
+                best.n_units = units;
+            }
+        }
+    }
+    if (nrhs >= 0 && nrhs <= MAX_RHS) {
+        auto& slot = h->plan_cache[nrhs];
+        slot.valid = true;
+        slot.rb = h->row_begin;
+        slot.re = h->row_end;
+        slot.plan = best;
+    }
+    return best;
+}
+
+cudaEvent_t get_event(lm_solver* h)
+{
+    if (!h->event_pool.empty()) {
+        cudaEvent_t e = h->event_pool.back();
+        h->event_pool.pop_back();
+        return e;
+    }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+
+int grid_1d(int64_t n) { return (int)std::max<int64_t>(1, (n + VEC_BLOCK - 1) / VEC_BLOCK); }
+int grid_red(int64_t n) { return (int)std::min<int64_t>(RED_MAX_BLOCKS, std::max<int64_t>(1, (n + VEC_BLOCK - 1) / VEC_BLOCK)); }
+
+
+}  // namespace

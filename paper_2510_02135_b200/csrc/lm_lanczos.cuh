@@ -1,0 +1,229 @@
+// lm_lanczos.cuh -- host driver of the Lanczos iteration for M^{1/2} W.
+// Included by lm_api.cu only, after lm_apply.cuh.
+#pragma once
+
+namespace {
+
+// ---------------------------------------------------------------- Lanczos driver (a7-a10)
+// nv <= MAX_RHS (angular: 2) independent Lanczos recurrences advanced in lockstep: one multi-right-hand-side
+// pair-kernel launch per iteration serves all of them, every other kernel runs
+// once per vector.  nv = 1 is lm_sqrt_mdot_w.  noise / outputs: [nv][dof] / [nv][3N].  iters_out: nv ints.
+template <typename T>
+int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out, T* ang_out, double scale, int accumulate, int* iters_out,
+                   cudaStream_t st)
+{
+    const int64_t dof = dof_of(h), n3 = 3 * h->N;
+    const int nc = h->angular ? 6 : 3;
+    const int kmax = h->max_iter;
+    const int ld = kmax + 2;
+    int rc;
+    if ((rc = ensure(h, &h->V, &h->V_bytes, (size_t)nv * (kmax + 1) * dof * sizeof(T))) != LM_OK) return rc;
+    if ((rc = ensure(h, &h->w, &h->w_bytes, (size_t)nv * dof * sizeof(T))) != LM_OK) return rc;
+    if (!h->d_scal) {
+        LM_CUDA(h, cudaMalloc((void**)&h->d_scal, MAX_RHS * 4 * sizeof(double)));
+        LM_CUDA(h, cudaMalloc((void**)&h->d_block, RED_MAX_BLOCKS * sizeof(double)));
+        LM_CUDA(h, cudaMalloc((void**)&h->d_ticket, sizeof(unsigned int)));
+        LM_CUDA(h, cudaMalloc((void**)&h->d_newest, sizeof(int)));
+        LM_CUDA(h, cudaMemsetAsync(h->d_ticket, 0, sizeof(unsigned int), st));
+        for (auto& e : h->lz_ev) LM_CUDA(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    if ((rc = ensure_capture_stream(h)) != LM_OK) return rc;
+    if (h->coef_cap < (size_t)(kmax + 2)) {
+        if (h->d_coef) { LM_CUDA(h, cudaFree(h->d_coef)); LM_CUDA(h, cudaFree(h->d_gram_part)); LM_CUDA(h, cudaFreeHost(h->h_gram)); LM_CUDA(h, cudaFreeHost(h->h_ab)); }
+        h->d_coef = nullptr;
+        h->coef_cap = 0;
+        LM_CUDA(h, cudaMalloc((void**)&h->d_coef, (size_t)MAX_RHS * (kmax + 2) * sizeof(double)));
+        LM_CUDA(h, cudaMalloc((void**)&h->d_gram_part, (size_t)(kmax + 2) * GRAM_MAX_BLOCKS * sizeof(double)));
+        LM_CUDA(h, cudaHostAlloc((void**)&h->h_gram, (size_t)MAX_RHS * ld * ld * sizeof(double), cudaHostAllocMapped));
+        LM_CUDA(h, cudaHostAlloc((void**)&h->h_ab, (size_t)MAX_RHS * 2 * ld * sizeof(double), cudaHostAllocMapped));
+        h->coef_cap = (size_t)(kmax + 2);
+    }
+    // per-vector views
+    auto Vq = [&](int q) { return (T*)h->V + (size_t)q * (kmax + 1) * dof; };
+    auto wq = [&](int q) { return (T*)h->w + (size_t)q * dof; };
+    auto scal = [&](int q) { return h->d_scal + 4 * q; };                       // [0] |z|^2  [1] alpha  [2] beta^2
+    auto ab = [&](int q) { return (volatile const double*)(h->h_ab + (size_t)q * 2 * ld); };
+    auto hg = [&](int q) { return (volatile const double*)(h->h_gram + (size_t)q * ld * ld); };
+    const int gr = grid_red(dof);
+    const int gg = (int)std::min<int64_t>(GRAM_MAX_BLOCKS, std::max<int64_t>(1, dof / (4 * VEC_BLOCK)));
+    const int64_t gchunk = (dof + gg - 1) / gg;
+    LaunchPlan plan;
+    if ((rc = prepare_apply<T>(h, nv, plan)) != LM_OK) return rc;
+    auto soa = [&](int q) { return (T*)h->vec_soa + (size_t)q * nc * h->npad; };
+    // Gram matrices of the bases, G[q][i][j] = V_q[i].V_q[j], filled one column per new basis vector
+    const int ldg = kmax + 1;
+    std::vector<std::vector<double>> G(nv, std::vector<double>((size_t)ldg * ldg, 0.0));
+    auto gram_store = [&](int q, int m) {
+        for (int j = 0; j <= m; ++j) G[q][(size_t)j * ldg + m] = G[q][(size_t)m * ldg + j] = hg(q)[(size_t)m * ld + j];
+    };
+    // new basis vectors V_q[*newest + 1] = x_q / sqrt(sumsq_q) (+ packed copies for the next apply), their Gram
+    // columns, then *newest += 1 (once: the recurrences move in lockstep)
+    auto new_vectors = [&](const T* x, int which_scal, cudaStream_t s2) {
+        for (int q = 0; q < nv; ++q) {
+            lanczos_scale_pack_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(x + (size_t)q * dof, h->N, h->npad, nc, scal(q) + which_scal, h->d_newest,
+                                                                              Vq(q), soa(q));
+            gram_column_kernel<T><<<dim3(gg, kmax + 1), VEC_BLOCK, 0, s2>>>(Vq(q), dof, h->d_newest, gchunk, h->d_gram_part, h->d_ticket,
+                                                                             h->h_gram + (size_t)q * ld * ld, ld);
+        }
+        lanczos_advance_kernel<<<1, 1, 0, s2>>>(h->d_newest);
+    };
+
+    // v_1 = z / |z|
+    LM_CUDA(h, cudaMemsetAsync(h->d_newest, 0xff, sizeof(int), st));            // *newest = -1
+    for (int q = 0; q < nv; ++q)
+        sumsq_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise + (size_t)q * dof, dof, h->d_block, h->d_ticket, scal(q), h->h_ab + (size_t)q * 2 * ld + 1);
+    new_vectors(noise, 0, st);
+    h->n_aux += 3 * nv + 1;
+    LM_CUDA(h, cudaGetLastError());
+    LM_CUDA(h, cudaStreamSynchronize(st));
+    std::vector<double> znorm(nv);
+    std::vector<char> done(nv, 0), conv(nv, 0);
+    std::vector<int> kfin(nv, 0);
+    std::vector<std::vector<double>> alphas(nv), betas(nv), c_prev(nv), c_cur(nv), c_fin(nv);
+    int remaining = nv;
+    for (int q = 0; q < nv; ++q) {
+        gram_store(q, 0);
+        znorm[q] = std::sqrt(ab(q)[1]);
+        if (!(znorm[q] > 0.0)) { done[q] = conv[q] = 1; --remaining; }            // zero noise: M^{1/2} 0 = 0
+    }
+    h->last_iters = 0;
+
+    // Iteration k on the device, with m = k - 1 = *newest, for every vector:  w = M v_k;  w -= beta_{k-1} v_{k-1};
+    // alpha_k;  w -= alpha_k v_k;  beta_k^2;  v_{k+1} = w / beta_k (+ packed for the next apply);  Gram column k.
+    // Everything the device needs stays on the device; the host only READS (alpha_k, beta_k^2, Gram column)
+    // from mapped pinned memory for the stopping test.  The launch sequence and its arguments are the
+    // same for every k, so it is captured once as a CUDA graph.
+    RhsOut<T> out{};
+    for (int q = 0; q < nv; ++q) {
+        out.lin[q] = wq(q);
+        out.ang[q] = h->angular ? wq(q) + n3 : nullptr;
+    }
+    auto body = [&](cudaStream_t s2, bool timed) -> int {
+        int rc2;
+        if ((rc2 = launch_pair<T>(h, nv, plan, out, s2, timed)) != LM_OK) return rc2;                      // w_q = M v_k,q
+        for (int q = 0; q < nv; ++q) {
+            lanczos_alpha_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q) + 2, dof, h->d_block, h->d_ticket, scal(q) + 1);
+            lanczos_beta_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q) + 1, dof, h->d_block, h->d_ticket, scal(q) + 2,
+                                                             h->h_ab + (size_t)q * 2 * ld);
+        }
+        new_vectors((const T*)h->w, 2, s2);
+        LM_CUDA(h, cudaGetLastError());
+        return LM_OK;
+    };
+    // One iteration of look-ahead when an apply is short: iteration k+1 is enqueued BEFORE the host waits
+    // for iteration k's scalars, so the device never idles on the host round trip.  The price is one
+    // wasted apply at convergence, so it is used only where an apply costs less than the round trips it
+    // saves (~25 iterations x 50 us); the same regime is launch-bound, so there the body runs as a graph.
+    const double apply_cost = (double)h->N * (double)h->N * (h->angular ? 2.3 : 1.0) * (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nv);
+    const bool lookahead = apply_cost < 2.0e9;
+    const bool use_graph = lookahead && !h->profiling && h->dist_ranks == 0 && std::getenv("LM_NO_GRAPH") == nullptr;
+    if (use_graph && remaining > 0) {
+        const lm_solver::GraphKey key = {h->V, h->w, h->vec_soa, h->partial, h->pos_soa, kmax, plan.variant, plan.j_splits, h->precision * 8 + nv};
+        if (!h->lz_graph || std::memcmp(&key, &h->lz_key, sizeof key) != 0) {
+            if (h->lz_graph) { LM_CUDA(h, cudaGraphExecDestroy(h->lz_graph)); h->lz_graph = nullptr; }
+            cudaGraph_t graph = nullptr;
+            LM_CUDA(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+            const int rc_body = body(h->cap_stream, false);
+            const cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
+            if (rc_body != LM_OK) { if (graph) cudaGraphDestroy(graph); return rc_body; }
+            LM_CUDA(h, ce);
+            const cudaError_t ci = cudaGraphInstantiate(&h->lz_graph, graph, 0);
+            cudaGraphDestroy(graph);
+            LM_CUDA(h, ci);
+            h->lz_key = key;
+        }
+    }
+    auto enqueue = [&](int k) -> int {
+        if (use_graph) {
+            LM_CUDA(h, cudaGraphLaunch(h->lz_graph, st));
+        } else {
+            const int rc2 = body(st, h->profiling);
+            if (rc2 != LM_OK) return rc2;
+        }
+        count_apply(h, plan);
+        h->n_aux += 4 * nv + 1;
+        LM_CUDA(h, cudaEventRecord(h->lz_ev[k & 1], st));
+        return LM_OK;
+    };
+
+    const bool debug = std::getenv("LM_DEBUG_LANCZOS") != nullptr;   // per-iteration trace on stderr
+    const double breakdown = (h->precision == LM_F32) ? 1e-6 : 1e-14;
+    int k = 0;
+    if (remaining > 0 && (rc = enqueue(1)) != LM_OK) return rc;
+    for (k = 1; k <= kmax && remaining > 0; ++k) {
+        if (lookahead && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
+        LM_CUDA(h, cudaEventSynchronize(h->lz_ev[k & 1]));
+        for (int q = 0; q < nv; ++q) {
+            if (done[q]) continue;
+            const double alpha = ab(q)[2 * k], beta = std::sqrt(std::max((double)ab(q)[2 * k + 1], 0.0));
+            if (!std::isfinite(alpha) || !std::isfinite(beta)) {
+                cudaStreamSynchronize(st);
+                return fail(h, LM_E_CUDA, "Lanczos: non-finite alpha/beta (non-finite input?)");
+            }
+            alphas[q].push_back(alpha);
+            c_cur[q].assign(k, 0.0);
+            if (!tridiag_sqrt_e1(k, alphas[q].data(), betas[q].data(), c_cur[q].data())) {
+                cudaStreamSynchronize(st);
+                return fail(h, LM_E_NOCONV, "Lanczos: tridiagonal eigensolve did not converge");
+            }
+            bool converged = false;
+            if (k >= 2) {
+                // |y_k - y_{k-1}|^2 / |z|^2 = delta^T G_k delta,  |y_{k-1}|^2 / |z|^2 = c_{k-1}^T G_{k-1} c_{k-1}
+                std::vector<double> delta(c_cur[q]);
+                for (int i = 0; i < k - 1; ++i) delta[i] -= c_prev[q][i];
+                double num = 0.0, den = 0.0;
+                for (int i = 0; i < k; ++i)
+                    for (int j = 0; j < k; ++j) num += delta[i] * G[q][(size_t)i * ldg + j] * delta[j];
+                for (int i = 0; i < k - 1; ++i)
+                    for (int j = 0; j < k - 1; ++j) den += c_prev[q][i] * G[q][(size_t)i * ldg + j] * c_prev[q][j];
+                if (std::sqrt(std::max(num, 0.0)) <= tol * std::sqrt(std::max(den, 0.0))) converged = true;
+                if (debug)
+                    std::fprintf(stderr, "[lm lanczos] vec=%d k=%d alpha=%.9e beta=%.9e step=%.3e\n", q, k, alpha, beta, std::sqrt(std::max(num, 0.0) / den));
+            }
+            if (beta <= breakdown * std::fabs(alpha)) converged = true;   // invariant subspace: iterate is exact
+            if (converged || k == kmax) {
+                done[q] = 1;
+                conv[q] = converged;
+                kfin[q] = k;
+                c_fin[q] = c_cur[q];
+                --remaining;
+                continue;
+            }
+            gram_store(q, k);
+            betas[q].push_back(beta);
+            c_prev[q] = c_cur[q];
+        }
+        if (!lookahead && remaining > 0 && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
+    }
+    // results: y_q = scale |z_q| V_q c_q  (a10)
+    bool all_converged = true;
+    std::vector<double> coef((size_t)nv * (kmax + 2), 0.0);
+    for (int q = 0; q < nv; ++q) {
+        all_converged = all_converged && conv[q];
+        for (int i = 0; i < kfin[q]; ++i) coef[(size_t)q * (kmax + 2) + i] = c_fin[q][i];
+        if (iters_out) iters_out[q] = kfin[q];
+        h->last_iters = std::max(h->last_iters, kfin[q]);
+    }
+    LM_CUDA(h, cudaMemcpyAsync(h->d_coef, coef.data(), coef.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    for (int q = 0; q < nv; ++q) {
+        T* lo = lin_out + (size_t)q * n3;
+        T* ao = h->angular ? ang_out + (size_t)q * n3 : nullptr;
+        if (kfin[q] == 0) {               // zero noise vector
+            if (!accumulate) {
+                LM_CUDA(h, cudaMemsetAsync(lo, 0, (size_t)n3 * sizeof(T), st));
+                if (h->angular) LM_CUDA(h, cudaMemsetAsync(ao, 0, (size_t)n3 * sizeof(T), st));
+            }
+            continue;
+        }
+        lanczos_combine_kernel<T><<<grid_1d(dof), VEC_BLOCK, 0, st>>>(Vq(q), dof, kfin[q], h->d_coef + (size_t)q * (kmax + 2), scale * znorm[q], accumulate,
+                                                                       n3, lo, ao);
+        h->n_aux++;
+    }
+    LM_CUDA(h, cudaGetLastError());
+    LM_CUDA(h, cudaStreamSynchronize(st));      // coef (pageable) must outlive the copy; drains a look-ahead iteration
+    if (!all_converged) return fail(h, LM_E_NOCONV, "Lanczos: max_iter reached before the tolerance was met (last iterate written)");
+    return LM_OK;
+}
+
+
+}  // namespace
