@@ -68,7 +68,12 @@ enum {
 /* Create a solver for N equal spheres of hydrodynamic radius a in an unbounded fluid of viscosity
  * eta.  include_angular != 0: torques are accepted and angular velocities returned (dof = 6N),
  * else forces -> linear velocities only (dof = 3N; "more efficient").  Uses the
- * current CUDA device; all later calls on the handle must run with that device current. */
+ * current CUDA device; all later calls on the handle must run with that device current.
+ * Any consistent unit system works, SI included (a = 1e-6, eta = 1e-3 ...): internally lengths are stored
+ * multiplied by the power of two nearest 1/a (exact), so the kernels always see a radius of order one.
+ * One caveat is the method's, not the kernels': with include_angular the 6N x 6N matrix mixes blocks
+ * ~ 1/(eta a) and ~ 1/(eta a^3), so its square root (lm_sqrt_mdot_w) is well scaled only in units with a of
+ * order one; in fp32 use such units for the angular noise. */
 int lm_create(lm_solver** out, int precision, int64_t N, double eta, double a, int include_angular);
 int lm_destroy(lm_solver* h);
 

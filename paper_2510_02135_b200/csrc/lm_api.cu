@@ -34,7 +34,7 @@ namespace {
 // ---------------------------------------------------------------- typed front ends
 template <typename T> int set_positions_t(lm_solver* h, const void* pos, cudaStream_t st)
 {
-    pack_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)pos, h->N, h->npad, (T*)h->pos_soa);
+    pack_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)pos, h->N, h->npad, (T)h->len_scale, (T*)h->pos_soa);
     h->n_aux++;
     LM_CUDA(h, cudaGetLastError());
     h->have_pos = true;
@@ -124,6 +124,8 @@ int lm_create(lm_solver** out, int precision, int64_t N, double eta, double a, i
     h->eta = eta;
     h->a = a;
     h->angular = include_angular ? 1 : 0;
+    h->len_scale = std::ldexp(1.0, -(int)std::lround(std::log2(a)));      // power of two nearest 1/a
+    if (precision == LM_F32 && (h->len_scale > 0x1p100 || h->len_scale < 0x1p-100)) { delete h; return LM_E_INVALID; }   // a outside fp32's comfortable range
     h->npad = (N + NPAD_QUANTUM - 1) / NPAD_QUANTUM * NPAD_QUANTUM;
     h->row_begin = 0;
     h->row_end = N;

@@ -53,7 +53,7 @@ template <typename T> int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& 
     p.i_end = h->row_end;
     p.npad = h->npad;
     p.n_units = plan.n_units;
-    p.c = make_consts<T>(h->eta, h->a);
+    p.c = make_consts<T>(h->eta, h->a * h->len_scale, h->len_scale);
 
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (timed) {
@@ -111,7 +111,7 @@ template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& i
     int rc = prepare_apply<T>(h, nrhs, plan);
     if (rc != LM_OK) return rc;
     auto direct = [&](cudaStream_t s2, bool timed) -> int {
-        pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(in, nrhs, nc, h->N, h->npad, (T*)h->vec_soa);
+        pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(in, nrhs, nc, h->N, h->npad, (T)h->len_scale, (T*)h->vec_soa);
         return launch_pair<T>(h, nrhs, plan, out, s2, timed);
     };
     // A short apply is bound by the host's three launches (~11 us measured against ~3 us of kernels each): when

@@ -36,11 +36,13 @@ int steric_device(lm_solver* h, double U0, double b, const T* ext, T* out, cudaS
     p.npad = h->npad;
     p.i_begin = h->row_begin;
     p.n_units = units;
-    p.tiny = make_consts<T>(h->eta, h->a).tiny;
-    p.d = (T)(2.0 * h->a);
-    p.rc2 = (T)((2.0 * h->a + K * b) * (2.0 * h->a + K * b));
+    // lengths in the internal unit (x len_scale); the force magnitude U0 / b stays in the caller's units
+    const double ls = h->len_scale, as = h->a * ls, bs = b * ls;
+    p.tiny = make_consts<T>(h->eta, as, ls).tiny;
+    p.d = (T)(2.0 * as);
+    p.rc2 = (T)((2.0 * as + K * bs) * (2.0 * as + K * bs));
     p.m0 = (T)(U0 / b);
-    p.inv_b = (T)(sizeof(T) == 4 ? 1.4426950408889634 / b : 1.0 / b);
+    p.inv_b = (T)(sizeof(T) == 4 ? 1.4426950408889634 / bs : 1.0 / bs);
     if (i_tiles > 0) {
         steric_pair_kernel<T><<<dim3(i_tiles, splits), STERIC_BLOCK, steric_smem_bytes<T>(), st>>>(p);
         steric_reduce_kernel<T><<<grid_1d(rows), VEC_BLOCK, 0, st>>>((const T*)h->partial, splits, h->row_begin, h->row_end, h->npad, ext, kout);
@@ -68,7 +70,7 @@ int rfd_device(lm_solver* h, const T* W, double delta, T* lin_out, T* ang_out, c
     void* const home = h->pos_soa;
     T* outs[2][2] = {{lin_out, ang_out}, {(T*)h->rfd[1], (T*)h->rfd[2]}};
     for (int side = 0; side < 2; ++side) {
-        shift_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)home, W, h->N, h->npad, (T)((side ? -0.5 : 0.5) * delta), (T*)h->rfd[0]);
+        shift_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)home, W, h->N, h->npad, (T)((side ? -0.5 : 0.5) * delta * h->len_scale), (T*)h->rfd[0]);
         h->n_aux++;
         h->pos_soa = h->rfd[0];                       // the apply reads the displaced copy; the handle's positions are untouched
         rc = apply_batch<T>(h, 1, W, nullptr, outs[side][0], h->angular ? outs[side][1] : nullptr, st);

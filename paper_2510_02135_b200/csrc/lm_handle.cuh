@@ -105,6 +105,7 @@ struct lm_solver {
     int precision = LM_F32;
     int64_t N = 0, npad = 0;
     double eta = 1.0, a = 1.0;
+    double len_scale = 1.0;    // power of two nearest 1/a: lengths are stored x len_scale, so the kernels see a radius in [0.71, 1.41]
     int angular = 0;
     int max_iter = 100;
     int device = 0, sm_count = 0;
@@ -211,7 +212,10 @@ int ensure(lm_solver* h, void** ptr, size_t* cap, size_t bytes)
     return LM_OK;
 }
 
-template <typename T> PairConsts<T> make_consts(double eta, double a)
+// Constants of the pair tensors in the internal length unit: `a` here is a * len_scale; a velocity computed
+// from scaled lengths is 1/len_scale times the true one (M_uF ~ 1/r), an angular velocity 1/len_scale^2
+// (M_wF ~ 1/r^2; the torques were scaled on packing), hence the two epilogue factors.  All powers of two: exact.
+template <typename T> PairConsts<T> make_consts(double eta, double a, double len_scale)
 {
     const double pi = 3.14159265358979323846264338327950288;
     PairConsts<T> c;
@@ -234,7 +238,8 @@ template <typename T> PairConsts<T> make_consts(double eta, double a)
     c.k4 = (T)(-c8 * 3.0 / (64.0 * a * a * a));
     c.k5 = (T)(1.0 / (2.0 * a * a * a));
     c.k6 = (T)(-3.0 / (16.0 * a * a * a * a));
-    c.C1 = (T)(1.0 / (8.0 * pi * eta));                // Oseen prefactor, applied once per target
+    c.C1_lin = (T)(len_scale / (8.0 * pi * eta));                  // Oseen prefactor, applied once per target
+    c.C1_ang = (T)(len_scale * len_scale / (8.0 * pi * eta));
     return c;
 }
 

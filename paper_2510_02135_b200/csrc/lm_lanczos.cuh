@@ -60,7 +60,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     // columns, then *newest += 1 (once: the recurrences move in lockstep)
     auto new_vectors = [&](const T* x, int which_scal, cudaStream_t s2) {
         for (int q = 0; q < nv; ++q) {
-            lanczos_scale_pack_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(x + (size_t)q * dof, h->N, h->npad, nc, scal(q) + which_scal, h->d_newest,
+            lanczos_scale_pack_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(x + (size_t)q * dof, h->N, h->npad, nc, (T)h->len_scale, scal(q) + which_scal, h->d_newest,
                                                                               Vq(q), soa(q));
             gram_column_kernel<T><<<dim3(gg, kmax + 1), VEC_BLOCK, 0, s2>>>(Vq(q), dof, h->d_newest, gchunk, h->d_gram_part, h->d_ticket,
                                                                              h->h_gram + (size_t)q * ld * ld, ld);

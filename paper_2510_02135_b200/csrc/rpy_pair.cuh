@@ -107,7 +107,7 @@ template <typename T> struct PairConsts {
     T four_a2; // (2a)^2
     T c2, nc3, c4, nc5, c6;               // translation-translation
     T c8, k1, k2, k3, k4, k5, k6;         // rotation-rotation and coupling (near branch)
-    T C1;                                 // 1/(8 pi eta): applied in the epilogue
+    T C1_lin, C1_ang;                     // 1/(8 pi eta) x the internal length unit (x its square): applied in the epilogue
 };
 
 // overlap detector of the far-field fast path: running minimum of r^2 over a group of pairs.
@@ -421,7 +421,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 #pragma unroll
     for (int q = 0; q < NP; ++q)
 #pragma unroll
-        for (int k = 0; k < NV; ++k) total[q][k] = mul2(total[q][k], p.c.C1);
+        for (int k = 0; k < NV; ++k) total[q][k] = mul2(total[q][k], (k % NC) < 3 ? p.c.C1_lin : p.c.C1_ang);
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
 #pragma unroll

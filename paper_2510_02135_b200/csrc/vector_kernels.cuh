@@ -11,23 +11,26 @@ namespace lm {
 constexpr int VEC_BLOCK = 256;       // threads per block of every kernel in this file
 constexpr int RED_MAX_BLOCKS = 1024; // upper bound on the grid of the reduction kernels
 
-// a1: interleaved positions (3N) -> x | y | z, each npad long, ghosts zero.
+// a1: interleaved positions (3N) -> x | y | z, each npad long, ghosts zero.  Lengths are stored multiplied by
+// `len_scale`, the power of two nearest 1/a (exact): the pair kernel then works with a radius in [0.71, 1.41]
+// whatever unit system the caller uses ("internal length unit").
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) pack_positions_kernel(const T* __restrict__ pos, int64_t N, int64_t npad, T* __restrict__ soa)
+__global__ void __launch_bounds__(VEC_BLOCK) pack_positions_kernel(const T* __restrict__ pos, int64_t N, int64_t npad, T len_scale, T* __restrict__ soa)
 {
     const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
     if (i >= npad) return;
     T x = T(0), y = T(0), z = T(0);
-    if (i < N) { x = pos[3 * i]; y = pos[3 * i + 1]; z = pos[3 * i + 2]; }
+    if (i < N) { x = pos[3 * i] * len_scale; y = pos[3 * i + 1] * len_scale; z = pos[3 * i + 2] * len_scale; }
     soa[i] = x;
     soa[npad + i] = y;
     soa[2 * npad + i] = z;
 }
 
 // a2: right-hand sides -> [nrhs*NC][npad] component arrays (NC = 3: Fx Fy Fz; NC = 6: + Tx Ty Tz),
-// ghosts zero; a null force / torque pointer means zeros.
+// ghosts zero; a null force / torque pointer means zeros.  Torques are stored multiplied by
+// `len_scale` (the internal length unit: a torque is a force times a length).
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) pack_rhs_kernel(RhsIn<T> in, int nrhs, int nc, int64_t N, int64_t npad, T* __restrict__ soa)
+__global__ void __launch_bounds__(VEC_BLOCK) pack_rhs_kernel(RhsIn<T> in, int nrhs, int nc, int64_t N, int64_t npad, T len_scale, T* __restrict__ soa)
 {
     const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
     if (i >= npad) return;
@@ -35,7 +38,7 @@ __global__ void __launch_bounds__(VEC_BLOCK) pack_rhs_kernel(RhsIn<T> in, int nr
         T v[6] = {T(0), T(0), T(0), T(0), T(0), T(0)};
         if (i < N) {
             if (in.f[q]) { v[0] = in.f[q][3 * i]; v[1] = in.f[q][3 * i + 1]; v[2] = in.f[q][3 * i + 2]; }
-            if (nc == 6 && in.t[q]) { v[3] = in.t[q][3 * i]; v[4] = in.t[q][3 * i + 1]; v[5] = in.t[q][3 * i + 2]; }
+            if (nc == 6 && in.t[q]) { v[3] = in.t[q][3 * i] * len_scale; v[4] = in.t[q][3 * i + 1] * len_scale; v[5] = in.t[q][3 * i + 2] * len_scale; }
         }
         for (int k = 0; k < nc; ++k) soa[(size_t)(q * nc + k) * npad + i] = v[k];
     }
@@ -154,7 +157,7 @@ __global__ void __launch_bounds__(VEC_BLOCK) sumsq_kernel(const T* __restrict__ 
 // vector packed as the pair kernel's structure-of-arrays right-hand side (a2) for the next apply:
 // soa[c][i], c < nc, ghosts zero.  x and V hold [3N linear | 3N angular].
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) lanczos_scale_pack_kernel(const T* __restrict__ x, int64_t N, int64_t npad, int nc,
+__global__ void __launch_bounds__(VEC_BLOCK) lanczos_scale_pack_kernel(const T* __restrict__ x, int64_t N, int64_t npad, int nc, T len_scale,
                                                                        const double* sumsq, const int* __restrict__ newest,
                                                                        T* __restrict__ V, T* __restrict__ soa)
 {
@@ -171,7 +174,7 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_scale_pack_kernel(const T* 
             val = (T)((double)x[idx] * inv);
             v_out[idx] = val;
         }
-        soa[(size_t)c * npad + i] = val;
+        soa[(size_t)c * npad + i] = c < 3 ? val : val * len_scale;       // angular part: internal length unit, as in pack_rhs
     }
 }
 

@@ -513,3 +513,43 @@ def test_repeated_small_applies_replay_a_graph_on_current_data(lm, torch, prec):
     ref = rpy.mdot(X2.cpu().numpy().reshape(N, 3), f)[0]
     assert rel(U2.cpu().numpy(), ref) <= TOL[prec] and rel(U.cpu().numpy(), ref) <= TOL[prec]
     s.close()
+
+
+@pytest.mark.parametrize("a,eta", [(1e-6, 1e-3), (1e-9, 1.0), (3.7e4, 2.5e-2)])
+def test_fp32_in_any_unit_system(lm, torch, a, eta):
+    """SI micrometre spheres in water (a = 1e-6 m, eta = 1e-3 Pa s), nanometres, and a large odd radius: the
+    internal power-of-two length unit keeps the fp32 angular blocks, the steric force and the Lanczos root in
+    range; same gates as for a = eta = 1."""
+    N = 600
+    rng = np.random.default_rng(12)
+    pos = (rng.random((N, 3)) * 13.0 * a).astype(np.float32)
+    F = (rng.standard_normal((N, 3)) * 1e-12).astype(np.float32)
+    T = (rng.standard_normal((N, 3)) * 1e-12 * a).astype(np.float32)
+    W = rng.standard_normal(6 * N).astype(np.float32)
+    s = lm.Solver("f32", N, eta, a, True)
+    s.set_positions(dev(torch, pos))
+    U = torch.empty(3 * N, dtype=torch.float32, device="cuda")
+    Om = torch.empty_like(U)
+    s.mdot(dev(torch, F), dev(torch, T), U, Om)
+    torch.cuda.synchronize()
+    Uo, Oo = rpy.mdot(pos, F, T, a=a, eta=eta, angular=True)
+    assert rel(U.cpu().numpy(), Uo) <= 2e-5 and rel(Om.cpu().numpy(), Oo) <= 2e-5
+    # The Lanczos root is checked on the translational solver: with include_angular the 6N x 6N matrix mixes
+    # blocks ~ 1/(eta a) and ~ 1/(eta a^3), so in such units its symmetric root spans ~ a^-1 orders of magnitude
+    # inside one vector -- a property of the method in those units (include/lm.h), not of the kernels.
+    st = lm.Solver("f32", N, eta, a, False)
+    st.set_positions(dev(torch, pos))
+    it = st.sqrt_mdot_w(dev(torch, W[: 3 * N]), 1e-3, U, None)
+    torch.cuda.synchronize()
+    y = U.cpu().numpy()
+    exact = rpy.dense_sqrt_mdot_w(pos, W[: 3 * N], a=a, eta=eta)
+    assert np.all(np.isfinite(y)) and 2 <= it < 100
+    assert rel(y, exact) <= 1e-2
+    st.close()
+    from oracle import bd
+    Fs = torch.empty(3 * N, dtype=torch.float32, device="cuda")
+    U0, b = 4 * 4.11e-21, 0.1 * a
+    s.steric_forces(U0, b, None, Fs)
+    torch.cuda.synchronize()
+    assert rel(Fs.cpu().numpy(), bd.steric_forces(pos, U0, b, 2 * a)) <= 2e-5
+    s.close()
