@@ -25,7 +25,8 @@ template <typename T> int prepare_apply(lm_solver* h, int nrhs, LaunchPlan& plan
 // this rank's block: the kernel writes into all-gather buffers of 3 B ranks elements, ONE grouped
 // ncclAllGather (in place: rank r's segment starts at 3 B r) completes every output on every rank, and the
 // first 3N elements are copied to the caller's buffers.
-template <typename T> int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>& out, cudaStream_t st, bool timed)
+template <typename T>
+int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>& out, cudaStream_t st, bool timed, bool reduce = true)
 {
     const int nc = h->angular ? 6 : 3;
     const auto& v = variants<T>(h)[plan.variant];
@@ -66,7 +67,7 @@ template <typename T> int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& 
         LM_CUDA(h, cudaEventRecord(e1, st));
         h->pending.emplace_back(e0, e1);
     }
-    if (plan.i_tiles > 0 && plan.j_splits > 1)
+    if (plan.i_tiles > 0 && plan.j_splits > 1 && reduce)      // reduce == false: the caller's next kernel sums the partials itself
         reduce_partials_kernel<T><<<dim3(grid_1d(h->row_end - h->row_begin), nrhs * nc), VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc,
                                                                                                          h->row_begin, h->row_end, h->npad, kout);
     LM_CUDA(h, cudaGetLastError());

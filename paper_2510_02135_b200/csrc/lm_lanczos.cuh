@@ -57,7 +57,8 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
         for (int j = 0; j <= m; ++j) G[q][(size_t)j * ldg + m] = G[q][(size_t)m * ldg + j] = hg(q)[(size_t)m * ld + j];
     };
     // new basis vectors V_q[*newest + 1] = x_q / sqrt(sumsq_q) (+ packed copies for the next apply), their Gram
-    // columns, then *newest += 1 (once: the recurrences move in lockstep)
+    // columns; *newest was advanced to their slot by the reduction that produced the norms (sumsq / beta kernel of
+    // the LAST vector: the recurrences move in lockstep)
     auto new_vectors = [&](const T* x, int which_scal, cudaStream_t s2) {
         for (int q = 0; q < nv; ++q) {
             lanczos_scale_pack_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(x + (size_t)q * dof, h->N, h->npad, nc, (T)h->len_scale, scal(q) + which_scal, h->d_newest,
@@ -65,15 +66,15 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
             gram_column_kernel<T><<<dim3(gg, kmax + 1), VEC_BLOCK, 0, s2>>>(Vq(q), dof, h->d_newest, gchunk, h->d_gram_part, h->d_ticket,
                                                                              h->h_gram + (size_t)q * ld * ld, ld);
         }
-        lanczos_advance_kernel<<<1, 1, 0, s2>>>(h->d_newest);
     };
 
     // v_1 = z / |z|
     LM_CUDA(h, cudaMemsetAsync(h->d_newest, 0xff, sizeof(int), st));            // *newest = -1
     for (int q = 0; q < nv; ++q)
-        sumsq_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise + (size_t)q * dof, dof, h->d_block, h->d_ticket, scal(q), h->h_ab + (size_t)q * 2 * ld + 1);
+        sumsq_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise + (size_t)q * dof, dof, h->d_block, h->d_ticket, scal(q), h->h_ab + (size_t)q * 2 * ld + 1,
+                                                  q == nv - 1 ? h->d_newest : nullptr);
     new_vectors(noise, 0, st);
-    h->n_aux += 3 * nv + 1;
+    h->n_aux += 3 * nv;
     LM_CUDA(h, cudaGetLastError());
     LM_CUDA(h, cudaStreamSynchronize(st));
     std::vector<double> znorm(nv);
@@ -98,13 +99,17 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
         out.lin[q] = wq(q);
         out.ang[q] = h->angular ? wq(q) + n3 : nullptr;
     }
+    // the alpha kernel doubles as the split-j reduce of the apply (one launch less per vector and iteration),
+    // except for row-sharded runs, where w must be all-gathered before any rank can use it
+    const bool fuse_reduce = plan.j_splits > 1 && plan.i_tiles > 0 && h->dist_ranks == 0;
     auto body = [&](cudaStream_t s2, bool timed) -> int {
         int rc2;
-        if ((rc2 = launch_pair<T>(h, nv, plan, out, s2, timed)) != LM_OK) return rc2;                      // w_q = M v_k,q
+        if ((rc2 = launch_pair<T>(h, nv, plan, out, s2, timed, !fuse_reduce)) != LM_OK) return rc2;       // w_q = M v_k,q
         for (int q = 0; q < nv; ++q) {
-            lanczos_alpha_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q) + 2, dof, h->d_block, h->d_ticket, scal(q) + 1);
+            lanczos_alpha_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q) + 2, dof, h->d_block, h->d_ticket, scal(q) + 1,
+                                                              fuse_reduce ? (const T*)h->partial : nullptr, plan.j_splits, nv, q, nc, h->npad);
             lanczos_beta_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q) + 1, dof, h->d_block, h->d_ticket, scal(q) + 2,
-                                                             h->h_ab + (size_t)q * 2 * ld);
+                                                             h->h_ab + (size_t)q * 2 * ld, q == nv - 1 ? h->d_newest : nullptr);
         }
         new_vectors((const T*)h->w, 2, s2);
         LM_CUDA(h, cudaGetLastError());
@@ -141,7 +146,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
             if (rc2 != LM_OK) return rc2;
         }
         count_apply(h, plan);
-        h->n_aux += 4 * nv + 1;
+        h->n_aux += 4 * nv;
         LM_CUDA(h, cudaEventRecord(h->lz_ev[k & 1], st));
         return LM_OK;
     };

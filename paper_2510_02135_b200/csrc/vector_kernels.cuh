@@ -105,7 +105,7 @@ __device__ __forceinline__ double warp_sum(double v)
 }
 
 __device__ __forceinline__ void block_reduce_to_scalar(double v, double* block_partials, unsigned int* ticket, double* result,
-                                                       double* host_mirror = nullptr)
+                                                       double* host_mirror = nullptr, int* advance = nullptr)
 {
     __shared__ double warp_part[VEC_BLOCK / 32];
     __shared__ bool is_last;
@@ -130,6 +130,7 @@ __device__ __forceinline__ void block_reduce_to_scalar(double v, double* block_p
         if (threadIdx.x == 0) {
             *result = s;
             if (host_mirror) *host_mirror = s;
+            if (advance) *advance += 1;       // every block has taken its ticket, hence read the old value: safe to move on
             *ticket = 0u;
         }
     }
@@ -138,14 +139,14 @@ __device__ __forceinline__ void block_reduce_to_scalar(double v, double* block_p
 // result = sum_i x_i^2          (|z|^2 of the noise vector)
 template <typename T>
 __global__ void __launch_bounds__(VEC_BLOCK) sumsq_kernel(const T* __restrict__ x, int64_t n, double* block_partials, unsigned int* ticket,
-                                                          double* result, double* host_mirror)
+                                                          double* result, double* host_mirror, int* advance)
 {
     double s = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * VEC_BLOCK) {
         const double v = (double)x[i];
         s = fma(v, v, s);
     }
-    block_reduce_to_scalar(s, block_partials, ticket, result, host_mirror);
+    block_reduce_to_scalar(s, block_partials, ticket, result, host_mirror, advance);
 }
 
 // The kernels of one Lanczos iteration read the index m of the NEWEST basis vector V[m] from device
@@ -153,7 +154,8 @@ __global__ void __launch_bounds__(VEC_BLOCK) sumsq_kernel(const T* __restrict__ 
 // the driver captures it once in a CUDA graph and replays it (the loop is launch-bound at small N).
 // Scalars the host needs for the stopping test are written straight into mapped pinned host memory.
 
-// V[*newest + 1] = x / sqrt(*sumsq)  (v_1 = z/|z| with *newest = -1; v_{k+1} = w/beta_k), and the same
+// V[*newest] = x / sqrt(*sumsq)  (v_1 = z/|z|; v_{k+1} = w/beta_k: the reduction that produced *sumsq has
+// already advanced *newest to the slot of the vector being written), and the same
 // vector packed as the pair kernel's structure-of-arrays right-hand side (a2) for the next apply:
 // soa[c][i], c < nc, ghosts zero.  x and V hold [3N linear | 3N angular].
 template <typename T>
@@ -166,7 +168,7 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_scale_pack_kernel(const T* 
     const double nrm = sqrt(*sumsq);
     const double inv = nrm > 0.0 ? 1.0 / nrm : 0.0;
     const int64_t n3 = 3 * N, dof = (int64_t)nc * N;
-    T* v_out = V + (size_t)(*newest + 1) * dof;
+    T* v_out = V + (size_t)(*newest) * dof;
     for (int c = 0; c < nc; ++c) {
         T val = T(0);
         if (i < N) {
@@ -178,18 +180,31 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_scale_pack_kernel(const T* 
     }
 }
 
-// v = V[*newest]:  w -= sqrt(*beta_prev_sq) * V[*newest - 1]  (skipped for *newest == 0);  *alpha = w . v
+// v = V[*newest]:  w -= sqrt(*beta_prev_sq) * V[*newest - 1]  (skipped for *newest == 0);  *alpha = w . v.
+// With `partial` != null the kernel is also the split-j reduce (a6) of the apply that precedes it: w is first
+// formed as the sum over the splits of the pair kernel's partials [split][rhs * nc + c][npad] (fixed order,
+// fp arithmetic in T exactly as reduce_partials_kernel), for right-hand side `rhs` of `nrhs`.
 template <typename T>
 __global__ void __launch_bounds__(VEC_BLOCK) lanczos_alpha_kernel(T* __restrict__ w, const T* __restrict__ V, const int* __restrict__ newest,
                                                                   const double* beta_prev_sq, int64_t n, double* block_partials,
-                                                                  unsigned int* ticket, double* alpha)
+                                                                  unsigned int* ticket, double* alpha, const T* __restrict__ partial, int splits,
+                                                                  int nrhs, int rhs, int nc, int64_t npad)
 {
     const int m = *newest;
     const T* v = V + (size_t)m * n;
     const T* v_prev = m > 0 ? v - n : nullptr;
     const double bp = v_prev ? sqrt(*beta_prev_sq) : 0.0;
+    const int64_t n3 = n / (nc / 3);
+    const size_t stride = (size_t)nrhs * nc * npad;
     double s = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * VEC_BLOCK) {
+        if (partial) {
+            const int64_t rem = i < n3 ? i : i - n3;
+            const T* p = partial + (size_t)(rhs * nc + (i < n3 ? 0 : 3) + (int)(rem % 3)) * npad + rem / 3;
+            T acc = T(0);
+            for (int sidx = 0; sidx < splits; ++sidx) acc += p[(size_t)sidx * stride];
+            w[i] = acc;
+        }
         double wi = (double)w[i];
         if (v_prev) {
             wi = fma(-bp, (double)v_prev[i], wi);
@@ -201,11 +216,12 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_alpha_kernel(T* __restrict_
     block_reduce_to_scalar(s, block_partials, ticket, alpha);
 }
 
-// w -= *alpha * V[*newest];  *beta_sq = |w|^2;  host_ab[2(m+1)] = alpha, host_ab[2(m+1)+1] = beta^2 (iteration k = m+1)
+// w -= *alpha * V[*newest];  *beta_sq = |w|^2;  host_ab[2(m+1)] = alpha, host_ab[2(m+1)+1] = beta^2 (iteration k = m+1);
+// then, if `advance` is given, *advance += 1 (the index moves to the slot of v_{k+1}; the last vector of a lockstep group does it)
 template <typename T>
 __global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__ w, const T* __restrict__ V, const int* __restrict__ newest,
                                                                  const double* alpha, int64_t n, double* block_partials, unsigned int* ticket,
-                                                                 double* beta_sq, double* host_ab)
+                                                                 double* beta_sq, double* host_ab, int* advance)
 {
     const int m = *newest;
     const T* v = V + (size_t)m * n;
@@ -216,11 +232,11 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__
         w[i] = wi;
         s = fma((double)wi, (double)wi, s);
     }
-    block_reduce_to_scalar(s, block_partials, ticket, beta_sq, host_ab + 2 * (m + 1) + 1);
+    block_reduce_to_scalar(s, block_partials, ticket, beta_sq, host_ab + 2 * (m + 1) + 1, advance);
     if (blockIdx.x == 0 && threadIdx.x == 0) host_ab[2 * (m + 1)] = a;
 }
 
-// Gram column for the stopping test (a9): with c = *newest + 1 the column of the vector just written,
+// Gram column for the stopping test (a9): with c = *newest the column of the vector just written,
 // g[j] = V[j] . V[c], j = 0..c, stored to host_gram[c * ld + j].  Lanczos without
 // re-orthogonalisation loses orthogonality of V, so |y_k - y_{k-1}| = |z| |V_k delta| is evaluated as
 // sqrt(delta^T G delta) with the true Gram matrix G = V^T V instead of assuming G = I.
@@ -233,7 +249,7 @@ __global__ void __launch_bounds__(VEC_BLOCK) gram_column_kernel(const T* __restr
 {
     __shared__ double warp_part[VEC_BLOCK / 32];
     __shared__ bool is_last;
-    const int c = *newest + 1;
+    const int c = *newest;
     const int j = blockIdx.y;
     if (j > c) return;
     const int64_t lo_i = (int64_t)blockIdx.x * chunk, hi_i = min(lo_i + chunk, dof);
@@ -263,10 +279,6 @@ __global__ void __launch_bounds__(VEC_BLOCK) gram_column_kernel(const T* __restr
         if (threadIdx.x == 0) *ticket = 0u;
     }
 }
-
-// *newest += 1, as its own launch after the Gram column: blocks of that kernel that exit early may be
-// scheduled after its last active block has finished, so the index must not move while it runs.
-__global__ void lanczos_advance_kernel(int* newest) { *newest += 1; }
 
 // a10: y = scale * sum_{m<k} coef[m] V[m]  split into the linear (first 3N) and angular (last 3N)
 // outputs; accumulate != 0 adds to what is already there (lm_hydrodynamic_velocities).
