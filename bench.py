@@ -59,7 +59,7 @@ def work_per_pair(angular: bool, nrhs: int, f64: bool):
 # DRAM traffic of ONE pair-kernel launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
 # `ncu --set full` captures profiles/r1_c<N>_pair_kernel_ncu_full.md (same launch configuration); it is a
 # recorded profile value, not measured by this run.  Configs 4 and 5 are dominated by the j-split partials.
-NCU_DRAM_BYTES_PER_LAUNCH = {1: 64.512e3, 2: 610.816e3, 3: 3.165952e6, 4: 151.673088e6 + 634.764544e6, 5: 29.353984e6 + 115.338496e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {1: 64512 + 0, 2: 610816 + 0, 3: 3.1657e+06 + 0, 4: 1.88692e+08 + 6.81801e+08, 5: 2.77366e+07 + 1.14173e+08}
 
 
 def nominal_lanes(f64: bool) -> int:
