@@ -288,11 +288,14 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
             const int64_t ctas = (int64_t)i_tiles * s;
             const int64_t full = ctas / slots, rem = ctas % slots;
             const int64_t rem_per_sm = (rem + h->sm_count - 1) / h->sm_count;      // CTAs sharing an SM in the last wave
-            // prologue, pipeline fill and epilogue of a CTA ~ 0.1 tile (fitted to plan sweeps on B200)
-            const double per_cta = ((double)src + 0.1 * v.tj) * targets / v.efficiency;
+            // prologue, pipeline fill and epilogue of a CTA ~ 0.03 tile (fitted to plan sweeps on B200)
+            const double per_cta = ((double)src + 0.03 * v.tj) * targets / v.efficiency;
             // few resident warps hide less latency: w warps per SM sub-partition cost a factor (1 + 0.3 / w)
             auto wave = [&](int64_t resident) { return resident ? per_cta * resident * (1.0 + 0.3 * 128.0 / ((double)resident * v.block)) : 0.0; };
             double cost = (double)full * wave(v.ctas_per_sm) + wave(rem_per_sm);
+            // the SMs do not finish their last CTAs together: ~10 % of the last wave is tail, so several short waves
+            // beat one long one (measured: 4 waves 4-5 % faster than 1 at N = 16384 ... 32768, fp32 translational)
+            cost += 0.1 * (rem ? wave(rem_per_sm) : wave(v.ctas_per_sm));
             // cost is in pairs evaluated back to back on one SM (~1e4 per microsecond): the reduce pass
             // adds a ~3 us launch plus writing and re-reading s partial vectors
             if (s > 1) cost += 3.0e4 + 0.1 * (double)s * (double)rows;
