@@ -59,7 +59,7 @@ def work_per_pair(angular: bool, nrhs: int, f64: bool):
 # DRAM traffic of ONE pair-kernel launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
 # `ncu --set full` captures profiles/r1_c<N>_pair_kernel_ncu_full.md (same launch configuration); it is a
 # recorded profile value, not measured by this run.  Configs 4 and 5 are dominated by the j-split partials.
-NCU_DRAM_BYTES_PER_LAUNCH = {1: 64512 + 0, 2: 610816 + 0, 3: 3.1657e+06 + 0, 4: 1.88692e+08 + 6.81801e+08, 5: 2.77366e+07 + 1.14173e+08}
+NCU_DRAM_BYTES_PER_LAUNCH = {1: 64512 + 0, 2: 610816 + 0, 3: 3.16595e+06 + 3.64288e+06, 4: 1.964e+08 + 1.24312e+09, 5: 2.74117e+07 + 1.13751e+08}
 
 
 def nominal_lanes(f64: bool) -> int:
