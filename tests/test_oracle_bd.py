@@ -185,3 +185,14 @@ def test_b9_rfd_is_the_directional_derivative_and_averages_to_zero():
     mean, sem = acc / S, np.sqrt(sq / S) / math.sqrt(S)
     assert np.sqrt(sq / S).max() > 1e-3                 # the samples themselves are not small
     assert np.all(np.abs(mean) <= 5 * sem)
+
+
+def test_b10_steric_force_dimensional_scaling():
+    """eq. (13): U depends on r only through (d - r)/b, so scaling all lengths (positions, d, b) by lam at fixed
+    U0 scales every force by 1/lam, and the force is linear in U0."""
+    rng = np.random.default_rng(10)
+    x = rng.random((30, 3)) * 6.0
+    F = bd.steric_forces(x, 4.0, 0.1, 2.0)
+    for lam in (0.656e-6, 3.0, 1.0e5):
+        np.testing.assert_allclose(bd.steric_forces(lam * x, 4.0, 0.1 * lam, 2.0 * lam), F / lam, rtol=1e-10)
+    np.testing.assert_allclose(bd.steric_forces(x, 10.0, 0.1, 2.0), 2.5 * F, rtol=1e-13)

@@ -348,3 +348,23 @@ def test_golden_two_particle():
     np.testing.assert_allclose(W, g["W_far"], rtol=1e-12)
     U, _ = rpy.mdot(2.5 * g["pos"], g["F"])
     np.testing.assert_allclose(U, g["U_far_t"], rtol=1e-12)
+
+
+@pytest.mark.parametrize("lam,eta", [(0.37, 1.0), (2.5e-6, 1e-3), (1.0e4, 7.0)])
+def test_p11_dimensional_scaling(lam, eta):
+    """Dimensional analysis of Stokes flow: with every length (positions AND radius) scaled by lam and the
+    viscosity by eta, the four blocks of eq. (7) scale as  M_uF ~ 1/(eta lam),  M_uT = M_wF ~ 1/(eta lam^2),
+    M_wT ~ 1/(eta lam^3).  A wrong power of a anywhere in the ten scalar formulas (either branch) breaks it."""
+    rng = np.random.default_rng(11)
+    N = 14
+    x = rng.random((N, 3)) * 5.0                      # overlapping and separated pairs at a = 1
+    F, T = rng.standard_normal((N, 3)), rng.standard_normal((N, 3))
+    zero = np.zeros((N, 3))
+    UF, WF = rpy.mdot(x, F, zero, angular=True)        # a = eta = 1
+    UT, WT = rpy.mdot(x, zero, T, angular=True)
+    UF2, WF2 = rpy.mdot(lam * x, F, zero, a=lam, eta=eta, angular=True)
+    UT2, WT2 = rpy.mdot(lam * x, zero, T, a=lam, eta=eta, angular=True)
+    np.testing.assert_allclose(UF2, UF / (eta * lam), rtol=1e-12)
+    np.testing.assert_allclose(WF2, WF / (eta * lam ** 2), rtol=1e-12)
+    np.testing.assert_allclose(UT2, UT / (eta * lam ** 2), rtol=1e-12)
+    np.testing.assert_allclose(WT2, WT / (eta * lam ** 3), rtol=1e-12)
