@@ -553,3 +553,34 @@ def test_fp32_in_any_unit_system(lm, torch, a, eta):
     torch.cuda.synchronize()
     assert rel(Fs.cpu().numpy(), bd.steric_forces(pos, U0, b, 2 * a)) <= 2e-5
     s.close()
+
+
+def test_seeded_sweep_of_sizes_and_shapes(lm, torch):
+    """40 seeded random (N, precision, angular, nrhs, density) combinations: ragged tails, every launch shape and
+    split count the chooser produces in this range, far-only and overlap-heavy geometries."""
+    rng = np.random.default_rng(2024)
+    for case_id in range(40):
+        N = int(rng.choice([rng.integers(1, 70), rng.integers(70, 1200), rng.integers(1200, 9000)]))
+        prec = "f32" if rng.random() < 0.5 else "f64"
+        angular = bool(rng.random() < 0.5)
+        nrhs = int(rng.choice([1, 2, 3, 4] if not angular else [1, 2, 3]))
+        side = float(N ** (1 / 3) * rng.choice([0.8, 2.0, 6.0]))     # heavy overlap ... dilute
+        dt = workloads.np_dtype(prec)
+        pos = (rng.random((N, 3)) * side).astype(dt)
+        F = rng.standard_normal((nrhs, N, 3)).astype(dt)
+        T = rng.standard_normal((nrhs, N, 3)).astype(dt) if angular else None
+        s = lm.Solver(prec, N, 1.0, 1.0, angular)
+        s.set_positions(dev(torch, pos))
+        U = torch.empty(nrhs * 3 * N, dtype=s.torch_dtype, device="cuda")
+        W = torch.empty(nrhs * 3 * N, dtype=s.torch_dtype, device="cuda") if angular else None
+        s.mdot_batch(nrhs, dev(torch, F).reshape(-1), None if T is None else dev(torch, T).reshape(-1), U, W)
+        torch.cuda.synchronize()
+        U = U.cpu().numpy().reshape(nrhs, N, 3)
+        W = W.cpu().numpy().reshape(nrhs, N, 3) if angular else None
+        for q in range(nrhs):
+            Uo, Wo = rpy.mdot(pos, F[q], None if T is None else T[q], angular=angular)
+            tag = (case_id, N, prec, angular, nrhs, q, side)
+            assert rel(U[q], Uo) <= TOL[prec], tag
+            if angular:
+                assert rel(W[q], Wo) <= TOL[prec], tag
+        s.close()
