@@ -584,3 +584,30 @@ def test_seeded_sweep_of_sizes_and_shapes(lm, torch):
             if angular:
                 assert rel(W[q], Wo) <= TOL[prec], tag
         s.close()
+
+
+def test_handles_release_their_device_memory(lm, torch):
+    """lm_destroy frees everything a handle allocated (packed arrays, Lanczos basis, graphs, staging, BD buffers)."""
+    N = 4000
+    c = workloads.random_case(N, 40.0, 5, "f32", True, with_noise=True)
+    def cycle():
+        s = lm.Solver("f32", N, 1.0, 1.0, True)
+        X = dev(torch, c["pos"]).reshape(-1).clone()
+        s.set_positions(X)
+        U = torch.empty(3 * N, dtype=torch.float32, device="cuda"); W = torch.empty_like(U)
+        for _ in range(3):
+            s.mdot(dev(torch, c["forces"]), dev(torch, c["torques"]), U, W)
+        s.sqrt_mdot_w(dev(torch, c["noise"]), 1e-2, U, W)
+        s.bd_step(X, dev(torch, c["forces"]).reshape(-1), None, dev(torch, c["noise"]), 1e-3, 1.0, 4.0, 0.1, 1e-2)
+        s.set_positions(X)                                   # lm_bd_step leaves the handle's packed positions stale
+        s.thermal_drift_rfd(dev(torch, c["noise"][: 3 * N]), 1e-2, U, W)
+        s.close()
+        del X, U, W
+    cycle()
+    torch.cuda.synchronize(); torch.cuda.empty_cache()
+    free0, _ = torch.cuda.mem_get_info()
+    for _ in range(20):
+        cycle()
+    torch.cuda.synchronize(); torch.cuda.empty_cache()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free0 - free1 < 8 * 2 ** 20, (free0, free1)        # < 8 MiB drift over 20 handles (one handle holds ~60 MiB)
