@@ -147,8 +147,8 @@ int lm_hydrodynamic_velocities_host(lm_solver* h, const void* forces, const void
  * lm_create / lm_bd_reset has no history and is forward Euler.  pos: 3N, read and overwritten.
  * noise: W^n, dof values as for lm_sqrt_mdot_w, or NULL (or kT == 0) for a deterministic step; tol:
  * Lanczos tolerance.  The handle keeps M^n F^n for the next step.  Synchronises the stream when noise
- * is given.  After the call the handle's packed positions are X^n (stale): call lm_set_positions
- * before lm_mdot etc.  Returns LM_E_NOCONV if Lanczos hit max_iter (the step is still taken). */
+ * is given.  After the call the handle's positions are the new X^{n+1} (as if lm_set_positions(pos) had
+ * been called).  Returns LM_E_NOCONV if Lanczos hit max_iter (the step is still taken). */
 int lm_steric_forces(lm_solver* h, double U0, double b, const void* ext_forces, void* forces_out, void* stream);
 int lm_bd_step(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise,
                double dt, double kT, double U0, double b, double tol, void* stream);

@@ -118,7 +118,7 @@ int bd_step_device(lm_solver* h, T* pos, const T* ext_f, const T* ext_t, const T
     h->n_aux++;
     LM_CUDA(h, cudaGetLastError());
     h->bd_have_prev = true;
-    h->have_pos = false;       // the packed copy now holds X^n, not the caller's X^{n+1}
+    if ((rc = set_positions_t<T>(h, pos, st)) != LM_OK) return rc;      // the handle follows the particles: packed copy = X^{n+1}
     return rc_noise;
 }
 

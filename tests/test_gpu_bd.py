@@ -266,3 +266,19 @@ def test_thermal_drift_rfd_matches_oracle_and_default_is_zero(lm, torch, prec, a
         s.thermal_drift_rfd(dev(torch, W), 0.0, lin, ang)
     assert e.value.code == lm.LM_E_INVALID
     s.close()
+
+
+def test_bd_step_leaves_the_handle_at_the_new_positions(lm, torch):
+    from oracle import rpy
+    c = case(400, 11.0, 24, "f64")
+    N = 400
+    s = lm.Solver("f64", N)
+    X = dev(torch, c["pos"]).reshape(-1).clone()
+    F = dev(torch, c["forces"]).reshape(-1)
+    s.bd_step(X, F, None, None, 1e-2, 0.0, 4.0, 0.1, 1e-3)
+    U = torch.empty(3 * N, dtype=torch.float64, device="cuda")
+    s.mdot(F, None, U)                                    # no lm_set_positions in between
+    torch.cuda.synchronize()
+    Uo, _ = rpy.mdot(X.cpu().numpy().reshape(N, 3), c["forces"])
+    assert rel(U.cpu().numpy(), Uo) <= 1e-12
+    s.close()

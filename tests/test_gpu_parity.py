@@ -599,7 +599,6 @@ def test_handles_release_their_device_memory(lm, torch):
             s.mdot(dev(torch, c["forces"]), dev(torch, c["torques"]), U, W)
         s.sqrt_mdot_w(dev(torch, c["noise"]), 1e-2, U, W)
         s.bd_step(X, dev(torch, c["forces"]).reshape(-1), None, dev(torch, c["noise"]), 1e-3, 1.0, 4.0, 0.1, 1e-2)
-        s.set_positions(X)                                   # lm_bd_step leaves the handle's packed positions stale
         s.thermal_drift_rfd(dev(torch, c["noise"][: 3 * N]), 1e-2, U, W)
         s.close()
         del X, U, W
