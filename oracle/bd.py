@@ -21,7 +21,7 @@ thermal_drift_rfd  eq. (11), one realisation (no average):
                    (the mobility depends on positions only); rows = linear (and angular) velocities.
                    For open boundaries its mean over W is the divergence of M, which is zero.
 
-Pins: tests/test_oracle_bd.py.  No function here is "parity unpinned".
+Pins: tests/test_oracle_bd.py (B1-B11; B11 pins the ``rows=`` branch of steric_forces).  No function here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -44,6 +44,8 @@ def steric_forces(pos, U0: float, b: float, d: float, rows=None) -> np.ndarray:
     x = np.asarray(pos, dtype=np.float64).reshape(-1, 3)
     N = x.shape[0]
     targets = range(N) if rows is None else [int(i) for i in rows]
+    if any(i < 0 or i >= N for i in targets):      # as rpy.mdot_rows: no silent wrap-around of a negative index
+        raise ValueError("row index out of range")
     F = np.zeros((len(targets), 3))
     for out, i in enumerate(targets):
         rv = x[i] - x                              # r_vec = x_i - x_j, points from j to i

@@ -9,6 +9,7 @@ mdot, mdot_rows   O2: U = M.[F;T], eq. (7), plain double loop in 
 dense             eq. (7) assembled densely (PAPER.md:196-198 uses the full matrix in its tests)
 dense_sqrt_mdot_w O3: principal symmetric square root by eigendecomposition
 lanczos_sqrt_mdot_w  O4: Lanczos iteration of ref. [35], step by step
+step_error_estimate  the stopping quantity of O4 (reading S3: the paper states no rule)
 tridiag_sqrt_e1   the small T_k^{1/2} e_1 problem inside O4
 
 Pins: tests/test_oracle_pins.py (mdot family), tests/test_oracle_sqrt.py (square roots).
@@ -156,21 +157,58 @@ def tridiag_sqrt_e1(alpha, beta) -> np.ndarray:
     return S @ (np.sqrt(lam) * S[0, :])
 
 
+def step_error_estimate(steps, window: int = 10, rho_max: float = 0.98) -> float:
+    """Error estimate of the newest Lanczos iterate from the relative steps s_2..s_k (reading S3).
+
+    ``steps`` = [s_2, ..., s_k], s_i = |y_i - y_{i-1}| / |y_{i-1}|, k >= 3.  The paper fixes no stopping rule
+    (PAPER.md:147); the rule of ref. [35] takes s_k itself as the error, which under-states it by the factor
+    rho/(1 - rho) when the steps shrink slowly (ratio rho per iteration): the iterate still has to travel
+    s_{k+1} + s_{k+2} + ... ~ s_k (rho + rho^2 + ...) = s_k rho / (1 - rho).  Here
+
+        m   = max(1, min(window, (k - 1) // 2))                  trailing window, in steps
+        rho = min( (sum of the last m steps / sum of the m steps before them)^(1/m), rho_max )
+        e_k = max(s_k, s_{k-1}) * max(1, rho / (1 - rho))
+
+    max(s_k, s_{k-1}): one small step is no evidence (the steps dip whenever a new Ritz value appears);
+    max(1, .): never less than the step rule of ref. [35]; rho_max bounds the amplification (x49)."""
+    s = [float(v) for v in steps]
+    n = len(s)                                   # n = k - 1 steps
+    if n < 2:
+        raise ValueError("needs at least the two steps s_2, s_3")
+    m = max(1, min(int(window), n // 2))
+    recent = sum(s[n - m:])
+    before = sum(s[n - 2 * m:n - m])
+    if before > 0.0:
+        rho = min((recent / before) ** (1.0 / m), rho_max)
+    else:
+        rho = 0.0                                # the earlier steps were exactly zero: nothing left to extrapolate
+    return max(s[-1], s[-2]) * max(1.0, rho / (1.0 - rho))
+
+
 def lanczos_sqrt_mdot_w(pos, noise, tol: float, a: float = 1.0, eta: float = 1.0, angular: bool = False,
-                        max_iter: int = 100, apply=None):
+                        max_iter: int = 100, apply=None, rule: str = "estimate", history: dict | None = None):
     """O4: Lanczos approximation of M^{1/2} z (ref. [35]), in the order written
     in SURVEY.md sec. 8(c) O4.  No re-orthogonalisation.  Returns (y, iterations, converged).
 
         v_1 = z/|z|, beta_0 = 0
         k = 1,2,..:  w = M v_k - beta_{k-1} v_{k-1};  alpha_k = w.v_k;  w -= alpha_k v_k;
                      beta_k = |w|;  v_{k+1} = w / beta_k
-                     c_k = T_k^{1/2} e_1;  y_k = |z| V_k c_k
-                     stop when k >= 2 and |y_k - y_{k-1}| / |y_{k-1}| <= tol  (S3), or beta_k ~ 0.
-    ``apply`` overrides the operator (default: the O(N^2) oracle apply)."""
+                     c_k = T_k^{1/2} e_1;  y_k = |z| V_k c_k;  s_k = |y_k - y_{k-1}| / |y_{k-1}|
+                     stop (reading S3; the paper states no rule):
+                       rule "estimate" (default): k >= 3 and step_error_estimate(s_2..s_k) <= tol
+                       rule "step" (ref. [35] as SURVEY O4 writes it): k >= 2 and s_k <= tol
+                     or beta_k ~ 0 (invariant subspace: y_k is exact).
+    ``apply`` overrides the operator (default: the O(N^2) oracle apply).  ``history``, if given, receives
+    "steps" = [s_2..s_k] and "estimates" = [e_3..e_k] (test diagnostics)."""
+    if rule not in ("estimate", "step"):
+        raise ValueError("rule must be 'estimate' or 'step'")
     z = np.asarray(noise, dtype=np.float64).reshape(-1)
     if apply is None:
         def apply(v):
             return apply_vec(pos, v, a, eta, angular)
+    steps, estimates = [], []
+    if history is not None:
+        history["steps"], history["estimates"] = steps, estimates
     znorm = np.linalg.norm(z)
     if znorm == 0.0:
         return np.zeros_like(z), 0, True
@@ -188,8 +226,14 @@ def lanczos_sqrt_mdot_w(pos, noise, tol: float, a: float = 1.0, eta: float = 1.0
         c = tridiag_sqrt_e1(alphas, betas)
         y = znorm * (np.stack(V, axis=1) @ c)
         if y_prev is not None:
-            if np.linalg.norm(y - y_prev) <= tol * np.linalg.norm(y_prev):
-                return y, k, True
+            steps.append(float(np.linalg.norm(y - y_prev) / np.linalg.norm(y_prev)))
+            if rule == "step":
+                if steps[-1] <= tol:
+                    return y, k, True
+            elif k >= 3:
+                estimates.append(step_error_estimate(steps))
+                if estimates[-1] <= tol:
+                    return y, k, True
         if beta <= 1e-14 * abs(alpha):          # invariant subspace: y_k is exact
             return y, k, True
         betas.append(beta)

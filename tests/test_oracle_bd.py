@@ -196,3 +196,31 @@ def test_b10_steric_force_dimensional_scaling():
     for lam in (0.656e-6, 3.0, 1.0e5):
         np.testing.assert_allclose(bd.steric_forces(lam * x, 4.0, 0.1 * lam, 2.0 * lam), F / lam, rtol=1e-10)
     np.testing.assert_allclose(bd.steric_forces(x, 10.0, 0.1, 2.0), 2.5 * F, rtol=1e-13)
+
+
+def test_b11_row_sampled_steric_forces_equal_the_full_call():
+    """``rows=`` (the row-sampled oracle used at N = 131072 by the GPU tests) returns exactly the listed rows of the
+    full call -- rows are independent --, in the order listed, duplicates included; an index outside [0, N) is an
+    error, never a silent wrap-around of a negative index.  Against the energy gradient too (B2's route), so the
+    sampled path is pinned by something other than the full path."""
+    rng = np.random.default_rng(11)
+    N, U0, b, d = 60, 4.0, 0.1, 2.0
+    x = rng.random((N, 3)) * 5.0
+    full = bd.steric_forces(x, U0, b, d)
+    rows = np.array([0, 17, 17, 59, 3, 0])
+    part = bd.steric_forces(x, U0, b, d, rows=rows)
+    assert part.shape == (6, 3)
+    assert np.array_equal(part, full[rows])
+    assert bd.steric_forces(x, U0, b, d, rows=[]).shape == (0, 3)
+    assert np.array_equal(bd.steric_forces(x, U0, b, d, rows=range(N)), full)
+    for bad in ([N], [-1], [0, N + 5]):
+        with pytest.raises((IndexError, ValueError)):
+            bd.steric_forces(x, U0, b, d, rows=bad)
+    h = 1e-6
+    for out, i in enumerate(rows[:4]):
+        for k in range(3):
+            xp, xm = x.copy(), x.copy()
+            xp[i, k] += h
+            xm[i, k] -= h
+            fd = -(energy(xp, U0, b, d) - energy(xm, U0, b, d)) / (2 * h)
+            assert part[out, k] == pytest.approx(fd, rel=2e-7, abs=1e-7)
