@@ -18,8 +18,13 @@ e2e     = same metric through the *_host C-ABI calls: pinned host buffers, H2D a
 roofline= the pair kernel against the FP32/FP64 FMA-pipe ("alu") roofline, DESIGN.md sec. 7.
 cpu_baseline = the CPU fp64 oracle (oracle/, untuned) on the box's host cores, bounded row sample.
 
-Multi-GPU (torchrun): the path does not shard in this build ("replicas only"):
-every rank runs an independent replica (seed + rank); scaling = "weak".
+configs = the other four BASELINE.json configs measured in the same run (a few steps each; single GPU, default
+          headline only): ms per launch, roofline fraction, e2e -- so that every number of BASELINE.md sec. 4 is on
+          the driver's record, not only the headline.
+
+Multi-GPU (torchrun): "replicas only" by default: every rank runs an independent replica
+(seed + 1000 rank), scaling = "weak"; `--parallelism sharded` row-shards ONE problem over the ranks (lm_dist_init:
+all-gather of the row blocks inside every apply), scaling = "strong".
 """
 from __future__ import annotations
 
@@ -56,10 +61,23 @@ def work_per_pair(angular: bool, nrhs: int, f64: bool):
     return instr, flops
 
 
-# DRAM traffic of ONE pair-kernel launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
-# `ncu --set full` captures profiles/r1_c<N>_pair_kernel_ncu_full.md (same launch configuration); it is a
-# recorded profile value, not measured by this run.  Configs 4 and 5 are dominated by the j-split partials.
-NCU_DRAM_BYTES_PER_LAUNCH = {1: 64512 + 0, 2: 610816 + 0, 3: 3.16595e+06 + 3.64288e+06, 4: 1.964e+08 + 1.24312e+09, 5: 2.74117e+07 + 1.13751e+08}
+def profile_traffic(config: int):
+    """DRAM bytes of ONE pair-kernel launch (dram__bytes_read.sum + dram__bytes_write.sum) read at run time from the
+    committed `ncu --set full` summary of the same launch configuration, profiles/r<round>_c<config>_pair_kernel_ncu_full.md
+    (newest round present).  A recorded profile value -- ncu cannot run inside a timed benchmark.  (bytes, path) or (None, None)."""
+    import glob
+    import re
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_c{config}_pair_kernel_ncu_full.md")), reverse=True):
+        text = open(path).read()
+        got = {}
+        for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            m = re.search(r"\|\s*" + re.escape(key) + r"\s*\|\s*(\w+)\s*\|\s*([0-9.eE+-]+)\s*\|", text)
+            if m and m.group(1) in unit:
+                got[key] = float(m.group(2)) * unit[m.group(1)]
+        if len(got) == 2:
+            return sum(got.values()), os.path.relpath(path, ROOT)
+    return None, None
 
 
 def nominal_lanes(f64: bool) -> int:
@@ -156,7 +174,7 @@ def run_reference(args, data):
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": config_dict(cfg, data["N"], None),
+        "data": "synthetic", "config": config_dict(cfg, data["N"]),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": info["cores"], "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -164,18 +182,188 @@ def run_reference(args, data):
     print(json.dumps(line))
 
 
-def config_dict(cfg, N, extra):
+def config_dict(cfg, N):
+    """Names the workload; identical for the CUDA arm and the reference arm (run-dependent facts go to `details`)."""
     d = {"workload": f"BASELINE.json configs[{cfg.index - 1}] ({cfg.name})", "op": cfg.op, "N": int(N), "precision": cfg.precision,
          "include_angular": bool(cfg.angular), "nrhs": int(cfg.nrhs), "geometry": f"{cfg.geometry}={cfg.geom_param:g}", "seed": int(cfg.seed),
          "a": cfg.a, "eta": cfg.eta}
     if cfg.tol:
         d["lanczos_tol"] = cfg.tol
-    if extra:
-        d.update(extra)
+    d["l2"] = "256 MiB device memset between steps, outside the event brackets (CUDA arm)"
     return d
 
 
 # ---------------------------------------------------------------- the CUDA arm
+class Arm:
+    """One config on this rank's GPU: device-resident and pinned-host inputs, the step functions, the timers."""
+
+    def __init__(self, lm, torch, dist, index, N_override, rank, world, sharded):
+        from paper_2510_02135_b200 import multi, workloads
+        self.lm, self.torch, self.dist, self.world = lm, torch, dist, world
+        cfg = self.cfg = workloads.CONFIGS[index]
+        # replicas: every rank its own problem (seed + 1000 rank); sharded: the same problem on every rank
+        self.data = data = workloads.generate(index, N_override, seed=cfg.seed if sharded else multi.replica_seed(cfg.seed, rank))
+        N = self.N = data["N"]
+        self.f64 = cfg.precision == "f64"
+        tdt = torch.float64 if self.f64 else torch.float32
+        self.stream = torch.cuda.current_stream()
+        self.solver = lm.Solver(cfg.precision, N, cfg.eta, cfg.a, cfg.angular)
+        if sharded:
+            multi.init_sharded(self.solver)
+
+        def pinned(x):
+            if x is None:
+                return None
+            t = torch.empty(x.shape, dtype=tdt, pin_memory=True)
+            t.numpy()[...] = x
+            return t
+
+        self.host = {k: pinned(data[k]) for k in ("pos", "forces", "torques", "noise")}
+        self.dev = {k: (None if v is None else v.cuda()) for k, v in self.host.items()}
+        nout = cfg.nrhs * 3 * N
+        self.d_lin = torch.empty(nout, dtype=tdt, device="cuda")
+        self.d_ang = torch.empty(nout, dtype=tdt, device="cuda") if cfg.angular else None
+        self.h_lin = torch.empty(nout, dtype=tdt, pin_memory=True)
+        self.h_ang = torch.empty(nout, dtype=tdt, pin_memory=True) if cfg.angular else None
+        self.h2d = sum(v.numel() * v.element_size() for v in self.host.values() if v is not None)
+        self.d2h = self.h_lin.numel() * self.h_lin.element_size() * (2 if cfg.angular else 1)
+
+    def close(self):
+        self.solver.close()
+        self.host = self.dev = self.d_lin = self.d_ang = self.h_lin = self.h_ang = None
+
+    def step_device(self):
+        cfg, s, dev = self.cfg, self.solver, self.dev
+        s.set_positions(dev["pos"])
+        if cfg.op == "sqrt+mdot":
+            s.hydrodynamic_velocities(dev["forces"], dev["torques"], dev["noise"], 1.0, cfg.tol, self.d_lin, self.d_ang)
+        elif cfg.op == "mdot_batch":
+            s.mdot_batch(cfg.nrhs, dev["forces"], dev["torques"], self.d_lin, self.d_ang)
+        else:
+            s.mdot(dev["forces"], dev["torques"], self.d_lin, self.d_ang)
+
+    def step_host(self):
+        cfg, s = self.cfg, self.solver
+        n = lambda t: None if t is None else t.numpy()
+        h = self.host
+        s.set_positions_host(n(h["pos"]))
+        if cfg.op == "sqrt+mdot":
+            s.hydrodynamic_velocities_host(n(h["forces"]), n(h["torques"]), n(h["noise"]), 1.0, cfg.tol, n(self.h_lin), n(self.h_ang))
+        elif cfg.op == "mdot_batch":
+            s.mdot_batch_host(cfg.nrhs, n(h["forces"]), n(h["torques"]), n(self.h_lin), n(self.h_ang))
+        else:
+            s.mdot_host(n(h["forces"]), n(h["torques"]), n(self.h_lin), n(self.h_ang))
+
+    def barrier(self):
+        self.torch.cuda.synchronize()
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def timed(self, step_fn, K, flush):
+        """K steps; each bracketed by CUDA events on the launching stream; the L2 flush between steps
+        sits outside the brackets.  Returns (sum of step ms, wall t0, wall t1)."""
+        torch = self.torch
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+        self.barrier()
+        t0 = time.time()
+        for e0, e1 in evs:
+            flush.zero_()
+            e0.record(self.stream)
+            step_fn()
+            e1.record(self.stream)
+        self.barrier()
+        t1 = time.time()
+        return sum(e0.elapsed_time(e1) for e0, e1 in evs), t0, t1
+
+    def measure(self, steps, warmup, flush, do_e2e, sampler=None):
+        """value pass (profiling OFF: the code path a user gets, CUDA-graph replay included), a short profiled pass
+        for the pair kernel's own launch time, and the e2e pass through the *_host calls."""
+        s, torch = self.solver, self.torch
+        for _ in range(warmup):
+            self.step_device()
+        torch.cuda.synchronize()
+        if sampler is not None:
+            sampler.start()
+            time.sleep(0.3)
+        s.reset_stats()
+        ms_total, w0, w1 = self.timed(self.step_device, steps, flush)
+        stats = s.get_stats()
+        clocks = sampler.stop(w0, w1) if sampler is not None else None
+        iters = s.last_iterations() if self.cfg.op == "sqrt+mdot" else None
+        hist = s.lanczos_history() if self.cfg.op == "sqrt+mdot" else None
+        # the pair kernel alone: every launch bracketed by CUDA events on its stream (direct launches, no graph)
+        s.set_profiling(True)
+        s.reset_stats()
+        psteps = max(1, min(steps, 3))
+        self.timed(self.step_device, psteps, flush)
+        pstats = s.get_stats()
+        s.set_profiling(False)
+        out = dict(ms_total=ms_total, stats=stats, pstats=pstats, clocks=clocks, iters=iters, hist=hist, e2e_ms=None, e2e_stats=None)
+        if do_e2e:
+            for _ in range(2):
+                self.step_host()
+            s.reset_stats()
+            out["e2e_ms"], _, _ = self.timed(self.step_host, steps, flush)
+            out["e2e_stats"] = s.get_stats()
+        return out
+
+
+def roofline_of(arm, m, sm_max_mhz, sms, probe_lane_ops, config_index, N_override):
+    cfg = arm.cfg
+    nrhs_launch = cfg.nrhs if cfg.op == "mdot_batch" else 1
+    instr, flops = work_per_pair(cfg.angular, nrhs_launch, arm.f64)
+    ps = m["pstats"]
+    launches = max(1, ps["pair_kernel_launches"])
+    pair_ms_avg = ps["pair_kernel_ms"] / launches
+    # lane-ops of all profiled launches (the first Lanczos apply of a config-3 step is a 2-RHS launch: 10 more per pair)
+    extra = 0.0
+    if cfg.op == "sqrt+mdot":
+        steps_prof = max(1, round(launches / max(1, (m["iters"] or 1))))
+        extra = 10.0 * steps_prof * float(arm.N) * arm.N
+    pairs_per_launch = ps["pairs"] / launches
+    lane_ops = instr * ps["pairs"] + extra
+    peak = sms * nominal_lanes(arm.f64) * sm_max_mhz * 1e6 / 1e12                 # T lane-ops/s at max clock
+    achieved = lane_ops / (ps["pair_kernel_ms"] * 1e-3) / 1e12
+    traffic, traffic_src = profile_traffic(config_index) if N_override is None else (None, None)
+    r = {
+        "bound": "alu", "kernel": f"rpy_pair_kernel<{cfg.precision}, nrhs={nrhs_launch}, angular={int(cfg.angular)}>",
+        "achieved": achieved, "peak": peak, "unit": "T FP-pipe lane-ops/s", "frac": achieved / peak,
+        "traffic": traffic, "traffic_unit": "bytes per launch: dram__bytes_read.sum + dram__bytes_write.sum of the committed ncu capture",
+        "traffic_source": traffic_src,
+        "algorithmic_bytes_per_launch": int(((arm.N + 31) // 32 * 32) * (3 + (6 if cfg.angular else 3) * nrhs_launch) * (8 if arm.f64 else 4)
+                                            + 3 * arm.N * (2 if cfg.angular else 1) * nrhs_launch * (8 if arm.f64 else 4)),
+        "peak_source": f"derived: {sms} SMs x {nominal_lanes(arm.f64)} lanes x {sm_max_mhz:.0f} MHz (clocks.max.sm); MEASURED_PEAKS.json has no ALU entry",
+        "lane_ops_per_pair": instr, "flops_per_pair": flops, "pairs_per_launch": pairs_per_launch,
+        "launch_ms_avg": pair_ms_avg, "launches_timed": ps["pair_kernel_launches"],
+        "flop_frac": flops * ps["pairs"] / (ps["pair_kernel_ms"] * 1e-3) / 1e12 / (2 * peak),
+        "kernel_gpairs_per_s": pairs_per_launch / (pair_ms_avg * 1e-3) / 1e9,
+    }
+    if probe_lane_ops:
+        r["measured_fma_peak"] = probe_lane_ops / 1e12
+        r["frac_of_measured_fma_peak"] = achieved / (probe_lane_ops / 1e12)
+    if m["clocks"] and m["clocks"].get("sm_mhz"):
+        r["frac_at_observed_clock"] = achieved / (sms * nominal_lanes(arm.f64) * m["clocks"]["sm_mhz"] * 1e6 / 1e12)
+    return r
+
+
+def lanczos_true_error(lm, torch, arm, y_f32):
+    """Relative error of the timed step's noise part against a 300-step fp64 run of the same recurrence (outside the
+    timed region): what `tol` delivered at this config (S3/S4)."""
+    d, N = arm.data, arm.N
+    s64 = lm.Solver("f64", N, arm.cfg.eta, arm.cfg.a, arm.cfg.angular)
+    s64.set_positions(torch.from_numpy(d["pos"].astype(np.float64)).cuda())
+    s64.set_max_iter(300)
+    yref = torch.empty(3 * N, dtype=torch.float64, device="cuda")
+    try:
+        s64.sqrt_mdot_w(torch.from_numpy(d["noise"].astype(np.float64)).cuda(), 1e-9, yref, None, allow_noconv=True)
+    finally:
+        pass
+    err = float((y_f32.double() - yref).norm() / yref.norm())
+    s64.close()
+    return err
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -186,6 +374,8 @@ def main():
     ap.add_argument("--N", type=int, default=None, help="override N (measurement sweeps only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the sub-records of the other four configs")
+    ap.add_argument("--lanczos-rule", default="estimate", choices=["estimate", "step"], help="stopping rule (DESIGN.md reading S3)")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "sharded"],
                     help="N > 1 ranks: independent replicas (default, weak scaling) or ONE problem row-sharded over the ranks "
                          "(lm_dist_init: all-gather of the row blocks inside every apply, strong scaling)")
@@ -216,126 +406,27 @@ def main():
         args.warmup = 3
 
     import paper_2510_02135_b200 as lm
+    from paper_2510_02135_b200 import multi, probe
 
-    from paper_2510_02135_b200 import multi
-    cfg = workloads.CONFIGS[args.config]
     sharded = args.parallelism == "sharded" and world > 1
-    # replicas: every rank its own problem (seed + 1000 rank); sharded: the same problem on every rank
-    data = workloads.generate(args.config, args.N, seed=cfg.seed if sharded else multi.replica_seed(cfg.seed, rank))
-    N = data["N"]
-    f64 = cfg.precision == "f64"
-    tdt = torch.float64 if f64 else torch.float32
-    dof = (6 if cfg.angular else 3) * N
-    stream = torch.cuda.current_stream()
-
-    solver = lm.Solver(cfg.precision, N, cfg.eta, cfg.a, cfg.angular)
-    if sharded:
-        multi.init_sharded(solver)
-
-    # ---- device-resident inputs (value) and pinned host inputs (e2e)
-    def pinned(x):
-        if x is None:
-            return None
-        t = torch.empty(x.shape, dtype=tdt, pin_memory=True)
-        t.numpy()[...] = x
-        return t
-
-    host = {k: pinned(data[k]) for k in ("pos", "forces", "torques", "noise")}
-    dev = {k: (None if v is None else v.cuda()) for k, v in host.items()}
-    nout = cfg.nrhs * 3 * N
-    d_lin = torch.empty(nout, dtype=tdt, device="cuda")
-    d_ang = torch.empty(nout, dtype=tdt, device="cuda") if cfg.angular else None
-    h_lin = torch.empty(nout, dtype=tdt, pin_memory=True)
-    h_ang = torch.empty(nout, dtype=tdt, pin_memory=True) if cfg.angular else None
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    arm = Arm(lm, torch, dist, args.config, args.N, rank, world, sharded)
+    cfg, N = arm.cfg, arm.N
+    if cfg.op == "sqrt+mdot":
+        arm.solver.set_option(lm.LM_OPT_LANCZOS_RULE, lm.LM_RULE_STEP if args.lanczos_rule == "step" else lm.LM_RULE_ESTIMATE)
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    m = arm.measure(args.steps, args.warmup, flush, not args.no_e2e, sampler)
 
-    def step_device():
-        solver.set_positions(dev["pos"])
-        if cfg.op == "sqrt+mdot":
-            solver.hydrodynamic_velocities(dev["forces"], dev["torques"], dev["noise"], 1.0, cfg.tol, d_lin, d_ang)
-        elif cfg.op == "mdot_batch":
-            solver.mdot_batch(cfg.nrhs, dev["forces"], dev["torques"], d_lin, d_ang)
-        else:
-            solver.mdot(dev["forces"], dev["torques"], d_lin, d_ang)
-
-    np_or_none = lambda t: None if t is None else t.numpy()
-
-    def step_host():
-        solver.set_positions_host(np_or_none(host["pos"]))
-        if cfg.op == "sqrt+mdot":
-            solver.hydrodynamic_velocities_host(np_or_none(host["forces"]), np_or_none(host["torques"]), np_or_none(host["noise"]), 1.0, cfg.tol,
-                                                np_or_none(h_lin), np_or_none(h_ang))
-        elif cfg.op == "mdot_batch":
-            solver.mdot_batch_host(cfg.nrhs, np_or_none(host["forces"]), np_or_none(host["torques"]), np_or_none(h_lin), np_or_none(h_ang))
-        else:
-            solver.mdot_host(np_or_none(host["forces"]), np_or_none(host["torques"]), np_or_none(h_lin), np_or_none(h_ang))
-
-    h2d = sum(v.numel() * v.element_size() for v in host.values() if v is not None)
-    d2h = h_lin.numel() * h_lin.element_size() * (2 if cfg.angular else 1)
-
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def timed(step_fn, K):
-        """K steps; each bracketed by CUDA events on the launching stream; the L2 flush between steps
-        sits outside the brackets.  Returns (sum of step ms, wall t0, wall t1)."""
-        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
-        barrier()
-        t0 = time.time()
-        for e0, e1 in evs:
-            flush.zero_()
-            e0.record(stream)
-            step_fn()
-            e1.record(stream)
-        barrier()
-        t1 = time.time()
-        return sum(e0.elapsed_time(e1) for e0, e1 in evs), t0, t1
-
-    for _ in range(args.warmup):
-        step_device()
-    torch.cuda.synchronize()
-
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
-        sampler.start()
-        time.sleep(0.3)
-    solver.set_profiling(True)
-    solver.reset_stats()
-    ms_total, w0, w1 = timed(step_device, args.steps)
-    stats = solver.get_stats()
-    solver.set_profiling(False)
-    clocks = sampler.stop(w0, w1) if rank == 0 else None
-    iters = solver.last_iterations() if cfg.op == "sqrt+mdot" else None
-
-    e2e_ms = None
-    if not args.no_e2e:
-        for _ in range(2):
-            step_host()
-        solver.reset_stats()
-        e2e_ms, _, _ = timed(step_host, args.steps)
-        e2e_stats = solver.get_stats()
-
-    # ---- max over ranks of the device time, sum over ranks of the pairs (replicas only)
-    ms_total, pairs_all = multi.aggregate_over_ranks(ms_total, stats["pairs"], device="cuda")
-    e2e_pairs_all = 0.0
-    if e2e_ms is not None:
-        e2e_ms, e2e_pairs_all = multi.aggregate_over_ranks(e2e_ms, e2e_stats["pairs"], device="cuda")
-
+    # ---- max over ranks of the device time, sum over ranks of the pairs
+    ms_total, pairs_all = multi.aggregate_over_ranks(m["ms_total"], m["stats"]["pairs"], device="cuda")
+    e2e_ms, e2e_pairs_all = None, 0.0
+    if m["e2e_ms"] is not None:
+        e2e_ms, e2e_pairs_all = multi.aggregate_over_ranks(m["e2e_ms"], m["e2e_stats"]["pairs"], device="cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    value = pairs_all / (ms_total * 1e-3) / 1e9
-    launches_pair = stats["pair_kernel_launches"]
-    pair_ms_avg = stats["pair_kernel_ms"] / max(1, launches_pair)
-
-    # ---- roofline of the dominant kernel: the pair kernel, FMA-pipe ("alu") bound
-    nrhs_launch = cfg.nrhs if cfg.op == "mdot_batch" else 1
-    instr, flops = work_per_pair(cfg.angular, nrhs_launch, f64)
     props = torch.cuda.get_device_properties(local_rank)
     sms = props.multi_processor_count
     try:
@@ -343,45 +434,68 @@ def main():
         sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     except Exception:
         sm_max_mhz = 1965.0
+    clocks = m["clocks"]
     if clocks and clocks.get("sm_max_mhz"):
         sm_max_mhz = float(clocks["sm_max_mhz"])
-    peak = sms * nominal_lanes(f64) * sm_max_mhz * 1e6 / 1e12                 # T lane-ops/s at max clock
-    pairs_per_launch = stats["pairs"] / max(1, launches_pair)                 # rank 0's share when row-sharded
-    achieved = instr * pairs_per_launch / (pair_ms_avg * 1e-3) / 1e12
-    probe = lm.lm_probe_fma_peak(lm.LM_F64 if f64 else lm.LM_F32, 0.3) / 1e12
-    roofline = {
-        "bound": "alu", "kernel": f"rpy_pair_kernel<{cfg.precision}, nrhs={nrhs_launch}, angular={int(cfg.angular)}>",
-        "achieved": achieved, "peak": peak, "unit": "T FP-pipe lane-ops/s", "frac": achieved / peak,
-        "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if args.N is None else None,
-        "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_c%d_pair_kernel_ncu_full.md)" % args.config,
-        "peak_source": f"derived: {sms} SMs x {nominal_lanes(f64)} lanes x {sm_max_mhz:.0f} MHz (clocks.max.sm); MEASURED_PEAKS.json has no ALU entry",
-        "lane_ops_per_pair": instr, "flops_per_pair": flops, "pairs_per_launch": pairs_per_launch,
-        "launch_ms_avg": pair_ms_avg, "launches_timed": launches_pair,
-        "flop_frac": flops * pairs_per_launch / (pair_ms_avg * 1e-3) / 1e12 / (2 * peak),
-        "measured_fma_peak": probe, "frac_of_measured_fma_peak": achieved / probe,
-        "kernel_gpairs_per_s": pairs_per_launch / (pair_ms_avg * 1e-3) / 1e9,
-    }
-    if clocks and clocks.get("sm_mhz"):
-        roofline["frac_at_observed_clock"] = achieved / (sms * nominal_lanes(f64) * clocks["sm_mhz"] * 1e6 / 1e12)
+    probes = {False: probe.fma_peak(lm.LM_F32, 0.3), True: probe.fma_peak(lm.LM_F64, 0.3)}
+    roofline = roofline_of(arm, m, sm_max_mhz, sms, probes[arm.f64], args.config, args.N)
+    stats = m["stats"]
+    nrhs_launch = cfg.nrhs if cfg.op == "mdot_batch" else 1
+    extra = {"parallelism": ("row-sharded, all-gather per apply" if sharded else "replicas only") if world > 1 else "1 GPU",
+             "pair_launches_per_step": stats["pair_kernel_launches"] / args.steps, "lanczos_iterations": m["iters"],
+             "launch": arm.solver.pair_launch_config(nrhs_launch)}
+    if cfg.op == "sqrt+mdot":
+        # what tol delivered: the noise part of the timed step against a long fp64 run (measured outside the timed region)
+        y = torch.empty(3 * N, dtype=torch.float32, device="cuda")
+        arm.solver.sqrt_mdot_w(arm.dev["noise"], cfg.tol, y, None)
+        hist = arm.solver.lanczos_history()
+        extra["lanczos_rule"] = args.lanczos_rule
+        extra["lanczos_error_estimate_at_stop"] = float(hist["estimate"][-1]) if args.lanczos_rule == "estimate" else float(hist["step"][-1])
+        if world == 1 and args.N is None:
+            extra["lanczos_true_rel_error_vs_fp64_300_steps"] = lanczos_true_error(lm, torch, arm, y)
+        del y
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "metric": METRIC, "value": pairs_all / (ms_total * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
-        "dtype": cfg.precision, "data": "synthetic",
-        "config": config_dict(cfg, N, {"l2": "256 MiB device memset between steps, outside the event brackets",
-                                       "parallelism": ("row-sharded, all-gather per apply" if sharded else "replicas only") if world > 1 else "1 GPU",
-                                       "pair_launches_per_step": launches_pair / args.steps, "lanczos_iterations": iters,
-                                       "launch": solver.pair_launch_config(nrhs_launch)}),
-        "ms_per_mdot": pair_ms_avg,
+        "dtype": cfg.precision, "data": "synthetic", "config": config_dict(cfg, N), "details": extra,
+        "ms_per_mdot": roofline["launch_ms_avg"],
         "gpu_launches": int(stats["pair_kernel_launches"] + stats["aux_launches"]),
         "clocks": clocks,
         "roofline": roofline,
     }
     if e2e_ms is not None:
         line["e2e"] = {"value": e2e_pairs_all / (e2e_ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
-                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "api": "lm_set_positions_host + lm_*_host (pinned host buffers)"}
+                       "h2d_bytes_per_step": int(arm.h2d), "d2h_bytes_per_step": int(arm.d2h), "api": "lm_set_positions_host + lm_*_host (pinned host buffers)"}
+    data_headline = arm.data
+    arm.close()
+
+    # ---- the other four configs, a few steps each, so that every config's numbers are on the driver's record
+    if world == 1 and args.config == 3 and args.N is None and not args.no_configs:
+        sub = {}
+        for index, (k, w) in {1: (20, 5), 2: (10, 3), 4: (2, 3), 5: (3, 3)}.items():
+            torch.cuda.empty_cache()
+            a2 = Arm(lm, torch, dist, index, None, 0, 1, False)
+            m2 = a2.measure(k, w, flush, True, ClockSampler(local_rank))
+            r2 = roofline_of(a2, m2, sm_max_mhz, sms, probes[a2.f64], index, None)
+            c2 = a2.cfg
+            sub[str(index)] = {
+                "workload": f"BASELINE.json configs[{index - 1}] ({c2.name})", "steps": k, "warmup": w,
+                "value": m2["stats"]["pairs"] / (m2["ms_total"] * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": m2["ms_total"] / k,
+                "ms_per_launch": r2["launch_ms_avg"], "kernel_gpairs_per_s": r2["kernel_gpairs_per_s"], "lane_ops_per_pair": r2["lane_ops_per_pair"],
+                "frac": r2["frac"], "flop_frac": r2["flop_frac"], "traffic": r2["traffic"], "traffic_source": r2["traffic_source"],
+                "algorithmic_bytes_per_launch": r2["algorithmic_bytes_per_launch"],
+                "e2e": {"value": m2["e2e_stats"]["pairs"] / (m2["e2e_ms"] * 1e-3) / 1e9, "ms_per_step": m2["e2e_ms"] / k,
+                        "h2d_bytes_per_step": int(a2.h2d), "d2h_bytes_per_step": int(a2.d2h)},
+                "launch": a2.solver.pair_launch_config(c2.nrhs if c2.op == "mdot_batch" else 1),
+                "gpu_launches": int(m2["stats"]["pair_kernel_launches"] + m2["stats"]["aux_launches"]),
+                "clocks": m2["clocks"],
+            }
+            a2.close()
+        line["configs"] = sub
+
     if world == 1 and not args.no_cpu_baseline:
-        info = oracle_rate(data, 12.0)
+        info = oracle_rate(data_headline, 12.0)
         line["cpu_baseline"] = {"value": info["pairs"] / info["seconds"] / 1e9, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
                                 "sample": f"{info['nrows']} sampled target rows x all {N} sources, one M.F apply, {info['seconds']:.1f} s"}
     print(json.dumps(line))

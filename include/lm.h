@@ -95,7 +95,8 @@ int lm_mdot_batch(lm_solver* h, int nrhs, const void* forces, const void* torque
 
 /* y = M^{1/2} W by Lanczos.  noise: dof values, [3N linear | 3N angular]
  * (the caller draws W ~ N(0,1); the paper's sqrtMdotW() draws it internally).
- * tol: stop when the relative change between successive iterates is <= tol (S3).
+ * tol: relative error requested of the iterate, as estimated by the stopping rule (LM_OPT_LANCZOS_RULE below;
+ * DESIGN.md reading S3: the default rule's estimate is within x0.5 ... x2 of the true error).
  * lin_out 3N, ang_out 3N (iff include_angular).  iters_out: HOST int*, may be NULL.
  * LM_E_NOCONV if max_iter is reached (result still written). */
 int lm_sqrt_mdot_w(lm_solver* h, const void* noise, double tol, void* lin_out, void* ang_out,
@@ -178,7 +179,8 @@ int lm_thermal_drift_rfd(lm_solver* h, const void* noise, double delta, void* li
  * per pair-kernel launch (over NVLink / NVSwitch) completes every output on every rank.  All entry points
  * (lm_mdot*, lm_sqrt_mdot_w*, lm_hydrodynamic_velocities, lm_thermal_drift_rfd, lm_steric_forces,
  * lm_bd_step) then work unchanged; only the O(N) vector kernels are replicated.  Ranks must run the
- * same GPU model: the Lanczos stopping decision is taken per rank from bit-identical scalars.
+ * same GPU model.  The Lanczos stopping verdict acted upon is rank 0's, broadcast after every iteration, so ranks
+ * cannot part ways even if their scalars ever differed in the last bit.
  *   lm_dist_unique_id : 128-byte NCCL unique id (host buffer); call on ONE rank and broadcast it to the
  *                       others by any means (torch.distributed, MPI, a file).
  *   lm_dist_init      : collective; creates this handle's communicator (current CUDA device) and fixes
@@ -194,11 +196,29 @@ int lm_dist_init(lm_solver* h, int nranks, int rank, const void* unique_id128);
 int lm_mdot_rows(lm_solver* h, int64_t row_begin, int64_t row_count, const void* forces, const void* torques,
                  void* lin_out, void* ang_out, void* stream);
 
-/* Lanczos controls and introspection.  Diagnostics through the environment (read at call time):
- * LM_DEBUG_LANCZOS=1 prints alpha_k, beta_k and the relative step of every iteration on stderr;
- * LM_NO_GRAPH=1 launches the iteration's kernels one by one instead of replaying the captured CUDA graph. */
+/* Lanczos controls and introspection.
+ * lm_set_option: per-handle switches (no environment variables, no global state):
+ *   LM_OPT_LANCZOS_RULE       LM_RULE_ESTIMATE (default) | LM_RULE_STEP -- what `tol` bounds (reading S3; the
+ *                             paper states no rule).  With s_k = |y_k - y_{k-1}| / |y_{k-1}|:
+ *                             STEP: stop at the first k >= 2 with s_k <= tol (the rule of ref. [35]; it under-states the
+ *                             true error by the factor rho/(1 - rho) when the steps shrink slowly: measured 15-20 x tol
+ *                             at N = 131072, phi = 5 %);  ESTIMATE: stop at the first k >= 3 with
+ *                             e_k = max(s_k, s_{k-1}) max(1, rho/(1 - rho)) <= tol, rho = the step ratio per iteration
+ *                             over the trailing min(10, (k-1)/2) steps, capped at 0.98 -- measured within x0.5 ... x2
+ *                             of the true relative error from N = 12 to N = 131072.
+ *   LM_OPT_GRAPH_REPLAY       1 (default) | 0: replay short applies / Lanczos iterations as CUDA graphs, or launch
+ *                             every kernel directly.
+ *   LM_OPT_SHARE_FIRST_APPLY  1 (default) | 0: in lm_hydrodynamic_velocities / lm_bd_step, M.[F;T] rides along with the
+ *                             first Lanczos apply in one 2-right-hand-side launch, or is a launch of its own.
+ * lm_lanczos_history: what the last Lanczos call measured for noise vector `vec` of its (last) group: for iteration
+ *   i + 1 (i < cap): alpha[i], beta[i], step[i] = s_{i+1} (NaN for i = 0), estimate[i] = e_{i+1} (NaN for i < 2; NaN
+ *   throughout under LM_RULE_STEP).  Any output may be NULL.  Returns the number of iterations recorded. */
+enum { LM_RULE_ESTIMATE = 0, LM_RULE_STEP = 1 };
+enum { LM_OPT_LANCZOS_RULE = 0, LM_OPT_GRAPH_REPLAY = 1, LM_OPT_SHARE_FIRST_APPLY = 2 };
+int lm_set_option(lm_solver* h, int option, int value);
 int lm_set_max_iter(lm_solver* h, int max_iter);     /* default 100; 1 <= max_iter <= 1000 */
 int lm_last_iterations(const lm_solver* h);           /* iterations of the last Lanczos call (or < 0) */
+int lm_lanczos_history(const lm_solver* h, int vec, int cap, double* alpha, double* beta, double* step, double* estimate);
 const char* lm_last_error(const lm_solver* h);        /* never NULL; "" if the last call succeeded */
 
 /* Launch accounting for benchmarks.  Counters accumulate from lm_create or the last reset.
@@ -216,16 +236,6 @@ int lm_get_stats(lm_solver* h, int64_t* pair_kernel_launches, int64_t* aux_launc
  * of `block` threads, `targets_per_thread` targets each, `smem_bytes` dynamic shared memory. */
 int lm_pair_launch_config(lm_solver* h, int nrhs, int* i_tiles, int* j_splits, int* block,
                           int* targets_per_thread, int* smem_bytes);
-
-/* Host-only helper of the Lanczos driver, exported so that it can be tested without a GPU:
- * c = T^{1/2} e_1 for the symmetric tridiagonal T = tridiag(beta[0..k-2]; alpha[0..k-1]) by an
- * implicit-shift QL eigensolve in fp64, negative eigenvalues clamped to 0.  c_out: k doubles. */
-int lm_host_tridiag_sqrt_e1(int k, const double* alpha, const double* beta, double* c_out);
-
-/* Diagnostic: measured FMA-pipe peak of the current device, in lane-operations per second
- * (one lane-op = one fp32 / fp64 FMA on one lane), from a register-only FFMA2 / DFMA loop run for
- * about `seconds`.  This is the roofline denominator bench.py reports next to the nominal one. */
-int lm_probe_fma_peak(int precision, double seconds, double* lane_ops_per_s);
 
 /* Library version string (static storage). */
 const char* lm_version(void);

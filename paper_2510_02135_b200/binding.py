@@ -17,6 +17,8 @@ import numpy as np
 
 LM_F32, LM_F64 = 0, 1
 LM_OK, LM_E_INVALID, LM_E_NOPOS, LM_E_ANGULAR, LM_E_NULL, LM_E_CUDA, LM_E_NOCONV = 0, -1, -2, -3, -4, -5, -6
+LM_RULE_ESTIMATE, LM_RULE_STEP = 0, 1
+LM_OPT_LANCZOS_RULE, LM_OPT_GRAPH_REPLAY, LM_OPT_SHARE_FIRST_APPLY = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liblm.so")
@@ -47,6 +49,8 @@ SIGNATURES = {
     "lm_dist_unique_id": (c_int, [c_void_p]),
     "lm_dist_init": (c_int, [c_void_p, c_int, c_int, c_void_p]),
     "lm_mdot_rows": (c_int, [c_void_p, c_int64, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "lm_set_option": (c_int, [c_void_p, c_int, c_int]),
+    "lm_lanczos_history": (c_int, [c_void_p, c_int, c_int, POINTER(c_double), POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
     "lm_set_max_iter": (c_int, [c_void_p, c_int]),
     "lm_last_iterations": (c_int, [c_void_p]),
     "lm_last_error": (c_char_p, [c_void_p]),
@@ -54,8 +58,6 @@ SIGNATURES = {
     "lm_reset_stats": (c_int, [c_void_p]),
     "lm_get_stats": (c_int, [c_void_p, POINTER(c_int64), POINTER(c_int64), POINTER(c_double), POINTER(c_double)]),
     "lm_pair_launch_config": (c_int, [c_void_p, c_int, POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int)]),
-    "lm_host_tridiag_sqrt_e1": (c_int, [c_int, POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
-    "lm_probe_fma_peak": (c_int, [c_int, c_double, POINTER(c_double)]),
     "lm_version": (c_char_p, []),
 }
 
@@ -84,18 +86,6 @@ def lm_version() -> str:
     return lib().lm_version().decode()
 
 
-def lm_host_tridiag_sqrt_e1(alpha, beta) -> np.ndarray:
-    alpha = np.ascontiguousarray(alpha, dtype=np.float64)
-    beta = np.ascontiguousarray(beta, dtype=np.float64)
-    k = alpha.size
-    out = np.zeros(k)
-    dp = POINTER(c_double)
-    rc = lib().lm_host_tridiag_sqrt_e1(k, alpha.ctypes.data_as(dp), beta.ctypes.data_as(dp) if k > 1 else None, out.ctypes.data_as(dp))
-    if rc != LM_OK:
-        raise LmError(rc, "lm_host_tridiag_sqrt_e1")
-    return out
-
-
 def lm_dist_row_block(N: int, nranks: int, rank: int):
     """(row_begin, row_end) of `rank`'s block of target rows -- host only, needs no GPU."""
     b, e = c_int64(0), c_int64(0)
@@ -111,14 +101,6 @@ def lm_dist_unique_id() -> bytes:
     if rc != LM_OK:
         raise LmError(rc, "lm_dist_unique_id: NCCL unavailable")
     return buf.raw
-
-
-def lm_probe_fma_peak(precision: int, seconds: float = 0.2) -> float:
-    out = c_double(0.0)
-    rc = lib().lm_probe_fma_peak(precision, seconds, ctypes.byref(out))
-    if rc != LM_OK:
-        raise LmError(rc, "lm_probe_fma_peak")
-    return out.value
 
 
 def _ptr(x):
@@ -303,6 +285,17 @@ class Solver:
         self._check(lib().lm_thermal_drift_rfd(self._h, _ptr(noise), float(delta), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
 
     # -- controls / introspection
+    def set_option(self, option: int, value: int):
+        self._check(lib().lm_set_option(self._h, int(option), int(value)))
+
+    def lanczos_history(self, vec: int = 0) -> dict:
+        """alpha_k, beta_k, relative step s_k and error estimate e_k of the last Lanczos call, k = 1 .. iterations."""
+        dp = POINTER(c_double)
+        cap = 1001
+        arrs = [np.full(cap, np.nan) for _ in range(4)]
+        k = lib().lm_lanczos_history(self._h, int(vec), cap, *[a.ctypes.data_as(dp) for a in arrs])
+        return dict(zip(("alpha", "beta", "step", "estimate"), (a[:k] for a in arrs)))
+
     def set_max_iter(self, n):
         self._check(lib().lm_set_max_iter(self._h, int(n)))
 

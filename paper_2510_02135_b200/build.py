@@ -15,8 +15,11 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblm.so")
 SOURCES = [os.path.join(CSRC, "lm_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("rpy_pair.cuh", "steric_pair.cuh", "vector_kernels.cuh", "lm_common.cuh", "tridiag_host.h",
-                                                    "lm_handle.cuh", "lm_apply.cuh", "lm_lanczos.cuh", "lm_bd.cuh")] + [
+                                                    "lanczos_host.h", "lm_handle.cuh", "lm_apply.cuh", "lm_lanczos.cuh", "lm_bd.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "lm.h")]
+# measurement helper of bench.py (FMA-pipe peak probe): its own library, not part of liblm.so
+PROBE_LIB = os.path.join(HERE, "liblm_probe.so")
+PROBE_SOURCES = [os.path.join(CSRC, "fma_probe.cu")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -44,6 +47,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
         subprocess.run(cmd, check=True)
+    if force or not os.path.exists(PROBE_LIB) or os.path.getmtime(PROBE_LIB) < os.path.getmtime(PROBE_SOURCES[0]):
+        subprocess.run([nvcc()] + NVCC_FLAGS + ["-o", PROBE_LIB] + PROBE_SOURCES, check=True)
     return LIB
 
 

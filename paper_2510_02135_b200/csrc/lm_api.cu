@@ -21,6 +21,7 @@
 #include "../../include/lm.h"
 #include "rpy_pair.cuh"
 #include "steric_pair.cuh"
+#include "lanczos_host.h"
 #include "tridiag_host.h"
 #include "vector_kernels.cuh"
 
@@ -73,37 +74,6 @@ int stage_out_alloc(lm_solver* h, int slot, const void* host, size_t bytes, void
     return LM_OK;
 }
 
-// register-only FMA loops for lm_probe_fma_peak
-__global__ void probe_ffma2_kernel(float* out, float a, float b, int iters)
-{
-    float2 x[8];
-    const float2 aa = make_float2(a, a), bb = make_float2(b, b);
-#pragma unroll
-    for (int i = 0; i < 8; ++i) x[i] = make_float2(threadIdx.x * 1e-3f + i, (float)i);
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < 8; ++i) x[i] = __ffma2_rn(x[i], aa, bb);
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) s += x[i].x + x[i].y;
-    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-__global__ void probe_dfma_kernel(double* out, double a, double b, int iters)
-{
-    double x[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) x[i] = threadIdx.x * 1e-3 + i;
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < 8; ++i) x[i] = fma(x[i], a, b);
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) s += x[i];
-    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-
 }  // namespace
 
 // ================================================================ C ABI
@@ -153,6 +123,8 @@ int lm_destroy(lm_solver* h)
     cudaFree(h->d_coef);
     cudaFree(h->d_gram_part);
     cudaFree(h->d_newest);
+    cudaFree(h->d_word);
+    if (h->h_word) cudaFreeHost(h->h_word);
     if (h->h_gram) cudaFreeHost(h->h_gram);
     if (h->h_ab) cudaFreeHost(h->h_ab);
     if (h->lz_graph) cudaGraphExecDestroy(h->lz_graph);
@@ -182,6 +154,36 @@ int lm_set_max_iter(lm_solver* h, int max_iter)
 }
 
 int lm_last_iterations(const lm_solver* h) { return h ? h->last_iters : -1; }
+
+int lm_set_option(lm_solver* h, int option, int value)
+{
+    if (!h) return LM_E_NULL;
+    switch (option) {
+    case LM_OPT_LANCZOS_RULE:
+        if (value != LM_RULE_ESTIMATE && value != LM_RULE_STEP) return fail(h, LM_E_INVALID, "LM_OPT_LANCZOS_RULE: LM_RULE_ESTIMATE or LM_RULE_STEP");
+        h->lz_rule = value;
+        return LM_OK;
+    case LM_OPT_GRAPH_REPLAY: h->graph_replay = value != 0; return LM_OK;
+    case LM_OPT_SHARE_FIRST_APPLY: h->share_first_apply = value != 0; return LM_OK;
+    default: return fail(h, LM_E_INVALID, "unknown option");
+    }
+}
+
+int lm_lanczos_history(const lm_solver* h, int vec, int cap, double* alpha, double* beta, double* step, double* estimate)
+{
+    if (!h) return LM_E_NULL;
+    if (vec < 0 || vec >= (int)h->lz_stop.size()) return 0;
+    const LanczosStopper& s = h->lz_stop[vec];
+    const int k = (int)s.alphas.size();
+    for (int i = 0; i < k && i < cap; ++i) {
+        // iteration i + 1: alpha and beta; the relative step exists from k = 2, the estimate from k = 3
+        if (alpha) alpha[i] = s.alphas[i];
+        if (beta) beta[i] = i < (int)s.betas.size() ? s.betas[i] : s.pending_beta;
+        if (step) step[i] = i >= 1 && i - 1 < (int)s.steps.size() ? s.steps[i - 1] : NAN;
+        if (estimate) estimate[i] = i >= 2 && i - 2 < (int)s.estimates.size() ? s.estimates[i - 2] : NAN;
+    }
+    return k;
+}
 
 int lm_set_positions(lm_solver* h, const void* pos, void* stream)
 {
@@ -252,23 +254,49 @@ int lm_sqrt_mdot_w_batch(lm_solver* h, int nvec, const void* noise, double tol, 
     return worst;
 }
 
+}  // extern "C"
+
+namespace {
+
+// out = M.[F;T] + prefactor M^{1/2} W: the deterministic right-hand side rides along with the first Lanczos apply
+// (one 2-right-hand-side launch) where a variant for it exists; otherwise M.[F;T] is a launch of its own
+template <typename T>
+int hydrodynamic_velocities_t(lm_solver* h, const T* forces, const T* torques, const T* noise, double noise_prefactor, double tol, T* lin_out, T* ang_out,
+                              cudaStream_t st)
+{
+    const bool have_det = forces || torques;
+    if (!noise) return apply_batch<T>(h, 1, forces, torques, lin_out, ang_out, st);
+    if (!have_det) return lanczos_device<T>(h, 1, noise, tol, lin_out, ang_out, noise_prefactor, 0, nullptr, st);
+    DetShare<T> det;
+    det.f = forces;
+    det.t = torques;
+    det.lin = lin_out;
+    det.ang = ang_out;
+    if (!h->share_first_apply) {
+        const int rc = apply_batch<T>(h, 1, forces, torques, lin_out, ang_out, st);
+        if (rc != LM_OK) return rc;
+        return lanczos_device<T>(h, 1, noise, tol, lin_out, ang_out, noise_prefactor, 1, nullptr, st);
+    }
+    // the Lanczos result is accumulated onto lin_out / ang_out at the end, after the shared launch has written M.[F;T] there
+    return lanczos_device<T>(h, 1, noise, tol, lin_out, ang_out, noise_prefactor, 1, nullptr, st, &det);
+}
+
+}  // namespace
+
+extern "C" {
+
 int lm_hydrodynamic_velocities(lm_solver* h, const void* forces, const void* torques, const void* noise, double noise_prefactor, double tol,
                                void* lin_out, void* ang_out, void* stream)
 {
     int rc = check_io(h, forces, torques, lin_out, ang_out, noise == nullptr);
     if (rc != LM_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    const bool have_det = forces || torques;
-    if (have_det) {
-        rc = lm_mdot_batch(h, 1, forces, torques, lin_out, ang_out, stream);
-        if (rc != LM_OK) return rc;
-    }
-    if (!noise) return LM_OK;
-    if (!(tol > 0.0) || !std::isfinite(tol)) return fail(h, LM_E_INVALID, "tol must be > 0");
-    const int acc = have_det ? 1 : 0;
+    if (noise && (!(tol > 0.0) || !std::isfinite(tol))) return fail(h, LM_E_INVALID, "tol must be > 0");
     return h->precision == LM_F32
-               ? lanczos_device<float>(h, 1, (const float*)noise, tol, (float*)lin_out, (float*)ang_out, noise_prefactor, acc, nullptr, st)
-               : lanczos_device<double>(h, 1, (const double*)noise, tol, (double*)lin_out, (double*)ang_out, noise_prefactor, acc, nullptr, st);
+               ? hydrodynamic_velocities_t<float>(h, (const float*)forces, (const float*)torques, (const float*)noise, noise_prefactor, tol, (float*)lin_out,
+                                                  (float*)ang_out, st)
+               : hydrodynamic_velocities_t<double>(h, (const double*)forces, (const double*)torques, (const double*)noise, noise_prefactor, tol,
+                                                   (double*)lin_out, (double*)ang_out, st);
 }
 
 // ---------------------------------------------------------------- host-pointer variants
@@ -542,55 +570,6 @@ int lm_pair_launch_config(lm_solver* h, int nrhs, int* i_tiles, int* j_splits, i
     if (block) *block = blk;
     if (targets_per_thread) *targets_per_thread = tpt;
     if (smem_bytes) *smem_bytes = smem;
-    return LM_OK;
-}
-
-int lm_host_tridiag_sqrt_e1(int k, const double* alpha, const double* beta, double* c_out)
-{
-    if (k < 1) return LM_E_INVALID;
-    if (!alpha || !c_out || (k > 1 && !beta)) return LM_E_NULL;
-    return tridiag_sqrt_e1(k, alpha, beta, c_out) ? LM_OK : LM_E_NOCONV;
-}
-
-int lm_probe_fma_peak(int precision, double seconds, double* lane_ops_per_s)
-{
-    if (!lane_ops_per_s) return LM_E_NULL;
-    if (precision != LM_F32 && precision != LM_F64) return LM_E_INVALID;
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return LM_E_CUDA;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return LM_E_CUDA;
-    const int threads = 256, grid = sms * 8, iters = 8192;
-    void* buf = nullptr;
-    if (cudaMalloc(&buf, (size_t)grid * threads * 8) != cudaSuccess) return LM_E_CUDA;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
-    auto launch = [&]() {
-        if (precision == LM_F32) probe_ffma2_kernel<<<grid, threads>>>((float*)buf, 1.0001f, 0.5f, iters);
-        else probe_dfma_kernel<<<grid, threads>>>((double*)buf, 1.0001, 0.5, iters);
-    };
-    const double ops_per_launch = (double)grid * threads * iters * (precision == LM_F32 ? 16.0 : 8.0);
-    launch();
-    launch();
-    cudaDeviceSynchronize();
-    double best = 0.0, elapsed = 0.0;
-    int reps = 0;
-    while (elapsed < seconds * 1e3 || reps < 3) {
-        cudaEventRecord(e0);
-        launch();
-        cudaEventRecord(e1);
-        cudaEventSynchronize(e1);
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, e0, e1);
-        elapsed += ms;
-        best = std::max(best, ops_per_launch / (ms * 1e-3));
-        if (++reps > 100000) break;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(buf);
-    if (cudaGetLastError() != cudaSuccess) return LM_E_CUDA;
-    *lane_ops_per_s = best;
     return LM_OK;
 }
 

@@ -20,13 +20,14 @@ template <typename T> int prepare_apply(lm_solver* h, int nrhs, LaunchPlan& plan
     return LM_OK;
 }
 
-// launch_pair: the pair kernel on the packed right-hand side already in h->vec_soa, then the split-j reduce.
+// launch_pair: the pair kernel on the packed right-hand side already in h->vec_soa, then the split-j reduce
+// (of the right-hand sides from `reduce_from` on).
 // Only the target rows [h->row_begin, h->row_end) are computed.  With a communicator (lm_dist_init) those are
 // this rank's block: the kernel writes into all-gather buffers of 3 B ranks elements, ONE grouped
 // ncclAllGather (in place: rank r's segment starts at 3 B r) completes every output on every rank, and the
 // first 3N elements are copied to the caller's buffers.
 template <typename T>
-int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>& out, cudaStream_t st, bool timed, bool reduce = true)
+int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>& out, cudaStream_t st, bool timed, int reduce_from = 0)
 {
     const int nc = h->angular ? 6 : 3;
     const auto& v = variants<T>(h)[plan.variant];
@@ -67,9 +68,10 @@ int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>&
         LM_CUDA(h, cudaEventRecord(e1, st));
         h->pending.emplace_back(e0, e1);
     }
-    if (plan.i_tiles > 0 && plan.j_splits > 1 && reduce)      // reduce == false: the caller's next kernel sums the partials itself
-        reduce_partials_kernel<T><<<dim3(grid_1d(h->row_end - h->row_begin), nrhs * nc), VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc,
-                                                                                                         h->row_begin, h->row_end, h->npad, kout);
+    // split-j reduce of the right-hand sides [reduce_from, nrhs); the caller's next kernel sums the partials of the others itself
+    if (plan.i_tiles > 0 && plan.j_splits > 1 && reduce_from < nrhs)
+        reduce_partials_kernel<T><<<dim3(grid_1d(h->row_end - h->row_begin), (nrhs - reduce_from) * nc), VEC_BLOCK, 0, st>>>(
+            (const T*)h->partial, plan.j_splits, nrhs, nc, reduce_from, h->row_begin, h->row_end, h->npad, kout);
     LM_CUDA(h, cudaGetLastError());
     if (dist) {
         NcclApi& nccl = nccl_api();
@@ -120,7 +122,7 @@ template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& i
     // once and replayed as a CUDA graph from then on; any other call is launched directly.
     const double cost = (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N * (h->angular ? 2.3 : 1.0) *
                         (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nrhs);
-    if (cost < 2.0e8 && !h->profiling && h->dist_ranks == 0 && std::getenv("LM_NO_GRAPH") == nullptr) {      // N <~ 14000 fp32
+    if (cost < 2.0e8 && !h->profiling && h->dist_ranks == 0 && h->graph_replay) {      // N <~ 14000 fp32
         lm_solver::ApplyKey key;
         std::memset(&key, 0, sizeof key);
         for (int q = 0; q < nrhs; ++q) { key.f[q] = in.f[q]; key.t[q] = in.t[q]; key.lin[q] = out.lin[q]; key.ang[q] = out.ang[q]; }

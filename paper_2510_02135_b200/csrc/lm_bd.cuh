@@ -101,16 +101,28 @@ int bd_step_device(lm_solver* h, T* pos, const T* ext_f, const T* ext_t, const T
         if ((rc = steric_device<T>(h, U0, b, ext_f, F, st)) != LM_OK) return rc;
     }
     const T* Fin = U0 != 0.0 ? F : ext_f;
-    if (have_force || ext_t) {
-        if ((rc = apply_batch<T>(h, 1, Fin, ext_t, vn, h->angular ? ang : nullptr, st)) != LM_OK) return rc;
-    } else {
-        LM_CUDA(h, cudaMemsetAsync(vn, 0, bytes, st));
-    }
+    const bool have_det = have_force || ext_t;
     int rc_noise = LM_OK;
     const bool noisy = noise && kT > 0.0;
-    if (noisy) {
-        rc_noise = lanczos_device<T>(h, 1, noise, tol, y, h->angular ? yang : nullptr, 1.0, 0, nullptr, st);
+    if (noisy && have_det && h->share_first_apply) {
+        // v_n = M^n [F^n; T] rides along with the first Lanczos apply (one 2-right-hand-side launch)
+        DetShare<T> det;
+        det.f = Fin;
+        det.t = ext_t;
+        det.lin = vn;
+        det.ang = h->angular ? ang : nullptr;
+        rc_noise = lanczos_device<T>(h, 1, noise, tol, y, h->angular ? yang : nullptr, 1.0, 0, nullptr, st, &det);
         if (rc_noise != LM_OK && rc_noise != LM_E_NOCONV) return rc_noise;
+    } else {
+        if (have_det) {
+            if ((rc = apply_batch<T>(h, 1, Fin, ext_t, vn, h->angular ? ang : nullptr, st)) != LM_OK) return rc;
+        } else {
+            LM_CUDA(h, cudaMemsetAsync(vn, 0, bytes, st));
+        }
+        if (noisy) {
+            rc_noise = lanczos_device<T>(h, 1, noise, tol, y, h->angular ? yang : nullptr, 1.0, 0, nullptr, st);
+            if (rc_noise != LM_OK && rc_noise != LM_E_NOCONV) return rc_noise;
+        }
     }
     const double cn = h->bd_have_prev ? 1.5 : 1.0, cp = h->bd_have_prev ? 0.5 : 0.0;
     bd_update_kernel<T><<<grid_1d(n3), VEC_BLOCK, 0, st>>>(pos, vn, vprev, noisy ? y : nullptr, n3, (T)(dt * cn), (T)(dt * cp),

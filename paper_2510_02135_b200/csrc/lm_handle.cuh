@@ -68,13 +68,14 @@ struct NcclApi {
     int (*CommInitRank)(Comm*, int, UniqueId, int) = nullptr;
     int (*CommDestroy)(Comm) = nullptr;
     int (*AllGather)(const void*, void*, size_t, int, Comm, cudaStream_t) = nullptr;
+    int (*Broadcast)(const void*, void*, size_t, int, int, Comm, cudaStream_t) = nullptr;
     int (*GroupStart)() = nullptr;
     int (*GroupEnd)() = nullptr;
     const char* (*GetErrorString)(int) = nullptr;
     bool ok = false;
     std::string why;
 };
-constexpr int NCCL_FLOAT32 = 7, NCCL_FLOAT64 = 8;   // ncclDataType_t values (nccl.h)
+constexpr int NCCL_INT32 = 2, NCCL_FLOAT32 = 7, NCCL_FLOAT64 = 8;   // ncclDataType_t values (nccl.h)
 
 inline NcclApi& nccl_api()
 {
@@ -90,10 +91,11 @@ inline NcclApi& nccl_api()
     api.CommInitRank = (int (*)(NcclApi::Comm*, int, NcclApi::UniqueId, int))sym("ncclCommInitRank");
     api.CommDestroy = (int (*)(NcclApi::Comm))sym("ncclCommDestroy");
     api.AllGather = (int (*)(const void*, void*, size_t, int, NcclApi::Comm, cudaStream_t))sym("ncclAllGather");
+    api.Broadcast = (int (*)(const void*, void*, size_t, int, int, NcclApi::Comm, cudaStream_t))sym("ncclBroadcast");
     api.GroupStart = (int (*)())sym("ncclGroupStart");
     api.GroupEnd = (int (*)())sym("ncclGroupEnd");
     api.GetErrorString = (const char* (*)(int))sym("ncclGetErrorString");
-    api.ok = api.GetUniqueId && api.CommInitRank && api.CommDestroy && api.AllGather && api.GroupStart && api.GroupEnd && api.GetErrorString;
+    api.ok = api.GetUniqueId && api.CommInitRank && api.CommDestroy && api.AllGather && api.Broadcast && api.GroupStart && api.GroupEnd && api.GetErrorString;
     return api;
 }
 }  // namespace lm
@@ -108,6 +110,9 @@ struct lm_solver {
     double len_scale = 1.0;    // power of two nearest 1/a: lengths are stored x len_scale, so the kernels see a radius in [0.71, 1.41]
     int angular = 0;
     int max_iter = 100;
+    int lz_rule = lm::RULE_ESTIMATE;   // Lanczos stopping rule (reading S3; LM_OPT_LANCZOS_RULE)
+    bool graph_replay = true;          // short applies / Lanczos iterations replayed as CUDA graphs (LM_OPT_GRAPH_REPLAY)
+    bool share_first_apply = true;     // M.[F;T] rides along with the first Lanczos apply (LM_OPT_SHARE_FIRST_APPLY)
     int device = 0, sm_count = 0;
     bool have_pos = false;
     std::string err;
@@ -130,6 +135,8 @@ struct lm_solver {
     double* h_ab = nullptr;    // [1] |z|^2; [2k], [2k+1]: alpha_k, beta_k^2
     double* h_gram = nullptr;  // column c at [c * (max_iter + 2) + j] = V[j].V[c], j <= c
     cudaEvent_t lz_ev[2] = {nullptr, nullptr};   // iteration k's scalars have landed (parity k & 1)
+    std::vector<lm::LanczosStopper> lz_stop;     // host state of the last Lanczos call, one per noise vector (lm_lanczos_history)
+    unsigned *d_word = nullptr, *h_word = nullptr;   // the stopping verdicts rank 0 broadcasts (row-sharded runs)
     // one Lanczos iteration captured as a CUDA graph (small N: the loop is launch-bound)
     cudaStream_t cap_stream = nullptr;
     cudaGraphExec_t lz_graph = nullptr;

@@ -1,8 +1,36 @@
 // lm_lanczos.cuh -- host driver of the Lanczos iteration for M^{1/2} W.
-// Included by lm_api.cu only, after lm_apply.cuh.
+// Included by lm_api.cu only, after lm_apply.cuh.  The stopping test itself lives in lanczos_host.h.
 #pragma once
 
 namespace {
+
+// One deterministic right-hand side [F;T] whose product M.[F;T] rides along with the FIRST Lanczos apply in one
+// multi-right-hand-side launch (eq. (9) PAPER.md:78 / the sum of PAPER.md:137-138 needs both; SURVEY.md sec. 7
+// step 7): the pair geometry of that launch is evaluated once for the two vectors.
+template <typename T> struct DetShare {
+    const T* f = nullptr;      // 3N forces or null
+    const T* t = nullptr;      // 3N torques or null
+    T* lin = nullptr;          // 3N: receives M.[F;T] (linear rows)
+    T* ang = nullptr;          // 3N (angular handles)
+};
+
+// rank 0's word for everybody (row-sharded runs; lanczos_host.h agree_on_stops)
+int broadcast_word(lm_solver* h, unsigned* word, cudaStream_t st)
+{
+    if (!h->d_word) {
+        LM_CUDA(h, cudaMalloc((void**)&h->d_word, sizeof(unsigned)));
+        LM_CUDA(h, cudaHostAlloc((void**)&h->h_word, sizeof(unsigned), cudaHostAllocDefault));
+    }
+    NcclApi& nccl = nccl_api();
+    *h->h_word = *word;
+    LM_CUDA(h, cudaMemcpyAsync(h->d_word, h->h_word, sizeof(unsigned), cudaMemcpyHostToDevice, st));
+    const int nrc = nccl.Broadcast(h->d_word, h->d_word, 1, NCCL_INT32, 0, (NcclApi::Comm)h->nccl_comm, st);
+    if (nrc != 0) return fail(h, LM_E_CUDA, std::string("ncclBroadcast failed: ") + nccl.GetErrorString(nrc));
+    LM_CUDA(h, cudaMemcpyAsync(h->h_word, h->d_word, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+    LM_CUDA(h, cudaStreamSynchronize(st));
+    *word = *h->h_word;
+    return LM_OK;
+}
 
 // ---------------------------------------------------------------- Lanczos driver (a7-a10)
 // nv <= MAX_RHS (angular: 2) independent Lanczos recurrences advanced in lockstep: one multi-right-hand-side
@@ -10,7 +38,7 @@ namespace {
 // once per vector.  nv = 1 is lm_sqrt_mdot_w.  noise / outputs: [nv][dof] / [nv][3N].  iters_out: nv ints.
 template <typename T>
 int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out, T* ang_out, double scale, int accumulate, int* iters_out,
-                   cudaStream_t st)
+                   cudaStream_t st, DetShare<T>* det = nullptr)
 {
     const int64_t dof = dof_of(h), n3 = 3 * h->N;
     const int nc = h->angular ? 6 : 3;
@@ -47,15 +75,19 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     const int gr = grid_red(dof);
     const int gg = (int)std::min<int64_t>(GRAM_MAX_BLOCKS, std::max<int64_t>(1, dof / (4 * VEC_BLOCK)));
     const int64_t gchunk = (dof + gg - 1) / gg;
-    LaunchPlan plan;
+    // launch plans: `plan` for the nv Lanczos vectors; `plan_det` for the first apply when a deterministic right-hand
+    // side rides along (one more vector; only where a variant for nv + 1 exists).  Both sized before any launch.
+    LaunchPlan plan, plan_det;
+    const bool share = det && choose_plan<T>(h, nv + 1).variant >= 0;
+    // no variant for nv + 1 vectors: M.[F;T] is a launch of its own, before the packed array holds v_1
+    if (det && !share && (rc = apply_batch<T>(h, 1, det->f, det->t, det->lin, det->ang, st)) != LM_OK) return rc;
+    if (share && (rc = prepare_apply<T>(h, nv + 1, plan_det)) != LM_OK) return rc;
     if ((rc = prepare_apply<T>(h, nv, plan)) != LM_OK) return rc;
     auto soa = [&](int q) { return (T*)h->vec_soa + (size_t)q * nc * h->npad; };
-    // Gram matrices of the bases, G[q][i][j] = V_q[i].V_q[j], filled one column per new basis vector
-    const int ldg = kmax + 1;
-    std::vector<std::vector<double>> G(nv, std::vector<double>((size_t)ldg * ldg, 0.0));
-    auto gram_store = [&](int q, int m) {
-        for (int j = 0; j <= m; ++j) G[q][(size_t)j * ldg + m] = G[q][(size_t)m * ldg + j] = hg(q)[(size_t)m * ld + j];
-    };
+    std::vector<LanczosStopper>& stop = h->lz_stop;
+    stop.resize(nv);
+    const double breakdown = (h->precision == LM_F32) ? 1e-6 : 1e-14;
+    for (int q = 0; q < nv; ++q) stop[q].reset(h->lz_rule, tol, breakdown, kmax);
     // new basis vectors V_q[*newest + 1] = x_q / sqrt(sumsq_q) (+ packed copies for the next apply), their Gram
     // columns; *newest was advanced to their slot by the reduction that produced the norms (sumsq / beta kernel of
     // the LAST vector: the recurrences move in lockstep)
@@ -74,20 +106,30 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
         sumsq_kernel<T><<<gr, VEC_BLOCK, 0, st>>>(noise + (size_t)q * dof, dof, h->d_block, h->d_ticket, scal(q), h->h_ab + (size_t)q * 2 * ld + 1,
                                                   q == nv - 1 ? h->d_newest : nullptr);
     new_vectors(noise, 0, st);
+    if (share) {                                       // the deterministic right-hand side goes into slot nv of the packed array
+        RhsIn<T> din{};
+        din.f[0] = det->f;
+        din.t[0] = det->t;
+        pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>(din, 1, nc, h->N, h->npad, (T)h->len_scale, soa(nv));
+        h->n_aux++;
+    }
     h->n_aux += 3 * nv;
     LM_CUDA(h, cudaGetLastError());
     LM_CUDA(h, cudaStreamSynchronize(st));
     std::vector<double> znorm(nv);
     std::vector<char> done(nv, 0), conv(nv, 0);
     std::vector<int> kfin(nv, 0);
-    std::vector<std::vector<double>> alphas(nv), betas(nv), c_prev(nv), c_cur(nv), c_fin(nv);
+    std::vector<std::vector<double>> c_fin(nv);
     int remaining = nv;
     for (int q = 0; q < nv; ++q) {
-        gram_store(q, 0);
+        stop[q].set_gram_column(0, hg(q));
         znorm[q] = std::sqrt(ab(q)[1]);
         if (!(znorm[q] > 0.0)) { done[q] = conv[q] = 1; --remaining; }            // zero noise: M^{1/2} 0 = 0
     }
     h->last_iters = 0;
+    // zero noise: no first apply to ride along with, M.[F;T] is a launch of its own (no iteration follows)
+    if (share && remaining == 0 && (rc = apply_batch<T>(h, 1, det->f, det->t, det->lin, det->ang, st)) != LM_OK) return rc;
+    const bool ride = share && remaining > 0;
 
     // Iteration k on the device, with m = k - 1 = *newest, for every vector:  w = M v_k;  w -= beta_{k-1} v_{k-1};
     // alpha_k;  w -= alpha_k v_k;  beta_k^2;  v_{k+1} = w / beta_k (+ packed for the next apply);  Gram column k.
@@ -101,13 +143,22 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     }
     // the alpha kernel doubles as the split-j reduce of the apply (one launch less per vector and iteration),
     // except for row-sharded runs, where w must be all-gathered before any rank can use it
-    const bool fuse_reduce = plan.j_splits > 1 && plan.i_tiles > 0 && h->dist_ranks == 0;
-    auto body = [&](cudaStream_t s2, bool timed) -> int {
+    auto fused = [&](const LaunchPlan& pl) { return pl.j_splits > 1 && pl.i_tiles > 0 && h->dist_ranks == 0; };
+    auto body = [&](cudaStream_t s2, bool timed, bool with_det) -> int {
         int rc2;
-        if ((rc2 = launch_pair<T>(h, nv, plan, out, s2, timed, !fuse_reduce)) != LM_OK) return rc2;       // w_q = M v_k,q
+        const LaunchPlan& pl = with_det ? plan_det : plan;
+        const int nr = with_det ? nv + 1 : nv;
+        RhsOut<T> o = out;
+        if (with_det) {
+            o.lin[nv] = det->lin;
+            o.ang[nv] = h->angular ? det->ang : nullptr;
+        }
+        const bool fuse = fused(pl);
+        // w_q = M v_k,q (and M.[F;T]); with a fused reduce only the deterministic vector is reduced here
+        if ((rc2 = launch_pair<T>(h, nr, pl, o, s2, timed, fuse ? nv : 0)) != LM_OK) return rc2;
         for (int q = 0; q < nv; ++q) {
             lanczos_alpha_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q) + 2, dof, h->d_block, h->d_ticket, scal(q) + 1,
-                                                              fuse_reduce ? (const T*)h->partial : nullptr, plan.j_splits, nv, q, nc, h->npad);
+                                                              fuse ? (const T*)h->partial : nullptr, pl.j_splits, nr, q, nc, h->npad);
             lanczos_beta_kernel<T><<<gr, VEC_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q) + 1, dof, h->d_block, h->d_ticket, scal(q) + 2,
                                                              h->h_ab + (size_t)q * 2 * ld, q == nv - 1 ? h->d_newest : nullptr);
         }
@@ -119,16 +170,18 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     // for iteration k's scalars, so the device never idles on the host round trip.  The price is one
     // wasted apply at convergence, so it is used only where an apply costs less than the round trips it
     // saves (~25 iterations x 50 us); the same regime is launch-bound, so there the body runs as a graph.
+    // Row-sharded runs agree on the verdict through the stream after every iteration: no look-ahead there.
     const double apply_cost = (double)h->N * (double)h->N * (h->angular ? 2.3 : 1.0) * (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nv);
-    const bool lookahead = apply_cost < 2.0e9;
-    const bool use_graph = lookahead && !h->profiling && h->dist_ranks == 0 && std::getenv("LM_NO_GRAPH") == nullptr;
+    const bool dist = h->dist_ranks > 0;
+    const bool lookahead = apply_cost < 2.0e9 && !dist;
+    const bool use_graph = lookahead && !h->profiling && h->graph_replay;
     if (use_graph && remaining > 0) {
         const lm_solver::GraphKey key = {h->V, h->w, h->vec_soa, h->partial, h->pos_soa, kmax, plan.variant, plan.j_splits, h->precision * 8 + nv};
         if (!h->lz_graph || std::memcmp(&key, &h->lz_key, sizeof key) != 0) {
             if (h->lz_graph) { LM_CUDA(h, cudaGraphExecDestroy(h->lz_graph)); h->lz_graph = nullptr; }
             cudaGraph_t graph = nullptr;
             LM_CUDA(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
-            const int rc_body = body(h->cap_stream, false);
+            const int rc_body = body(h->cap_stream, false, false);
             const cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
             if (rc_body != LM_OK) { if (graph) cudaGraphDestroy(graph); return rc_body; }
             LM_CUDA(h, ce);
@@ -138,68 +191,70 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
             h->lz_key = key;
         }
     }
+    int enqueued = 0;
     auto enqueue = [&](int k) -> int {
-        if (use_graph) {
+        const bool with_det = ride && k == 1;           // the first apply carries the deterministic right-hand side
+        if (use_graph && !with_det) {
             LM_CUDA(h, cudaGraphLaunch(h->lz_graph, st));
         } else {
-            const int rc2 = body(st, h->profiling);
+            const int rc2 = body(st, h->profiling, with_det);
             if (rc2 != LM_OK) return rc2;
         }
-        count_apply(h, plan);
+        if (with_det && plan_det.j_splits > 1 && fused(plan_det)) h->n_aux++;    // the deterministic vector's own reduce
+        count_apply(h, with_det ? plan_det : plan);
         h->n_aux += 4 * nv;
+        ++enqueued;
         LM_CUDA(h, cudaEventRecord(h->lz_ev[k & 1], st));
         return LM_OK;
     };
 
-    const bool debug = std::getenv("LM_DEBUG_LANCZOS") != nullptr;   // per-iteration trace on stderr
-    const double breakdown = (h->precision == LM_F32) ? 1e-6 : 1e-14;
-    int k = 0;
+    int k = 0, consumed = 0;
     if (remaining > 0 && (rc = enqueue(1)) != LM_OK) return rc;
     for (k = 1; k <= kmax && remaining > 0; ++k) {
         if (lookahead && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
         LM_CUDA(h, cudaEventSynchronize(h->lz_ev[k & 1]));
+        ++consumed;
+        // this rank's verdicts: bit q = vector q stops at this k (converged, or k == kmax); bit 31 = a failure
+        unsigned word = 0u;
+        int local_fail = LM_OK;
+        std::vector<char> verdict(nv, 0);
         for (int q = 0; q < nv; ++q) {
             if (done[q]) continue;
             const double alpha = ab(q)[2 * k], beta = std::sqrt(std::max((double)ab(q)[2 * k + 1], 0.0));
-            if (!std::isfinite(alpha) || !std::isfinite(beta)) {
-                cudaStreamSynchronize(st);
-                return fail(h, LM_E_CUDA, "Lanczos: non-finite alpha/beta (non-finite input?)");
-            }
-            alphas[q].push_back(alpha);
-            c_cur[q].assign(k, 0.0);
-            if (!tridiag_sqrt_e1(k, alphas[q].data(), betas[q].data(), c_cur[q].data())) {
-                cudaStreamSynchronize(st);
-                return fail(h, LM_E_NOCONV, "Lanczos: tridiagonal eigensolve did not converge");
-            }
-            bool converged = false;
-            if (k >= 2) {
-                // |y_k - y_{k-1}|^2 / |z|^2 = delta^T G_k delta,  |y_{k-1}|^2 / |z|^2 = c_{k-1}^T G_{k-1} c_{k-1}
-                std::vector<double> delta(c_cur[q]);
-                for (int i = 0; i < k - 1; ++i) delta[i] -= c_prev[q][i];
-                double num = 0.0, den = 0.0;
-                for (int i = 0; i < k; ++i)
-                    for (int j = 0; j < k; ++j) num += delta[i] * G[q][(size_t)i * ldg + j] * delta[j];
-                for (int i = 0; i < k - 1; ++i)
-                    for (int j = 0; j < k - 1; ++j) den += c_prev[q][i] * G[q][(size_t)i * ldg + j] * c_prev[q][j];
-                if (std::sqrt(std::max(num, 0.0)) <= tol * std::sqrt(std::max(den, 0.0))) converged = true;
-                if (debug)
-                    std::fprintf(stderr, "[lm lanczos] vec=%d k=%d alpha=%.9e beta=%.9e step=%.3e\n", q, k, alpha, beta, std::sqrt(std::max(num, 0.0) / den));
-            }
-            if (beta <= breakdown * std::fabs(alpha)) converged = true;   // invariant subspace: iterate is exact
-            if (converged || k == kmax) {
+            if (!std::isfinite(alpha) || !std::isfinite(beta)) { local_fail = LM_E_CUDA; word |= 0x80000000u; break; }
+            const LanczosStopper::Verdict v = stop[q].feed(k, alpha, beta);
+            if (v == LanczosStopper::EIGENSOLVE_FAILED) { local_fail = LM_E_NOCONV; word |= 0x80000000u; break; }
+            verdict[q] = v == LanczosStopper::CONVERGED;
+            if (verdict[q]) word |= 1u << q;
+        }
+        const unsigned local_word = word;
+        int rc_x = LM_OK;
+        word = agree_on_stops(local_word, [&](unsigned* wd) { rc_x = broadcast_word(h, wd, st); }, dist && h->dist_ranks > 1);
+        if (rc_x != LM_OK) return rc_x;
+        if ((word | local_word) & 0x80000000u) {
+            cudaStreamSynchronize(st);
+            if (local_fail == LM_E_NOCONV) return fail(h, LM_E_NOCONV, "Lanczos: tridiagonal eigensolve did not converge");
+            if (local_fail == LM_E_CUDA) return fail(h, LM_E_CUDA, "Lanczos: non-finite alpha/beta (non-finite input?)");
+            return fail(h, LM_E_CUDA, "Lanczos: rank 0 reported a failure");
+        }
+        for (int q = 0; q < nv; ++q) {
+            if (done[q]) continue;
+            const bool stops = (word >> q) & 1u;
+            if (stops || k == kmax) {
                 done[q] = 1;
-                conv[q] = converged;
+                conv[q] = stops;
                 kfin[q] = k;
-                c_fin[q] = c_cur[q];
+                c_fin[q] = stop[q].c_cur;
                 --remaining;
                 continue;
             }
-            gram_store(q, k);
-            betas[q].push_back(beta);
-            c_prev[q] = c_cur[q];
+            stop[q].advance();
+            stop[q].set_gram_column(k, hg(q) + (size_t)k * ld);
         }
         if (!lookahead && remaining > 0 && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
     }
+    // a look-ahead iteration enqueued but never consumed did no useful pair evaluations
+    if (enqueued > consumed) h->pairs -= (double)(enqueued - consumed) * (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N;
     // results: y_q = scale |z_q| V_q c_q  (a10)
     bool all_converged = true;
     std::vector<double> coef((size_t)nv * (kmax + 2), 0.0);

@@ -16,7 +16,7 @@
 //   * sources are staged as structure-of-arrays tiles by 1-D TMA bulk copies
 //     (cp.async.bulk.shared::cluster.global, SASS UBLKCP) completing on an mbarrier,
 //     double buffered -- no thread issues a global load in the main loop; a stage is released
-//     without a CTA barrier: every warp counts itself out, the last one out issues the refill;
+//     without a CTA barrier: every warp arrives on the stage's `empty` mbarrier, the last one out issues the refill;
 //   * fp32 arithmetic is packed two targets per instruction (FFMA2 / FMUL2 / FADD2, the
 //     sm_100 f32x2 forms);  1/r from MUFU.RSQ (fp32) or MUFU.RSQ64H + one cubically convergent
 //     correction (fp64);
@@ -164,6 +164,33 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         "bra LM_WAIT_%=;\n\t"
         "LM_DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
+// Consumer release of a stage (the CUTLASS consumer_release / producer_acquire pattern without a dedicated
+// producer): every warp arrives on the stage's `empty` mbarrier once it has read the tile for the last time
+// (mbarrier.arrive has release semantics at CTA scope); the arrival that finds ONE arrival pending in the state it
+// replaced completes the phase.  That warp then observes the completed phase (test_wait: acquire), which orders every
+// warp's generic-proxy reads of the tile before the TMA (async-proxy) refill it goes on to issue.
+__device__ __forceinline__ bool mbar_arrive_is_last(uint64_t* bar)
+{
+    uint64_t state;
+    uint32_t pending;
+    asm volatile("mbarrier.arrive.shared::cta.b64 %0, [%1];" : "=l"(state) : "r"(smem_u32(bar)) : "memory");
+    asm("mbarrier.pending_count.b64 %0, %1;" : "=r"(pending) : "l"(state));
+    return pending == 1u;
+}
+// One non-blocking look at a phase (acquire when it reports completion).  Used by the warp whose own arrival has
+// just completed the phase -- no spin loop, so the compiler keeps the surrounding code convergent.
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0u;
+}
 // 1-D bulk copy global -> shared, completion counted in bytes on `bar` (SASS: UBLKCP)
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
 {
@@ -281,7 +308,7 @@ struct PairKernelTraits {
     static constexpr int NP = TPT / 2;                 // packed target pairs per thread
     static constexpr int ARRAYS = 3 + NV;              // x, y, z + vector components
     static constexpr int STAGE_BYTES = ARRAYS * TJ * (int)sizeof(T);
-    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + STAGES * 8 + STAGES * 8;   // tiles | full mbarriers | done counters
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + STAGES * 8 + STAGES * 8;   // tiles | full mbarriers | empty mbarriers
     static constexpr int TARGETS = BLOCK * TPT;        // targets per CTA
 };
 
@@ -296,7 +323,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
     extern __shared__ __align__(128) unsigned char smem_raw[];
     T* tiles = reinterpret_cast<T*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * Tr::STAGE_BYTES);
-    unsigned int* done = reinterpret_cast<unsigned int*>(full + STAGES);   // warps that finished with a stage (monotonic)
+    uint64_t* empty = full + STAGES;                  // per stage: the BLOCK / 32 warps that have finished with it
     constexpr unsigned int NWARPS = BLOCK / 32;
 
     const int tid = threadIdx.x;
@@ -325,7 +352,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(&full[s], 1);
-            done[s] = 0u;
+            mbar_init(&empty[s], NWARPS);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -408,12 +435,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 #pragma unroll
             for (int k = 0; k < NV; ++k) total[q][k] = add2(total[q][k], acc[q][k]);
 
-        // release the stage without a CTA-wide barrier: every warp counts itself out, the LAST one to
-        // leave refills the stage (TMA) -- no warp ever waits for another except on the data it needs
+        // release the stage without a CTA-wide barrier: every warp arrives on the stage's `empty` mbarrier, the LAST
+        // one to leave refills the stage (TMA) -- no warp ever waits for another except on the data it needs
         __syncwarp();
-        if ((tid & 31) == 0) {
-            const unsigned int left = atomicAdd(&done[stage], 1u) + 1u;
-            if (left % NWARPS == 0u && lt + STAGES < my_tiles) issue(lt + STAGES);
+        if ((tid & 31) == 0 && mbar_arrive_is_last(&empty[stage]) && lt + STAGES < my_tiles) {
+            // the phase was completed by this very arrival: observing it (acquire) orders the other warps' reads first
+            if (mbar_test(&empty[stage], (uint32_t)((lt / STAGES) & 1))) issue(lt + STAGES);
         }
     }
 

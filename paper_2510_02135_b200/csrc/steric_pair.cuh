@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(STERIC_BLOCK, 2) steric_pair_kernel(const Ster
     extern __shared__ __align__(128) unsigned char smem_raw[];
     T* tiles = reinterpret_cast<T*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * 3 * TJ * sizeof(T));
-    unsigned int* done = reinterpret_cast<unsigned int*>(full + STAGES);
+    uint64_t* empty = full + STAGES;                  // per stage: the warps that have finished with it (rpy_pair.cuh mbar_arrive_is_last)
 
     const int tid = threadIdx.x;
     const int64_t i0 = p.i_begin + (int64_t)blockIdx.x * STERIC_TARGETS;
@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(STERIC_BLOCK, 2) steric_pair_kernel(const Ster
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(&full[s], 1);
-            done[s] = 0u;
+            mbar_init(&empty[s], NWARPS);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -126,9 +126,8 @@ __global__ void __launch_bounds__(STERIC_BLOCK, 2) steric_pair_kernel(const Ster
             }
         }
         __syncwarp();
-        if ((tid & 31) == 0) {
-            const unsigned int left = atomicAdd(&done[stage], 1u) + 1u;
-            if (left % NWARPS == 0u && lt + STAGES < my_tiles) issue(lt + STAGES);
+        if ((tid & 31) == 0 && mbar_arrive_is_last(&empty[stage]) && lt + STAGES < my_tiles) {
+            if (mbar_test(&empty[stage], (uint32_t)((lt / STAGES) & 1))) issue(lt + STAGES);   // completed by this arrival: acquire, then refill
         }
     }
 

@@ -44,16 +44,17 @@ __global__ void __launch_bounds__(VEC_BLOCK) pack_rhs_kernel(RhsIn<T> in, int nr
     }
 }
 
-// a6: sum the j-split partials in a fixed order (deterministic) and write interleaved outputs.
+// a6: sum the j-split partials in a fixed order (deterministic) and write interleaved outputs, for the right-hand
+// sides [q_begin, nrhs) (the Lanczos driver reduces its own vectors inside its alpha kernel).
 // One thread per (right-hand side, component, particle): consecutive threads read consecutive
 // addresses of one partial array; the loads of the splits are independent and unrolled.
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) reduce_partials_kernel(const T* __restrict__ partial, int splits, int nrhs, int nc, int64_t i_begin,
-                                                                    int64_t i_end, int64_t npad, RhsOut<T> out)
+__global__ void __launch_bounds__(VEC_BLOCK) reduce_partials_kernel(const T* __restrict__ partial, int splits, int nrhs, int nc, int q_begin,
+                                                                    int64_t i_begin, int64_t i_end, int64_t npad, RhsOut<T> out)
 {
     const int64_t i = i_begin + (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;   // target rows [i_begin, i_end)
     if (i >= i_end) return;
-    const int qk = blockIdx.y, q = qk / nc, k = qk % nc;
+    const int qk = q_begin * nc + blockIdx.y, q = qk / nc, k = qk % nc;          // right-hand sides [q_begin, nrhs): gridDim.y = (nrhs - q_begin) nc
     const size_t stride = (size_t)nrhs * nc * npad;
     const T* p = partial + (size_t)qk * npad + i;
     T s = T(0);
@@ -219,9 +220,9 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_alpha_kernel(T* __restrict_
 // w -= *alpha * V[*newest];  *beta_sq = |w|^2;  host_ab[2(m+1)] = alpha, host_ab[2(m+1)+1] = beta^2 (iteration k = m+1);
 // then, if `advance` is given, *advance += 1 (the index moves to the slot of v_{k+1}; the last vector of a lockstep group does it)
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__ w, const T* __restrict__ V, const int* __restrict__ newest,
+__global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__ w, const T* __restrict__ V, const int* newest,
                                                                  const double* alpha, int64_t n, double* block_partials, unsigned int* ticket,
-                                                                 double* beta_sq, double* host_ab, int* advance)
+                                                                 double* beta_sq, double* host_ab, int* advance)   // `advance` may alias `newest`: neither is __restrict__
 {
     const int m = *newest;
     const T* v = V + (size_t)m * n;

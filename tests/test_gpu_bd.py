@@ -167,13 +167,13 @@ def test_bd_stochastic_step_matches_oracle(lm, torch, prec):
     if prec == "f64":
         o = run_oracle(c, 2, dt, kT, U0, b, tol, False, mode="dense")
         for n in range(2):
-            assert rel(g[n] - x0, o[n] - x0) <= 50 * tol      # vs the exact root (S4 iii)
+            assert rel(g[n] - x0, o[n] - x0) <= 3 * tol       # vs the exact root (S4 iii, default rule)
     else:
         o = run_oracle(c, 2, dt, kT, U0, b, tol, False, mode="lanczos")
         od = run_oracle(c, 2, dt, kT, U0, b, tol, False, mode="dense")
         for n in range(2):
-            assert rel(g[n] - x0, o[n] - x0) <= 10 * tol       # same rule, fp32 vs fp64 (S4 ii)
-            assert rel(g[n] - x0, od[n] - x0) <= 10 * tol      # vs the exact root (S4 iii)
+            assert rel(g[n] - x0, o[n] - x0) <= 3 * tol        # same rule, fp32 vs fp64 (S4 ii)
+            assert rel(g[n] - x0, od[n] - x0) <= 3 * tol       # vs the exact root (S4 iii)
 
 
 def test_bd_single_sphere_diffuses_with_stokes_einstein(lm, torch):
@@ -190,8 +190,8 @@ def test_bd_single_sphere_diffuses_with_stokes_einstein(lm, torch):
 def test_bd_reset_host_variant_and_errors(lm, torch):
     c = case(300, 10.0, 23, "f64")
     dt, U0, b = 1e-3, 4.0, 0.1
-    g = run_gpu(lm, torch, "f64", c, 3, dt, 0.5, U0, b, 1e-8, False)
-    gh = run_gpu(lm, torch, "f64", c, 3, dt, 0.5, U0, b, 1e-8, False, host=True)
+    g = run_gpu(lm, torch, "f64", c, 3, dt, 0.5, U0, b, 1e-4, False)
+    gh = run_gpu(lm, torch, "f64", c, 3, dt, 0.5, U0, b, 1e-4, False, host=True)
     for n in range(3):
         np.testing.assert_array_equal(g[n], gh[n])
     N = 300

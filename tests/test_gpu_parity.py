@@ -23,6 +23,31 @@ def rel(a, b):
     return np.linalg.norm(a - b) / np.linalg.norm(b)
 
 
+def close(a, b, tol):
+    """The M.F gate: rel-L2 <= tol (north_star) AND every element within 8 tol of the largest entry (one bad row
+    in a million passes a norm)."""
+    a = np.asarray(a, dtype=np.float64).reshape(-1)
+    b = np.asarray(b, dtype=np.float64).reshape(-1)
+    return rel(a, b) <= tol and np.abs(a - b).max() <= 8 * tol * np.abs(b).max()
+
+
+def lanczos_gates(rule, prec, it, ko, y, yo, tol, tag=()):
+    """S4(ii): the CUDA path and the fp64 Lanczos oracle run the SAME stopping rule.  Plain Lanczos (no
+    re-orthogonalisation, S15) amplifies rounding differences geometrically once the top Ritz values have converged
+    (k >~ 15-20), and the stop step is a discontinuous function of the steps, so: while the two fp64 recurrences
+    still coincide (k <= 20) the stop step is the oracle's and the iterates agree to 1e-6; beyond that, and in
+    fp32, the stop steps agree within max(2, k/3) (measured: up to +27 % in fp32, whose noisier steps raise the
+    rule's ratio estimate) and the two results -- both within the rule's error of the exact root -- within 2 tol of
+    each other (rule "estimate"; the rule of ref. [35], "step", under-states the error, its iterates at nearby steps
+    differ by the true error: 12 tol at tol >= 1e-3, 50 tol below, as against the dense root)."""
+    if prec == "f64" and ko <= 20:
+        assert it == ko, (tag, it, ko)
+        assert rel(y, yo) <= 1e-6, (tag, rel(y, yo))
+    else:
+        assert abs(it - ko) <= max(2, ko // 3), (tag, it, ko)
+        assert rel(y, yo) <= (2 if rule == "estimate" else (12 if tol >= 1e-3 else 50)) * tol, (tag, it, ko, rel(y, yo))
+
+
 @pytest.fixture(scope="module")
 def lm():
     import paper_2510_02135_b200 as lm
@@ -136,9 +161,9 @@ def test_mdot_batch(lm, torch, prec, angular, nrhs):
     U = U.cpu().numpy().reshape(nrhs, N, 3)
     for q in range(nrhs):
         Uo, Wo = rpy.mdot(pos, F[q], T[q] if angular else None, angular=angular)
-        assert rel(U[q], Uo) <= TOL[prec]
+        assert close(U[q], Uo, TOL[prec])
         if angular:
-            assert rel(W.cpu().numpy().reshape(nrhs, N, 3)[q], Wo) <= TOL[prec]
+            assert close(W.cpu().numpy().reshape(nrhs, N, 3)[q], Wo, TOL[prec])
 
 
 # ---------------------------------------------------------------- the five configs
@@ -146,14 +171,14 @@ def test_config1_full(lm, torch):
     d = workloads.generate(1)
     U, _, s = gpu_mdot(lm, torch, "f64", d["pos"], d["forces"], None, False)
     Uo, _ = rpy.mdot(d["pos"], d["forces"])
-    assert rel(U, Uo) <= 1e-12
+    assert close(U, Uo, 1e-12)
 
 
 def test_config2_full(lm, torch):
     d = workloads.generate(2)
     U, W, s = gpu_mdot(lm, torch, "f32", d["pos"], d["forces"], d["torques"], True)
     Uo, Wo = rpy.mdot(d["pos"], d["forces"], d["torques"], angular=True)
-    assert rel(U, Uo) <= 2e-5 and rel(W, Wo) <= 2e-5
+    assert close(U, Uo, 2e-5) and close(W, Wo, 2e-5)
 
 
 def _sampled_rows(N, n, seed):
@@ -185,7 +210,7 @@ def test_config4_full_size_sampled_rows(lm, torch):
     rows = _sampled_rows(N, 48, 4)
     for q in range(4):
         Uo, _ = rpy.mdot_rows(d["pos"], rows, d["forces"][q])
-        assert rel(U[q][rows], Uo) <= 2e-5
+        assert close(U[q][rows], Uo, 2e-5)
 
 
 def test_config5_full_size_sampled_rows(lm, torch):
@@ -193,15 +218,17 @@ def test_config5_full_size_sampled_rows(lm, torch):
     U, W, s = gpu_mdot(lm, torch, "f64", d["pos"], d["forces"], d["torques"], True)
     rows = _sampled_rows(d["N"], 96, 5)
     Uo, Wo = rpy.mdot_rows(d["pos"], rows, d["forces"], d["torques"], angular=True)
-    assert rel(U[rows], Uo) <= 1e-12 and rel(W[rows], Wo) <= 1e-12
+    assert close(U[rows], Uo, 1e-12) and close(W[rows], Wo, 1e-12)
 
 
 # ---------------------------------------------------------------- Lanczos sqrt(M).W
-def gpu_sqrt(lm, torch, prec, pos, noise, tol, angular, max_iter=None, allow_noconv=False):
+def gpu_sqrt(lm, torch, prec, pos, noise, tol, angular, max_iter=None, allow_noconv=False, rule=None):
     N = pos.shape[0]
     s = lm.Solver(prec, N, 1.0, 1.0, angular)
     if max_iter:
         s.set_max_iter(max_iter)
+    if rule is not None:
+        s.set_option(lm.LM_OPT_LANCZOS_RULE, {"estimate": lm.LM_RULE_ESTIMATE, "step": lm.LM_RULE_STEP}[rule])
     s.set_positions(dev(torch, pos))
     y = torch.empty(3 * N, dtype=s.torch_dtype, device="cuda")
     ya = torch.empty(3 * N, dtype=s.torch_dtype, device="cuda") if angular else None
@@ -225,22 +252,138 @@ def test_lanczos_iterates_match_oracle_step_by_step(lm, torch, prec, angular):
 
 
 @pytest.mark.parametrize("prec,angular", [("f64", False), ("f64", True), ("f32", False), ("f32", True)])
-def test_lanczos_stopping_rule_vs_oracle_lanczos_and_dense(lm, torch, prec, angular):
-    """Gates of DESIGN.md S4.  (i) With the oracle's own stopping rule (relative change of successive
-    iterates, S3) the CUDA path stops at the same step in fp64 and within a few steps in fp32 -- the
-    rule fires at the FIRST crossing of a non-monotone sequence, so it is sensitive to rounding --
-    and the two results agree to O(tol).  (ii) The true error against the exact dense root is
-    <= 10 tol at tol >= 1e-3 (the rule under-states it; measured x1.6-x7.6 here) and <= 50 tol at 1e-5."""
+@pytest.mark.parametrize("rule", ["estimate", "step"])
+def test_lanczos_stopping_rule_vs_oracle_lanczos_and_dense(lm, torch, prec, angular, rule):
+    """Gates of DESIGN.md S4 for both rules of reading S3.  (i) With the same rule on both sides the CUDA path stops
+    at the oracle's step in fp64 and within a few steps in fp32, and the two results agree to O(tol).  (ii) Against
+    the exact dense root: rule "estimate" (default) delivers the requested tolerance within a factor 3 (measured here:
+    0.3 ... 2.1 tol); rule "step"
+    (ref. [35]) under-states the error: <= 10 tol at tol >= 1e-3, <= 50 tol at 1e-5 on this small problem."""
     case = workloads.random_case(400, 14.0, 21, prec, angular, with_noise=True)
     exact = rpy.dense_sqrt_mdot_w(case["pos"], case["noise"], angular=angular)
-    for tol, slack in ((1e-2, 10.0), (1e-3, 10.0), (1e-5, 50.0)):
-        y, it, _ = gpu_sqrt(lm, torch, prec, case["pos"], case["noise"], tol, angular)
-        yo, ko, conv = rpy.lanczos_sqrt_mdot_w(case["pos"], case["noise"], tol, angular=angular)
+    tols = (1e-2, 1e-3, 1e-5) if prec == "f64" else (1e-2, 1e-3, 1e-4)
+    for tol in tols:
+        y, it, s = gpu_sqrt(lm, torch, prec, case["pos"], case["noise"], tol, angular, rule=rule)
+        yo, ko, conv = rpy.lanczos_sqrt_mdot_w(case["pos"], case["noise"], tol, angular=angular, rule=rule)
         assert conv
-        if tol >= 1e-3:
-            assert abs(it - ko) <= (0 if prec == "f64" else max(1, ko // 4)), (tol, it, ko)
-            assert rel(y, yo) <= (1e-6 if prec == "f64" else 10 * tol), (tol, rel(y, yo))
+        lanczos_gates(rule, prec, it, ko, y, yo, tol, tol)
+        slack = 3.0 if rule == "estimate" else (10.0 if tol >= 1e-3 else 50.0)
         assert rel(y, exact) <= slack * tol, (tol, it, rel(y, exact))
+        # the history the library reports is the one it stopped on
+        hist = s.lanczos_history()
+        assert len(hist["alpha"]) == it and np.isnan(hist["step"][0]) and np.all(hist["step"][1:] > 0)
+        if rule == "estimate":
+            assert hist["estimate"][-1] <= tol and np.all(hist["estimate"][2:-1] > tol)
+            assert hist["estimate"][-1] == pytest.approx(rpy.step_error_estimate(hist["step"][1:]), rel=1e-12)
+        else:
+            assert hist["step"][-1] <= tol and np.all(hist["step"][1:-1] > tol) and np.all(np.isnan(hist["estimate"]))
+        s.close()
+
+
+def _memo_apply(pos):
+    """The oracle's O(N^2) apply with a cache keyed on the input vector: the Lanczos oracle called again with a
+    larger max_iter (or another stopping rule) replays the same sequence of applies, each ~20 s at N = 131072."""
+    cache = {}
+
+    def apply(v):
+        key = hash(v.tobytes())
+        if key not in cache:
+            cache[key] = rpy.apply_vec(pos, v)
+        return cache[key]
+    return apply
+
+
+def test_lanczos_large_n_path_fixed_k_iterates_vs_oracle_config3(lm, torch):
+    """The driver path config 3 and bench.py run (N = 131072: direct launches, no look-ahead, the alpha kernel
+    summing the 37 j-split partials) against the fp64 Lanczos oracle: fixed k (max_iter = k, tol unreachable) for
+    k = 2, 4, 6 -- six full O(N^2) oracle applies.  Gates as test_lanczos_iterates_match_oracle_step_by_step."""
+    d = workloads.generate(3)
+    apply = _memo_apply(d["pos"])
+    for k, bound in ((2, 2e-6), (4, 3e-6), (6, 5e-6)):
+        y, it, s = gpu_sqrt(lm, torch, "f32", d["pos"], d["noise"], 1e-30, False, max_iter=k, allow_noconv=True)
+        cfgl = s.pair_launch_config(1)
+        assert cfgl["j_splits"] > 1                         # the fused split-j reduce is on this path
+        yo, ko, conv = rpy.lanczos_sqrt_mdot_w(d["pos"], d["noise"], 1e-30, max_iter=k, apply=apply)
+        assert it == ko == k and not conv
+        assert rel(y, yo) <= bound, (k, rel(y, yo))
+        assert np.abs(y - yo).max() <= 8 * bound * np.abs(yo).max()
+        s.close()
+
+
+def test_hydrodynamic_velocities_config3_vs_oracle(lm, torch):
+    """lm_hydrodynamic_velocities -- the call bench.py times -- at config 3: with max_iter = 3 the result is
+    M.F + prefactor * y_3; the oracle gives M.F on sampled rows (exact for those rows) and y_3 from three full
+    applies.  Also checks that the shared first launch (M.F riding along with the first Lanczos apply, a 2-RHS
+    launch) and the separate launches give the same answer."""
+    d = workloads.generate(3)
+    N, pref = d["N"], 0.37
+    s = lm.Solver("f32", N)
+    s.set_positions(dev(torch, d["pos"]))
+    s.set_max_iter(3)
+    F, z = dev(torch, d["forces"]), dev(torch, d["noise"])
+    H = torch.empty(3 * N, dtype=torch.float32, device="cuda")
+    H2 = torch.empty_like(H)
+    s.reset_stats()
+    with pytest.raises(lm.LmError) as ei:
+        s.hydrodynamic_velocities(F, None, z, pref, 1e-30, H)
+    assert ei.value.code == lm.LM_E_NOCONV                  # the result is still written
+    assert s.get_stats()["pair_kernel_launches"] == 3       # 1 shared 2-RHS launch + 2, not 1 + 3
+    s.set_option(lm.LM_OPT_SHARE_FIRST_APPLY, 0)
+    s.reset_stats()
+    with pytest.raises(lm.LmError):
+        s.hydrodynamic_velocities(F, None, z, pref, 1e-30, H2)
+    assert s.get_stats()["pair_kernel_launches"] == 4
+    torch.cuda.synchronize()
+    H, H2 = H.cpu().numpy().reshape(N, 3), H2.cpu().numpy().reshape(N, 3)
+    assert rel(H, H2) <= 2e-6
+    y3, k3, _ = rpy.lanczos_sqrt_mdot_w(d["pos"], d["noise"], 1e-30, max_iter=3, apply=_memo_apply(d["pos"]))
+    rows = _sampled_rows(N, 192, 33)
+    Uo, _ = rpy.mdot_rows(d["pos"], rows, d["forces"])
+    want = Uo + pref * y3.reshape(N, 3)[rows]
+    assert close(H[rows], want, 2e-5) and close(H2[rows], want, 2e-5)
+    s.close()
+
+
+@pytest.mark.parametrize("rule,tol", [("step", 1e-3), ("estimate", 1e-2)])
+def test_lanczos_large_n_path_stopping_rule_vs_oracle(lm, torch, rule, tol):
+    """N = 65536 at phi = 5 % (config 3's recipe at half size; still the direct-launch path) with the stopping rule on
+    both sides.  The oracle runs the whole fp64 recurrence (~30-40 O(N^2) applies, shared between the two rules
+    through the apply cache).  Gates S4(ii), lanczos_gates above: stop step within max(2, k/3), results within 2 tol
+    ("estimate") of each other; for the rule of ref. [35] ("step") the iterates of nearby steps differ by the true
+    error, measured ~10 tol here, so its gate is the step count and 12 tol."""
+    N = 65536
+    d = workloads.generate(3, N)
+    if not hasattr(test_lanczos_large_n_path_stopping_rule_vs_oracle, "apply"):
+        test_lanczos_large_n_path_stopping_rule_vs_oracle.apply = _memo_apply(d["pos"])
+    y, it, s = gpu_sqrt(lm, torch, "f32", d["pos"], d["noise"], tol, False, rule=rule)
+    assert s.pair_launch_config(1)["j_splits"] > 1
+    yo, ko, conv = rpy.lanczos_sqrt_mdot_w(d["pos"], d["noise"], tol, rule=rule, apply=test_lanczos_large_n_path_stopping_rule_vs_oracle.apply)
+    assert conv
+    lanczos_gates(rule, "f32", it, ko, y, yo, tol, rule)
+    s.close()
+
+
+def test_lanczos_config3_true_error_of_the_default_rule(lm, torch):
+    """What tol means at the headline config: the tol = 1e-3 iterate (default rule, fp32) against a 300-step fp64
+    run of the same CUDA recurrence -- itself checked against the oracle step by step above -- is within 3 tol;
+    the rule of ref. [35] stops ~3x earlier at 15-20 tol (asserted only to be worse, S3/S4)."""
+    d = workloads.generate(3)
+    N = d["N"]
+    s64 = lm.Solver("f64", N)
+    s64.set_positions(dev(torch, d["pos"].astype(np.float64)))
+    s64.set_max_iter(300)
+    yref = torch.empty(3 * N, dtype=torch.float64, device="cuda")
+    s64.sqrt_mdot_w(dev(torch, d["noise"].astype(np.float64)), 1e-9, yref, None, allow_noconv=True)
+    yref = yref.cpu().numpy()
+    s64.close()
+    y, it, s = gpu_sqrt(lm, torch, "f32", d["pos"], d["noise"], 1e-3, False)
+    e_est = rel(y, yref)
+    s.close()
+    ys, its, s = gpu_sqrt(lm, torch, "f32", d["pos"], d["noise"], 1e-3, False, rule="step")
+    e_step = rel(ys, yref)
+    s.close()
+    assert 40 <= it <= 100 and e_est <= 3e-3, (it, e_est)
+    assert its < it and e_step > e_est, (its, e_step)
 
 
 def test_lanczos_square_root_twice_config3_size(lm, torch):
@@ -254,16 +397,16 @@ def test_lanczos_square_root_twice_config3_size(lm, torch):
     y2 = torch.empty_like(z)
     Mz = torch.empty_like(z)
     errs = {}
-    for tol in (1e-3, 1e-4):      # (at this N the iteration needs > 100 steps for 1e-5, in fp64 too)
+    for tol in (1e-2, 3e-3):      # (at this N the default rule needs ~70 steps for 1e-3 and > 100 for 3e-4, in fp64 too)
         it1 = s.sqrt_mdot_w(z, tol, y1)
         it2 = s.sqrt_mdot_w(y1, tol, y2)
         s.mdot(z, None, Mz)
         torch.cuda.synchronize()
         assert 5 < it1 < 100 and 5 < it2 < 100
         errs[tol] = rel(y2.cpu().numpy(), Mz.cpu().numpy())
-    # two applications, each with a true error of up to ~25 tol (S3/S4: the rule under-states it)
-    assert errs[1e-3] <= 50 * 1e-3, errs
-    assert errs[1e-4] <= 50 * 1e-4 and errs[1e-4] < errs[1e-3], errs
+    # two applications, each within ~2 tol of the exact root (default rule, S4)
+    assert errs[1e-2] <= 6 * 1e-2, errs
+    assert errs[3e-3] <= 6 * 3e-3 and errs[3e-3] < errs[1e-2], errs
 
 
 def test_lanczos_exact_cases_and_noconv(lm, torch):
@@ -336,7 +479,7 @@ def test_hydrodynamic_velocities_is_mdot_plus_noise(lm, torch, prec, angular):
     # against the oracle: M.F + pref * Lanczos
     Uo, Wo = rpy.mdot(case["pos"], case["forces"], case["torques"], angular=angular)
     yo, _, _ = rpy.lanczos_sqrt_mdot_w(case["pos"], case["noise"], tol, angular=angular)
-    assert rel(Hl.cpu().numpy(), Uo.reshape(-1) + pref * yo[:3 * N]) <= 10 * tol
+    assert rel(Hl.cpu().numpy(), Uo.reshape(-1) + pref * yo[:3 * N]) <= 2 * tol
     # noise = None: deterministic part only
     s.hydrodynamic_velocities(F, T, None, 0.0, tol, Hl, Ha)
     torch.cuda.synchronize()
@@ -414,7 +557,8 @@ def test_stats_and_launch_config(lm, torch):
     s.mdot(dev(torch, d["forces"]), None, dev(torch, np.empty_like(d["forces"])))
     st = s.get_stats()
     assert st["pair_kernel_launches"] == 1 and st["pair_kernel_ms"] > 0
-    assert lm.lm_probe_fma_peak(lm.LM_F32, 0.05) > 1e13
+    from paper_2510_02135_b200 import probe
+    assert probe.fma_peak(lm.LM_F32, 0.05) > 1e13
 
 
 # ---------------------------------------------------------------- several noise vectors per call
@@ -448,14 +592,13 @@ def test_sqrt_mdot_w_batch_each_vector_matches_oracle(lm, torch, prec, angular, 
         yo, ko, conv = rpy.lanczos_sqrt_mdot_w(case["pos"], W[q], tol, angular=angular)
         exact = rpy.dense_sqrt_mdot_w(case["pos"], W[q], angular=angular)
         assert conv
-        assert abs(iters[q] - ko) <= (0 if prec == "f64" else max(1, ko // 4)), (q, iters[q], ko)
-        assert rel(y, yo) <= (1e-6 if prec == "f64" else 10 * tol), (q, rel(y, yo))
-        assert rel(y, exact) <= 10 * tol, (q, rel(y, exact))
+        lanczos_gates("estimate", prec, iters[q], ko, y, yo, tol, q)
+        assert rel(y, exact) <= 3 * tol, (q, rel(y, exact))
     # the single-vector call gives the same answer for vector 0 (up to the pair kernel's summation order)
     y1, it1, _ = gpu_sqrt(lm, torch, prec, case["pos"], W[0], tol, angular)
     y0 = lin[0] if not angular else np.concatenate([lin[0], ang[0]])
-    assert abs(it1 - iters[0]) <= (0 if prec == "f64" else 1)
-    assert rel(y0, y1) <= (1e-10 if prec == "f64" else 5 * tol)
+    assert abs(it1 - iters[0]) <= (1 if prec == "f64" else max(2, it1 // 4)), (it1, iters[0])
+    assert rel(y0, y1) <= (1e-5 if prec == "f64" else 2 * tol), rel(y0, y1)
     s.close()
 
 
@@ -580,9 +723,9 @@ def test_seeded_sweep_of_sizes_and_shapes(lm, torch):
         for q in range(nrhs):
             Uo, Wo = rpy.mdot(pos, F[q], None if T is None else T[q], angular=angular)
             tag = (case_id, N, prec, angular, nrhs, q, side)
-            assert rel(U[q], Uo) <= TOL[prec], tag
+            assert close(U[q], Uo, TOL[prec]), tag
             if angular:
-                assert rel(W[q], Wo) <= TOL[prec], tag
+                assert close(W[q], Wo, TOL[prec]), tag
         s.close()
 
 
