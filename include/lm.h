@@ -8,6 +8,8 @@
  *   -----------------------------------------------  ---------------------------------
  *   NBody("open","open","open") + initialize(         lm_create
  *     viscosity, hydrodynamicRadius, includeAngular)
+ *   NBody("open","open","single_wall") +              lm_create + lm_set_wall
+ *     setParameters(wallHeight)
  *   setPositions                                      lm_set_positions
  *   Mdot(forces, torques) -> (linear, angular)        lm_mdot, lm_mdot_batch
  *   sqrtMdotW()           -> (linear, angular)        lm_sqrt_mdot_w
@@ -76,6 +78,20 @@ enum {
  * order one; in fp32 use such units for the angular noise. */
 int lm_create(lm_solver** out, int precision, int64_t N, double eta, double a, int include_angular);
 int lm_destroy(lm_solver* h);
+
+/* Geometry ("open","open","single_wall") of the paper's NBody solver: a no-slip wall in
+ * the plane z = wall_height, fluid above it (setParameters(wallHeight)).  enabled = 0 returns to
+ * open boundaries.  Every entry point then works with the single-wall mobility
+ *     M~ = B M(x~) B,
+ * M = free-space RPY blocks + the wall correction of the "Swan-Brady kernel" (ref. [37]): the Faxen operators
+ * applied to the image part of the half-space Green's function, which is eq. (8) exactly for spheres that do not
+ * cut the wall (closed forms: DESIGN.md appendix A); x~ = the positions with every height above the wall raised to at
+ * least a, B = diag(b_i) on all six components of particle i, b_i = min(1, max(h_i, 0)/a) -- the "damping matrix
+ * approach" that keeps M~ symmetric positive (semi-)definite and takes a particle's mobility to zero continuously
+ * as it reaches the wall (readings S18-S20).  lm_thermal_drift_rfd then estimates a
+ * non-zero drift, lm_steric_forces / lm_bd_step add the particle-wall repulsion of eq. (13) with
+ * r = height of the centre and d = a.  Call before lm_set_positions (it invalidates the positions). */
+int lm_set_wall(lm_solver* h, int enabled, double wall_height);
 
 /* Store the particle positions (3N).  The library keeps its own packed copy; `pos` may be reused
  * by the caller as soon as the stream has passed this call. */

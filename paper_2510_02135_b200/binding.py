@@ -28,6 +28,7 @@ _lib = None
 SIGNATURES = {
     "lm_create": (c_int, [POINTER(c_void_p), c_int, c_int64, c_double, c_double, c_int]),
     "lm_destroy": (c_int, [c_void_p]),
+    "lm_set_wall": (c_int, [c_void_p, c_int, c_double]),
     "lm_set_positions": (c_int, [c_void_p, c_void_p, c_void_p]),
     "lm_mdot": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "lm_mdot_batch": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
@@ -177,6 +178,10 @@ class Solver:
             self.close()
         except Exception:
             pass
+
+    def set_wall(self, enabled: bool, wall_height: float = 0.0):
+        """Geometry ("open","open","single_wall") with the wall at z = wall_height."""
+        self._check(lib().lm_set_wall(self._h, int(bool(enabled)), float(wall_height)))
 
     # -- device entry points (torch CUDA tensors)
     def set_positions(self, pos, stream=None):

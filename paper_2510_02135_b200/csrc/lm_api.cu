@@ -35,7 +35,7 @@ namespace {
 // ---------------------------------------------------------------- typed front ends
 template <typename T> int set_positions_t(lm_solver* h, const void* pos, cudaStream_t st)
 {
-    pack_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)pos, h->N, h->npad, (T)h->len_scale, (T*)h->pos_soa);
+    pack_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)pos, h->N, h->npad, (T)h->len_scale, wall_pack<T>(h), (T*)h->pos_soa);
     h->n_aux++;
     LM_CUDA(h, cudaGetLastError());
     h->have_pos = true;
@@ -102,7 +102,7 @@ int lm_create(lm_solver** out, int precision, int64_t N, double eta, double a, i
     auto bail = [&](int code) { lm_destroy(h); return code; };
     if (cudaGetDevice(&h->device) != cudaSuccess) return bail(LM_E_CUDA);
     if (cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess) return bail(LM_E_CUDA);
-    if (cudaMalloc(&h->pos_soa, (size_t)3 * h->npad * esize(h)) != cudaSuccess) return bail(LM_E_CUDA);
+    if (cudaMalloc(&h->pos_soa, (size_t)POS_ARRAYS * h->npad * esize(h)) != cudaSuccess) return bail(LM_E_CUDA);
     const int rc = precision == LM_F32 ? init_variants<float>(h) : init_variants<double>(h);
     if (rc != LM_OK) return bail(rc);
     *out = h;
@@ -154,6 +154,19 @@ int lm_set_max_iter(lm_solver* h, int max_iter)
 }
 
 int lm_last_iterations(const lm_solver* h) { return h ? h->last_iters : -1; }
+
+int lm_set_wall(lm_solver* h, int enabled, double wall_height)
+{
+    if (!h) return LM_E_NULL;
+    h->err.clear();
+    if (!std::isfinite(wall_height)) return fail(h, LM_E_INVALID, "wall_height must be finite");
+    h->wall = enabled ? 1 : 0;
+    h->wall_z = wall_height;
+    h->have_pos = false;                              // the packed copy (raised heights, damping factors) depends on the wall
+    h->bd_have_prev = false;
+    for (auto& slot : h->plan_cache) slot.valid = false;
+    return LM_OK;
+}
 
 int lm_set_option(lm_solver* h, int option, int value)
 {

@@ -50,6 +50,7 @@ int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>&
     p.vec = (const T*)h->vec_soa;
     p.out = kout;
     p.partial = (T*)h->partial;
+    p.damp = damp_of<T>(h);
     p.N = h->N;
     p.i_begin = h->row_begin;
     p.i_end = h->row_end;
@@ -114,14 +115,14 @@ template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& i
     int rc = prepare_apply<T>(h, nrhs, plan);
     if (rc != LM_OK) return rc;
     auto direct = [&](cudaStream_t s2, bool timed) -> int {
-        pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(in, nrhs, nc, h->N, h->npad, (T)h->len_scale, (T*)h->vec_soa);
+        pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(in, nrhs, nc, h->N, h->npad, (T)h->len_scale, damp_of<T>(h), (T*)h->vec_soa);
         return launch_pair<T>(h, nrhs, plan, out, s2, timed);
     };
     // A short apply is bound by the host's three launches (~11 us measured against ~3 us of kernels each): when
     // the SAME call (same buffers, same plan) comes twice in a row -- a time-stepping loop -- it is captured
     // once and replayed as a CUDA graph from then on; any other call is launched directly.
     const double cost = (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N * (h->angular ? 2.3 : 1.0) *
-                        (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nrhs);
+                        (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nrhs) * (h->wall ? 3.4 : 1.0);
     if (cost < 2.0e8 && !h->profiling && h->dist_ranks == 0 && h->graph_replay) {      // N <~ 14000 fp32
         lm_solver::ApplyKey key;
         std::memset(&key, 0, sizeof key);

@@ -31,6 +31,7 @@ int steric_device(lm_solver* h, double U0, double b, const T* ext, T* out, cudaS
     const double K = sizeof(T) == 4 ? 20.0 : 40.0;           // exp(-K) below the type's epsilon
     StericParams<T> p;
     p.pos = (const T*)h->pos_soa;
+    p.z_array = h->wall ? 3 : 2;                             // the forces act at the true heights, not the raised ones
     p.partial = (T*)h->partial;
     p.N = h->N;
     p.npad = h->npad;
@@ -45,7 +46,9 @@ int steric_device(lm_solver* h, double U0, double b, const T* ext, T* out, cudaS
     p.inv_b = (T)(sizeof(T) == 4 ? 1.4426950408889634 / bs : 1.0 / bs);
     if (i_tiles > 0) {
         steric_pair_kernel<T><<<dim3(i_tiles, splits), STERIC_BLOCK, steric_smem_bytes<T>(), st>>>(p);
-        steric_reduce_kernel<T><<<grid_1d(rows), VEC_BLOCK, 0, st>>>((const T*)h->partial, splits, h->row_begin, h->row_end, h->npad, ext, kout);
+        // particle-wall repulsion: eq. (13) with d = a, heights in the internal unit
+        steric_reduce_kernel<T><<<grid_1d(rows), VEC_BLOCK, 0, st>>>((const T*)h->partial, splits, h->row_begin, h->row_end, h->npad, ext, kout,
+                                                                     h->wall ? (const T*)h->pos_soa + (size_t)3 * h->npad : nullptr, (T)as, (T)(U0 / b), (T)(1.0 / bs));
         h->n_aux += 2;
     }
     LM_CUDA(h, cudaGetLastError());
@@ -64,13 +67,13 @@ int rfd_device(lm_solver* h, const T* W, double delta, T* lin_out, T* ang_out, c
 {
     const int64_t n3 = 3 * h->N;
     int rc;
-    if ((rc = ensure(h, &h->rfd[0], &h->rfd_bytes[0], (size_t)3 * h->npad * sizeof(T))) != LM_OK) return rc;
+    if ((rc = ensure(h, &h->rfd[0], &h->rfd_bytes[0], (size_t)POS_ARRAYS * h->npad * sizeof(T))) != LM_OK) return rc;
     if ((rc = ensure(h, &h->rfd[1], &h->rfd_bytes[1], (size_t)n3 * sizeof(T))) != LM_OK) return rc;
     if (h->angular && (rc = ensure(h, &h->rfd[2], &h->rfd_bytes[2], (size_t)n3 * sizeof(T))) != LM_OK) return rc;
     void* const home = h->pos_soa;
     T* outs[2][2] = {{lin_out, ang_out}, {(T*)h->rfd[1], (T*)h->rfd[2]}};
     for (int side = 0; side < 2; ++side) {
-        shift_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)home, W, h->N, h->npad, (T)((side ? -0.5 : 0.5) * delta * h->len_scale), (T*)h->rfd[0]);
+        shift_positions_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>((const T*)home, W, h->N, h->npad, (T)((side ? -0.5 : 0.5) * delta * h->len_scale), wall_pack<T>(h), (T*)h->rfd[0]);
         h->n_aux++;
         h->pos_soa = h->rfd[0];                       // the apply reads the displaced copy; the handle's positions are untouched
         rc = apply_batch<T>(h, 1, W, nullptr, outs[side][0], h->angular ? outs[side][1] : nullptr, st);

@@ -19,19 +19,20 @@ template <typename T> struct Variant {
     int nrhs, ang, block, tpt, tj, sub, smem;
     int ctas_per_sm;      // filled at first use (occupancy API)
     double efficiency;    // relative per-pair throughput used by the launch chooser
+    int wall;             // 1: the single-wall variant (free-space pair + wall correction)
 };
 
-template <typename T, int NRHS, bool ANG, int TPT, int SUB, int MINB> Variant<T> make_large()
+template <typename T, int NRHS, bool ANG, int TPT, int SUB, int MINB, bool WALL = false> Variant<T> make_large()
 {
     using Tr = PairKernelTraits<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB>;
     static_assert(NPAD_QUANTUM % SUB == 0, "every SUB divides NPAD_QUANTUM");
-    return {rpy_pair_kernel<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB, MINB>, NRHS, ANG, L_BLOCK, TPT, L_TJ, SUB, Tr::SMEM_BYTES, 0, 1.0};
+    return {rpy_pair_kernel<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB, MINB, WALL>, NRHS, ANG, L_BLOCK, TPT, L_TJ, SUB, Tr::SMEM_BYTES, 0, 1.0, WALL};
 }
-template <typename T, int NRHS, bool ANG, int SUB, int MINB> Variant<T> make_small()
+template <typename T, int NRHS, bool ANG, int SUB, int MINB, bool WALL = false> Variant<T> make_small()
 {
     using Tr = PairKernelTraits<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB>;
     static_assert(NPAD_QUANTUM % SUB == 0, "every SUB divides NPAD_QUANTUM");
-    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB, MINB>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, SUB, Tr::SMEM_BYTES, 0, 0.8};
+    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB, MINB, WALL>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, SUB, Tr::SMEM_BYTES, 0, 0.8, WALL};
 }
 
 template <typename T> std::vector<Variant<T>> build_variants();
@@ -40,14 +41,23 @@ template <> std::vector<Variant<float>> build_variants<float>()
     return {make_large<float, 1, false, 4, 32, 2>(), make_large<float, 2, false, 4, 32, 1>(), make_large<float, 4, false, 4, 32, 1>(),
             make_large<float, 1, true, 2, 32, 2>(),  make_large<float, 2, true, 2, 32, 1>(),
             make_small<float, 1, false, 32, 8>(), make_small<float, 2, false, 32, 8>(), make_small<float, 4, false, 32, 6>(),
-            make_small<float, 1, true, 32, 8>(),  make_small<float, 2, true, 32, 6>()};
+            make_small<float, 1, true, 32, 8>(),  make_small<float, 2, true, 32, 6>(),
+            // single wall (the wall correction roughly triples the per-pair work and the live registers)
+            make_large<float, 1, false, 2, 32, 2, true>(), make_large<float, 2, false, 2, 32, 1, true>(),
+            make_large<float, 1, true, 2, 32, 1, true>(),  make_large<float, 2, true, 2, 32, 1, true>(),
+            make_small<float, 1, false, 32, 6, true>(), make_small<float, 2, false, 32, 6, true>(),
+            make_small<float, 1, true, 32, 4, true>(),  make_small<float, 2, true, 32, 4, true>()};
 }
 template <> std::vector<Variant<double>> build_variants<double>()
 {
     return {make_large<double, 1, false, 4, 32, 1>(), make_large<double, 2, false, 2, 32, 1>(), make_large<double, 4, false, 2, 32, 1>(),
             make_large<double, 1, true, 2, 32, 1>(),  make_large<double, 2, true, 2, 32, 1>(),
             make_small<double, 1, false, 32, 8>(), make_small<double, 2, false, 32, 6>(), make_small<double, 4, false, 32, 4>(),
-            make_small<double, 1, true, 32, 6>(),  make_small<double, 2, true, 32, 4>()};
+            make_small<double, 1, true, 32, 6>(),  make_small<double, 2, true, 32, 4>(),
+            make_large<double, 1, false, 2, 32, 1, true>(), make_large<double, 2, false, 2, 32, 1, true>(),
+            make_large<double, 1, true, 2, 32, 1, true>(),  make_large<double, 2, true, 2, 32, 1, true>(),
+            make_small<double, 1, false, 32, 4, true>(), make_small<double, 2, false, 32, 4, true>(),
+            make_small<double, 1, true, 32, 3, true>(),  make_small<double, 2, true, 32, 2, true>()};
 }
 
 struct LaunchPlan {
@@ -109,6 +119,8 @@ struct lm_solver {
     double eta = 1.0, a = 1.0;
     double len_scale = 1.0;    // power of two nearest 1/a: lengths are stored x len_scale, so the kernels see a radius in [0.71, 1.41]
     int angular = 0;
+    int wall = 0;              // geometry ("open","open","single_wall"): lm_set_wall
+    double wall_z = 0.0;       // the wall is the plane z = wall_z, fluid above (the paper's setParameters(wallHeight))
     int max_iter = 100;
     int lz_rule = lm::RULE_ESTIMATE;   // Lanczos stopping rule (reading S3; LM_OPT_LANCZOS_RULE)
     bool graph_replay = true;          // short applies / Lanczos iterations replayed as CUDA graphs (LM_OPT_GRAPH_REPLAY)
@@ -247,6 +259,9 @@ template <typename T> PairConsts<T> make_consts(double eta, double a, double len
     c.k6 = (T)(-3.0 / (16.0 * a * a * a * a));
     c.C1_lin = (T)(len_scale / (8.0 * pi * eta));                  // Oseen prefactor, applied once per target
     c.C1_ang = (T)(len_scale * len_scale / (8.0 * pi * eta));
+    c.wa2 = (T)(a * a);
+    c.wzz0 = (T)(-8.0 * a * a / 3.0);
+    c.wzz1 = (T)(20.0 * a * a);
     return c;
 }
 
@@ -282,7 +297,7 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
     double best_cost = 1e300;
     for (int vi = 0; vi < (int)vs.size(); ++vi) {
         const auto& v = vs[vi];
-        if (v.nrhs != nrhs || v.ang != h->angular) continue;
+        if (v.nrhs != nrhs || v.ang != h->angular || v.wall != h->wall) continue;
         const int targets = v.block * v.tpt;
         const int64_t rows = std::max<int64_t>(h->row_end - h->row_begin, 0);          // target rows of this rank / call
         const int i_tiles = (int)((rows + targets - 1) / targets);
@@ -305,7 +320,7 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
             cost += 0.1 * (rem ? wave(rem_per_sm) : wave(v.ctas_per_sm));
             // cost is in pairs evaluated back to back on one SM (~1e4 per microsecond): the reduce pass
             // adds a ~3 us launch plus writing and re-reading s partial vectors
-            if (s > 1) cost += 3.0e4 + 0.1 * (double)s * (double)rows;
+            if (s > 1) cost += (3.0e4 + 0.1 * (double)s * (double)rows) / (h->wall ? 3.4 : 1.0);   // (a wall pair costs ~3.4 free-space pairs)
             if (cost < best_cost) {
                 best_cost = cost;
                 best.variant = vi;
@@ -336,6 +351,11 @@ cudaEvent_t get_event(lm_solver* h)
     cudaEventCreate(&e);
     return e;
 }
+
+// single wall: the damping factors b (array 4 of the packed positions), and how the packers raise heights
+template <typename T> const T* damp_of(const lm_solver* h) { return h->wall ? (const T*)h->pos_soa + (size_t)4 * h->npad : nullptr; }
+template <typename T> WallPack<T> wall_pack(const lm_solver* h) { return {h->wall, (T)h->wall_z, (T)(h->a * h->len_scale)}; }
+constexpr int POS_ARRAYS = 5;    // x | y | z (raised height with a wall) | height | damping factor  (the last two only with a wall)
 
 int grid_1d(int64_t n) { return (int)std::max<int64_t>(1, (n + VEC_BLOCK - 1) / VEC_BLOCK); }
 int grid_red(int64_t n) { return (int)std::min<int64_t>(RED_MAX_BLOCKS, std::max<int64_t>(1, (n + VEC_BLOCK - 1) / VEC_BLOCK)); }

@@ -94,7 +94,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     auto new_vectors = [&](const T* x, int which_scal, cudaStream_t s2) {
         for (int q = 0; q < nv; ++q) {
             lanczos_scale_pack_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, s2>>>(x + (size_t)q * dof, h->N, h->npad, nc, (T)h->len_scale, scal(q) + which_scal, h->d_newest,
-                                                                              Vq(q), soa(q));
+                                                                              Vq(q), soa(q), damp_of<T>(h));
             gram_column_kernel<T><<<dim3(gg, kmax + 1), VEC_BLOCK, 0, s2>>>(Vq(q), dof, h->d_newest, gchunk, h->d_gram_part, h->d_ticket,
                                                                              h->h_gram + (size_t)q * ld * ld, ld);
         }
@@ -110,7 +110,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
         RhsIn<T> din{};
         din.f[0] = det->f;
         din.t[0] = det->t;
-        pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>(din, 1, nc, h->N, h->npad, (T)h->len_scale, soa(nv));
+        pack_rhs_kernel<T><<<grid_1d(h->npad), VEC_BLOCK, 0, st>>>(din, 1, nc, h->N, h->npad, (T)h->len_scale, damp_of<T>(h), soa(nv));
         h->n_aux++;
     }
     h->n_aux += 3 * nv;
@@ -171,7 +171,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     // wasted apply at convergence, so it is used only where an apply costs less than the round trips it
     // saves (~25 iterations x 50 us); the same regime is launch-bound, so there the body runs as a graph.
     // Row-sharded runs agree on the verdict through the stream after every iteration: no look-ahead there.
-    const double apply_cost = (double)h->N * (double)h->N * (h->angular ? 2.3 : 1.0) * (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nv);
+    const double apply_cost = (double)h->N * (double)h->N * (h->angular ? 2.3 : 1.0) * (h->precision == LM_F64 ? 2.5 : 1.0) * (0.6 + 0.4 * nv) * (h->wall ? 3.4 : 1.0);
     const bool dist = h->dist_ranks > 0;
     const bool lookahead = apply_cost < 2.0e9 && !dist;
     const bool use_graph = lookahead && !h->profiling && h->graph_replay;

@@ -64,6 +64,7 @@ __device__ __forceinline__ P2<double> add2(P2<double> a, P2<double> b) { return 
 // scalar-broadcast forms (the scalar is a source quantity or a constant, identical for both targets)
 template <typename T> __device__ __forceinline__ P2<T> fma2(P2<T> a, T s, P2<T> c) { return fma2(a, splat(s), c); }
 template <typename T> __device__ __forceinline__ P2<T> fma2(P2<T> a, T s, T c) { return fma2(a, splat(s), splat(c)); }
+template <typename T> __device__ __forceinline__ P2<T> fma2(P2<T> a, P2<T> b, T c) { return fma2(a, b, splat(c)); }
 template <typename T> __device__ __forceinline__ P2<T> mul2(P2<T> a, T s) { return mul2(a, splat(s)); }
 template <typename T> __device__ __forceinline__ P2<T> add2(P2<T> a, T s) { return add2(a, splat(s)); }
 
@@ -108,6 +109,7 @@ template <typename T> struct PairConsts {
     T c2, nc3, c4, nc5, c6;               // translation-translation
     T c8, k1, k2, k3, k4, k5, k6;         // rotation-rotation and coupling (near branch)
     T C1_lin, C1_ang;                     // 1/(8 pi eta) x the internal length unit (x its square): applied in the epilogue
+    T wa2, wzz0, wzz1;                    // single-wall correction: a^2, -8 a^2/3, 20 a^2 (wall_apply)
 };
 
 // overlap detector of the far-field fast path: running minimum of r^2 over a group of pairs.
@@ -135,6 +137,8 @@ template <typename T> struct PairParams {
     const T* __restrict__ vec;  // [nrhs*NC][npad] packed right-hand sides, ghosts are zeros
     RhsOut<T> out;              // j_splits == 1: per right-hand side, 3N interleaved each
     T* __restrict__ partial;    // j_splits  > 1: [j_splits][nrhs*NC][npad]
+    const T* __restrict__ damp; // single wall: damping factors b_i [npad] (ghosts 0), applied to the targets in the epilogue
+                                // (the packed right-hand sides already carry b_j); pos z = raised height above the wall
     int64_t N;
     int64_t i_begin, i_end;     // target rows handled by this launch: [i_begin, i_end) (whole problem: [0, N));
                                 // i-tile b covers i_begin + b * TARGETS ...  (row-sharded applies)
@@ -290,6 +294,95 @@ __device__ __forceinline__ void pair_apply(const PairConsts<T>& c, const PairGeo
     }
 }
 
+// ---------------------------------------------------------------- single wall
+// The correction by which a no-slip wall at height 0 changes the pair mobility (the "Swan-Brady kernel"
+// of ref. [37]): the Faxen operators applied to the image part of the half-space Green's function, DESIGN.md
+// appendix A (closed forms) and reading S18; heights are >= a (reading S19: raised before packing), so the image
+// distance |R| >= 2a, the forms are smooth and there is no near/far select.  Notation: R = x_i - x_j*,
+// D = -R = (dx, dy, nZ) with nZ = -(z_i + z_j), h = z_j, u = 1/|R|^2, i1 = 1/|R|, i3 = i1 u, t = Z^2 u, p = a^2 u,
+// w = z_i z_j u; everything "/ C1" like the free-space scalars.  |R|^2 = r^2 + 4 z_i z_j.
+//   translation:  U += tI F + D (tRR q - tRz F_z) + zhat (tzz F_z - tzR q),   q = D.F
+//     tI  = i1 [-1 - 2w + p (-2/3 + 2t)  + p^2 (2/3 - 10/3 t)]      tRz = i3 [2h - nZ (-12w + p (-4 + 20t) + p^2 (40/3 - 140/3 t))]
+//     tRR = i3 [-1 + 6w + p (2 - 10t)    + p^2 (-10/3 + 70/3 t)]    tzR = i3 [2h + 20/3 p^2 nZ]
+//     tzz = i3 [-4h^2 + p (-4 Z^2 - 8/3 a^2 + 20 a^2 t)]
+//   rotation:     W += rI T + D (rRR s - rRz T_z) + zhat (rzz T_z - rzR s),   s = D.T,  i5 = i3 u
+//     rI = i3 (7/2 - 6t)   rRR = -9/2 i5   rRz = -3 nZ i5   rzR = -6 nZ i5   rzz = -3 i3
+//   coupling w <- F:  W += B (zhat x F) + P S + zhat i3 (dy F_x - dx F_y),   P = (-dy, dx, 0),  S = -C q + Dc F_z
+//     B = i3 [-dz - 2p nZ]     -C = i5 [6h + 10 p nZ]     Dc = i3 [1 - 12 h nZ u + p (2 - 20t)]
+//   coupling u <- T (the transpose of the block of the swapped pair):  m = dy T_x - dx T_y
+//     U += B' (T_y, -T_x, 0) + (dx, dy, -nZ) C' m + zhat D' m + i3 (-dy, dx, 0) T_z
+//     B' = i3 [dz - 2p nZ]     C' = i5 [-6 z_i - 10 p nZ]     D' = i3 [1 + 12 z_i (-nZ) u ... ] = i3 [1 + 12 nz nZ u + p (2 - 20t)], nz = -z_i
+// nz = -z_i and nz4 = 4 z_i are per-target registers; zj, V[] the warp-uniform source.
+template <typename T, int NRHS, bool ANG>
+__device__ __forceinline__ void wall_apply(const PairConsts<T>& c, const PairGeom<T>& gm, P2<T> nz, P2<T> z4, T zj, const T (&V)[NRHS * (ANG ? 6 : 3)],
+                                           P2<T> (&acc)[NRHS * (ANG ? 6 : 3)])
+{
+    constexpr int NC = ANG ? 6 : 3;
+    const P2<T> dx = gm.dx, dy = gm.dy;
+    const T h = zj, h2 = zj + zj;
+    const P2<T> nZ = add2(nz, -h);
+    const P2<T> R2 = fma2(z4, h, gm.r2);
+    const P2<T> i1 = rsqrt2(R2);
+    const P2<T> u = mul2(i1, i1), i3 = mul2(i1, u);
+    const P2<T> Z2 = mul2(nZ, nZ), t = mul2(Z2, u), p = mul2(u, c.wa2), p2 = mul2(p, p);
+    const P2<T> w = mul2(mul2(nz, -h), u);
+    const P2<T> tI = mul2(i1, fma2(p2, fma2(t, T(-10.0 / 3.0), T(2.0 / 3.0)), fma2(p, fma2(t, T(2), T(-2.0 / 3.0)), fma2(w, T(-2), T(-1)))));
+    const P2<T> tRR = mul2(i3, fma2(p2, fma2(t, T(70.0 / 3.0), T(-10.0 / 3.0)), fma2(p, fma2(t, T(-10), T(2)), fma2(w, T(6), T(-1)))));
+    const P2<T> inner = fma2(p2, fma2(t, T(-140.0 / 3.0), T(40.0 / 3.0)), fma2(p, fma2(t, T(20), T(-4)), mul2(w, T(-12))));
+    const P2<T> ntRz = mul2(i3, fma2(nZ, inner, -h2));                              // -tRz
+    const P2<T> ntzR = mul2(i3, fma2(mul2(p2, T(-20.0 / 3.0)), nZ, -h2));            // -tzR
+    const P2<T> tzz = mul2(i3, fma2(p, fma2(Z2, T(-4), fma2(t, c.wzz1, c.wzz0)), T(-4) * h * h));
+    if constexpr (!ANG) {
+#pragma unroll
+        for (int q = 0; q < NRHS; ++q) {
+            const T Fx = V[q * NC + 0], Fy = V[q * NC + 1], Fz = V[q * NC + 2];
+            const P2<T> qF = fma2(nZ, Fz, fma2(dy, Fy, mul2(dx, Fx)));
+            const P2<T> A = fma2(tRR, qF, mul2(ntRz, Fz));
+            const P2<T> B = fma2(tzz, Fz, mul2(ntzR, qF));
+            acc[q * NC + 0] = fma2(tI, Fx, fma2(dx, A, acc[q * NC + 0]));
+            acc[q * NC + 1] = fma2(tI, Fy, fma2(dy, A, acc[q * NC + 1]));
+            acc[q * NC + 2] = fma2(tI, Fz, fma2(nZ, A, add2(B, acc[q * NC + 2])));
+        }
+    } else {
+        const P2<T> dz = gm.dz;
+        const P2<T> i5 = mul2(i3, u);
+        const P2<T> pz = mul2(p, nZ);                                               // p nZ
+        const P2<T> poly = fma2(t, T(-20), T(2));                                   // 2 - 20 t
+        const P2<T> rI = mul2(i3, fma2(t, T(-6), T(3.5)));
+        const P2<T> cB = mul2(i3, fma2(pz, T(-2), mul2(dz, T(-1))));                // B  = i3 (-dz - 2 p nZ)
+        const P2<T> cBp = mul2(i3, fma2(pz, T(-2), dz));                            // B' = i3 ( dz - 2 p nZ)
+        const P2<T> nC = mul2(i5, fma2(pz, T(10), T(6) * h));                       // -C = i5 (6h + 10 p nZ)
+        const P2<T> cCp = mul2(i5, fma2(pz, T(-10), mul2(nz, T(6))));               // C' = i5 (6 nz - 10 p nZ)
+        const P2<T> nzu = mul2(nZ, u);
+        const P2<T> cD = mul2(i3, fma2(p, poly, fma2(nzu, T(-12) * h, T(1))));      // Dc = i3 (1 - 12 h nZ u + p (2 - 20t))
+        const P2<T> cDp = mul2(i3, fma2(p, poly, fma2(mul2(nzu, nz), T(12), T(1))));// D' = i3 (1 + 12 nz nZ u + p (2 - 20t))
+        const P2<T> zC = fma2(nZ, mul2(cCp, T(-1)), cDp);                           // Z C' + D' = -nZ C' + D'
+#pragma unroll
+        for (int q = 0; q < NRHS; ++q) {
+            const T Fx = V[q * NC + 0], Fy = V[q * NC + 1], Fz = V[q * NC + 2];
+            const T Tx = V[q * NC + 3], Ty = V[q * NC + 4], Tz = V[q * NC + 5];
+            const P2<T> qF = fma2(nZ, Fz, fma2(dy, Fy, mul2(dx, Fx)));
+            const P2<T> qT = fma2(nZ, Tz, fma2(dy, Ty, mul2(dx, Tx)));
+            const P2<T> A = fma2(tRR, qF, mul2(ntRz, Fz));
+            const P2<T> B = fma2(tzz, Fz, mul2(ntzR, qF));
+            const P2<T> m = fma2(dy, Tx, mul2(dx, -Ty));                            // P'.T = dy T_x - dx T_y
+            const P2<T> Cm = mul2(cCp, m);
+            const P2<T> i3Tz = mul2(i3, Tz);
+            // U += tI F + D A + zhat B + [B' T_y + dx C'm - dy i3 T_z,  -B' T_x + dy C'm + dx i3 T_z,  (Z C' + D') m]
+            acc[q * NC + 0] = fma2(dy, mul2(i3Tz, T(-1)), fma2(dx, Cm, fma2(cBp, Ty, fma2(tI, Fx, fma2(dx, A, acc[q * NC + 0])))));
+            acc[q * NC + 1] = fma2(dx, i3Tz, fma2(dy, Cm, fma2(cBp, -Tx, fma2(tI, Fy, fma2(dy, A, acc[q * NC + 1])))));
+            acc[q * NC + 2] = fma2(zC, m, fma2(tI, Fz, fma2(nZ, A, add2(B, acc[q * NC + 2]))));
+            // W += rI T + D AT + zhat BT + [-B F_y - dy S,  B F_x + dx S,  i3 (dy F_x - dx F_y)]
+            const P2<T> AT = mul2(i5, fma2(mul2(nZ, T(3)), Tz, mul2(qT, T(-4.5))));  // rRR s - rRz T_z = i5 (-9/2 s + 3 nZ T_z)
+            const P2<T> BT = fma2(mul2(mul2(nZ, T(6)), i5), qT, mul2(i3Tz, T(-3)));  // rzz T_z - rzR s = -3 i3 T_z + 6 nZ i5 s
+            const P2<T> S = fma2(nC, qF, mul2(cD, Fz));
+            acc[q * NC + 3] = fma2(dy, mul2(S, T(-1)), fma2(cB, -Fy, fma2(rI, Tx, fma2(dx, AT, acc[q * NC + 3]))));
+            acc[q * NC + 4] = fma2(dx, S, fma2(cB, Fx, fma2(rI, Ty, fma2(dy, AT, acc[q * NC + 4]))));
+            acc[q * NC + 5] = fma2(i3, fma2(dy, Fx, mul2(dx, -Fy)), fma2(rI, Tz, fma2(nZ, AT, add2(BT, acc[q * NC + 5]))));
+        }
+    }
+}
+
 // ---------------------------------------------------------------- kernel
 template <typename T> struct Vec16;                   // 16-byte shared-memory load = 4 sources (fp32) or 2 (fp64)
 template <> struct Vec16<float> { static constexpr int N = 4; using type = float4; };
@@ -312,7 +405,7 @@ struct PairKernelTraits {
     static constexpr int TARGETS = BLOCK * TPT;        // targets per CTA
 };
 
-template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES, int SUB, int MINB>
+template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES, int SUB, int MINB, bool WALL = false>
 __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<T> p)
 {
     using Tr = PairKernelTraits<T, NRHS, ANG, TPT, BLOCK, TJ, STAGES, SUB>;
@@ -372,6 +465,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
         ny[q] = mk2(-p.pos[p.npad + ia], -p.pos[p.npad + ib]);
         nz[q] = mk2(-p.pos[2 * p.npad + ia], -p.pos[2 * p.npad + ib]);
     }
+    P2<T> z4[WALL ? NP : 1];                        // single wall: 4 z_i, so that |R|^2 = r^2 + (4 z_i) z_j is one FMA
+    if constexpr (WALL) {
+#pragma unroll
+        for (int q = 0; q < NP; ++q) z4[q] = mul2(nz[q], T(-4));
+    }
     P2<T> total[NP][NV];
 #pragma unroll
     for (int q = 0; q < NP; ++q)
@@ -422,7 +520,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 #pragma unroll
                         for (int k = 0; k < NV; ++k) Vs[k] = vget(Vv[k], e0 + e);
 #pragma unroll
-                        for (int q = 0; q < NP; ++q) pair_apply<T, NRHS, ANG, FAR, EARLY>(p.c, gm[e][q], Vs, acc[q]);
+                        for (int q = 0; q < NP; ++q) {
+                            pair_apply<T, NRHS, ANG, FAR, EARLY>(p.c, gm[e][q], Vs, acc[q]);
+                            if constexpr (WALL) wall_apply<T, NRHS, ANG>(p.c, gm[e][q], nz[q], z4[q], vget(Z, e0 + e), Vs, acc[q]);
+                        }
                     }
                 };
                 if (!hit) body(std::true_type{});
@@ -444,11 +545,19 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
         }
     }
 
-    // ---- epilogue: apply the factored-out Oseen prefactor once per target
+    // ---- epilogue: apply the factored-out Oseen prefactor once per target (single wall: times the damping factor b_i)
 #pragma unroll
-    for (int q = 0; q < NP; ++q)
+    for (int q = 0; q < NP; ++q) {
+        P2<T> fl = splat(p.c.C1_lin), fa = splat(p.c.C1_ang);
+        if constexpr (WALL) {
+            const int64_t ia = min(i0 + (2 * q) * BLOCK + tid, p.npad - 1), ib = min(i0 + (2 * q + 1) * BLOCK + tid, p.npad - 1);
+            const P2<T> b = mk2(p.damp[ia], p.damp[ib]);
+            fl = mul2(fl, b);
+            fa = mul2(fa, b);
+        }
 #pragma unroll
-        for (int k = 0; k < NV; ++k) total[q][k] = mul2(total[q][k], (k % NC) < 3 ? p.c.C1_lin : p.c.C1_ang);
+        for (int k = 0; k < NV; ++k) total[q][k] = mul2(total[q][k], (k % NC) < 3 ? fl : fa);
+    }
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
 #pragma unroll

@@ -18,7 +18,8 @@
 namespace lm {
 
 template <typename T> struct StericParams {
-    const T* __restrict__ pos;   // [3][npad]  x | y | z
+    const T* __restrict__ pos;   // [3][npad]  x | y | z   (single wall: [5][npad], the true height is array 3)
+    int z_array;                 // which array holds z: 2, or 3 with a wall (array 2 is then the RAISED height of the mobility)
     T* __restrict__ partial;     // [j_splits][3][npad]
     int64_t N, npad;
     int64_t i_begin;             // first target row of this launch (row-sharded runs; 0 otherwise)
@@ -65,7 +66,7 @@ __global__ void __launch_bounds__(STERIC_BLOCK, 2) steric_pair_kernel(const Ster
         T* dst = tiles + (size_t)stage * 3 * TJ;
         mbar_expect_tx(&full[stage], bytes * 3);
 #pragma unroll
-        for (int a = 0; a < 3; ++a) bulk_g2s(dst + a * TJ, p.pos + a * p.npad + j0, bytes, &full[stage]);
+        for (int a = 0; a < 3; ++a) bulk_g2s(dst + a * TJ, p.pos + (size_t)(a == 2 ? p.z_array : a) * p.npad + j0, bytes, &full[stage]);
     };
 
     if (tid == 0) {
@@ -83,7 +84,7 @@ __global__ void __launch_bounds__(STERIC_BLOCK, 2) steric_pair_kernel(const Ster
     const int64_t ia = min(i0 + tid, p.npad - 1), ib = min(i0 + BLOCK + tid, p.npad - 1);
     const P2<T> nx = mk2(-p.pos[ia], -p.pos[ib]);
     const P2<T> ny = mk2(-p.pos[p.npad + ia], -p.pos[p.npad + ib]);
-    const P2<T> nz = mk2(-p.pos[2 * p.npad + ia], -p.pos[2 * p.npad + ib]);
+    const P2<T> nz = mk2(-p.pos[(size_t)p.z_array * p.npad + ia], -p.pos[(size_t)p.z_array * p.npad + ib]);
     P2<T> fx = splat(T(0)), fy = splat(T(0)), fz = splat(T(0));
 
     for (int lt = 0; lt < my_tiles; ++lt) {
@@ -143,10 +144,13 @@ __global__ void __launch_bounds__(STERIC_BLOCK, 2) steric_pair_kernel(const Ster
     }
 }
 
-// F[3i+k] = ext[3i+k] + sum over splits of partial  (fixed order: deterministic)
+// F[3i+k] = ext[3i+k] + sum over splits of partial  (fixed order: deterministic).
+// Single wall (`height` != null: the particles' heights above the wall, internal unit): plus the particle-wall repulsion
+// of eq. (13) with r = height of the centre and d = a, F_z += U0/b (r < d), U0/b exp((d - r)/b) (r >= d).
 template <typename T>
 __global__ void __launch_bounds__(256) steric_reduce_kernel(const T* __restrict__ partial, int splits, int64_t i_begin, int64_t i_end, int64_t npad,
-                                                            const T* __restrict__ ext, T* __restrict__ out)
+                                                            const T* __restrict__ ext, T* __restrict__ out, const T* __restrict__ height, T wall_d,
+                                                            T wall_m0, T wall_inv_b)
 {
     const int64_t i = i_begin + (int64_t)blockIdx.x * 256 + threadIdx.x;   // target rows [i_begin, i_end)
     if (i >= i_end) return;
@@ -154,6 +158,10 @@ __global__ void __launch_bounds__(256) steric_reduce_kernel(const T* __restrict_
     for (int k = 0; k < 3; ++k) {
         T s = ext ? ext[3 * i + k] : T(0);
         for (int q = 0; q < splits; ++q) s += partial[((size_t)q * 3 + k) * npad + i];
+        if (height && k == 2) {
+            const T r = height[i];
+            s += r < wall_d ? wall_m0 : wall_m0 * exp((wall_d - r) * wall_inv_b);
+        }
         out[3 * i + k] = s;
     }
 }

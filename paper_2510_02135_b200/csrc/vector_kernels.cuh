@@ -14,33 +14,57 @@ constexpr int RED_MAX_BLOCKS = 1024; // upper bound on the grid of the reduction
 // a1: interleaved positions (3N) -> x | y | z, each npad long, ghosts zero.  Lengths are stored multiplied by
 // `len_scale`, the power of two nearest 1/a (exact): the pair kernel then works with a radius in [0.71, 1.41]
 // whatever unit system the caller uses ("internal length unit").
+//
+// Single wall (`wall` != 0; reading S19, "damping matrix approach"): five arrays
+// x | y | z~ | h | b  with h = (z - wall_z) the height of the centre above the wall, z~ = max(h, a) the RAISED height the
+// pair kernel works with, and b = min(1, max(h, 0)/a) the damping factor (ghosts: z~ = a, b = 0).  All lengths x len_scale.
+template <typename T> struct WallPack { int on; T wall_z, a_scaled; };   // wall_z in the caller's unit, a_scaled = a * len_scale
+
+template <typename T> __device__ __forceinline__ void wall_raise(T h, T a_scaled, T& z_raised, T& b)
+{
+    z_raised = h > a_scaled ? h : a_scaled;
+    b = h >= a_scaled ? T(1) : (h > T(0) ? h / a_scaled : T(0));
+}
+
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) pack_positions_kernel(const T* __restrict__ pos, int64_t N, int64_t npad, T len_scale, T* __restrict__ soa)
+__global__ void __launch_bounds__(VEC_BLOCK) pack_positions_kernel(const T* __restrict__ pos, int64_t N, int64_t npad, T len_scale, WallPack<T> wall,
+                                                                   T* __restrict__ soa)
 {
     const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
     if (i >= npad) return;
     T x = T(0), y = T(0), z = T(0);
-    if (i < N) { x = pos[3 * i] * len_scale; y = pos[3 * i + 1] * len_scale; z = pos[3 * i + 2] * len_scale; }
+    if (i < N) { x = pos[3 * i] * len_scale; y = pos[3 * i + 1] * len_scale; z = (wall.on ? pos[3 * i + 2] - wall.wall_z : pos[3 * i + 2]) * len_scale; }
     soa[i] = x;
     soa[npad + i] = y;
-    soa[2 * npad + i] = z;
+    if (!wall.on) {
+        soa[2 * npad + i] = z;
+        return;
+    }
+    T zr = wall.a_scaled, b = T(0);
+    if (i < N) wall_raise(z, wall.a_scaled, zr, b);
+    soa[2 * npad + i] = zr;
+    soa[3 * npad + i] = z;
+    soa[4 * npad + i] = b;
 }
 
 // a2: right-hand sides -> [nrhs*NC][npad] component arrays (NC = 3: Fx Fy Fz; NC = 6: + Tx Ty Tz),
 // ghosts zero; a null force / torque pointer means zeros.  Torques are stored multiplied by
 // `len_scale` (the internal length unit: a torque is a force times a length).
+// `damp` (single wall, else null): the sources' damping factors b_j, folded into the packed values (M~ = B M B).
 template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) pack_rhs_kernel(RhsIn<T> in, int nrhs, int nc, int64_t N, int64_t npad, T len_scale, T* __restrict__ soa)
+__global__ void __launch_bounds__(VEC_BLOCK) pack_rhs_kernel(RhsIn<T> in, int nrhs, int nc, int64_t N, int64_t npad, T len_scale, const T* __restrict__ damp,
+                                                             T* __restrict__ soa)
 {
     const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
     if (i >= npad) return;
+    const T b = damp ? damp[i] : T(1);
     for (int q = 0; q < nrhs; ++q) {
         T v[6] = {T(0), T(0), T(0), T(0), T(0), T(0)};
         if (i < N) {
             if (in.f[q]) { v[0] = in.f[q][3 * i]; v[1] = in.f[q][3 * i + 1]; v[2] = in.f[q][3 * i + 2]; }
             if (nc == 6 && in.t[q]) { v[3] = in.t[q][3 * i] * len_scale; v[4] = in.t[q][3 * i + 1] * len_scale; v[5] = in.t[q][3 * i + 2] * len_scale; }
         }
-        for (int k = 0; k < nc; ++k) soa[(size_t)(q * nc + k) * npad + i] = v[k];
+        for (int k = 0; k < nc; ++k) soa[(size_t)(q * nc + k) * npad + i] = damp ? v[k] * b : v[k];
     }
 }
 
@@ -73,17 +97,26 @@ __global__ void __launch_bounds__(VEC_BLOCK) reduce_partials_kernel(const T* __r
 
 // eq. (11) PAPER.md:151-155 (random finite difference): packed positions displaced along W,
 // out[c][i] = soa[c][i] + s W[3i+c]  (s = +-delta/2); ghosts stay where they are.
+// Single wall: the height h (array 3) is displaced and the raised height and damping factor are formed anew.
 template <typename T>
 __global__ void __launch_bounds__(VEC_BLOCK) shift_positions_kernel(const T* __restrict__ soa, const T* __restrict__ W, int64_t N, int64_t npad, T s,
-                                                                    T* __restrict__ out)
+                                                                    WallPack<T> wall, T* __restrict__ out)
 {
     const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
     if (i >= npad) return;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        T v = soa[(size_t)c * npad + i];
+        T v = soa[(size_t)((wall.on && c == 2) ? 3 : c) * npad + i];
         if (i < N) v += s * W[3 * i + c];
-        out[(size_t)c * npad + i] = v;
+        if (wall.on && c == 2) {
+            T zr = wall.a_scaled, b = T(0);
+            if (i < N) wall_raise(v, wall.a_scaled, zr, b);
+            out[(size_t)2 * npad + i] = zr;
+            out[(size_t)3 * npad + i] = v;
+            out[(size_t)4 * npad + i] = b;
+        } else {
+            out[(size_t)c * npad + i] = v;
+        }
     }
 }
 
@@ -162,7 +195,7 @@ __global__ void __launch_bounds__(VEC_BLOCK) sumsq_kernel(const T* __restrict__ 
 template <typename T>
 __global__ void __launch_bounds__(VEC_BLOCK) lanczos_scale_pack_kernel(const T* __restrict__ x, int64_t N, int64_t npad, int nc, T len_scale,
                                                                        const double* sumsq, const int* __restrict__ newest,
-                                                                       T* __restrict__ V, T* __restrict__ soa)
+                                                                       T* __restrict__ V, T* __restrict__ soa, const T* __restrict__ damp)
 {
     const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
     if (i >= npad) return;
@@ -177,7 +210,9 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_scale_pack_kernel(const T* 
             val = (T)((double)x[idx] * inv);
             v_out[idx] = val;
         }
-        soa[(size_t)c * npad + i] = c < 3 ? val : val * len_scale;       // angular part: internal length unit, as in pack_rhs
+        T packed = c < 3 ? val : val * len_scale;                        // angular part: internal length unit, as in pack_rhs
+        if (damp) packed *= damp[i];                                     // single wall: the source's damping factor
+        soa[(size_t)c * npad + i] = packed;
     }
 }
 

@@ -120,3 +120,46 @@ def fcc(n_cells: int, number_density: float, jitter: float, seed: int) -> np.nda
     pos = ((g + base[None]) * cell).reshape(-1, 3)
     rng = np.random.default_rng(seed)
     return pos + (rng.random(pos.shape) - 0.5) * 2.0 * jitter
+
+
+# ---------------------------------------------------------------- single-wall workloads
+MICROROLLER_A = 0.656          # radius in micrometres
+MICROROLLER_N = 32768          # N = 2^15
+
+
+def wall_slab_case(N: int, side: float, z_lo: float, z_hi: float, seed: int, precision: str = "f64", angular: bool = False,
+                   with_noise: bool = False, wall_z: float = 0.0) -> dict:
+    """Free-form wall test case: x, y uniform in a square of the given side, heights above the wall uniform in
+    [z_lo, z_hi] (z_lo < a: particles cutting the wall; z_lo < 0: particles under it)."""
+    dt = np_dtype(precision)
+    rng = np.random.default_rng(seed)
+    pos = np.column_stack([rng.random(N) * side, rng.random(N) * side, wall_z + z_lo + rng.random(N) * (z_hi - z_lo)])
+    forces = rng.standard_normal((N, 3))
+    torques = rng.standard_normal((N, 3)) if angular else None
+    noise = rng.standard_normal((6 if angular else 3) * N) if with_noise else None
+    cast = lambda v: None if v is None else np.ascontiguousarray(v.astype(dt))
+    return dict(N=N, pos=cast(pos), forces=cast(forces), torques=cast(torques), noise=cast(noise), wall_z=float(wall_z))
+
+
+def microroller_monolayer(N: int = MICROROLLER_N, a: float = MICROROLLER_A, h_g_over_a: float = 1.5, seed: int = 5, precision: str = "f32",
+                          with_noise: bool = False) -> dict:
+    """The initial configuration of the paper's microroller suspension, synthetic: the x-y plane of a
+    60a x 4915a strip (scaled with N so that the area fraction stays that of N = 2^15) is gridded in cells of side 2a,
+    N distinct cells are drawn at random (no two particles overlap) and each particle sits at the centre of its cell;
+    the height of each centre is a + an exponential of mean k_BT/mg = h_g - a (Gibbs-Boltzmann above the contact
+    height; h_g = 1.5a or 6.1a in the paper).  Forces and torques ~ N(0,1) (the paper drives the rollers with one
+    constant torque; random inputs exercise every block).  Wall at z = 0."""
+    dt = np_dtype(precision)
+    rng = np.random.default_rng(seed)
+    nx = 30
+    ny = max(-(-2457 * N // MICROROLLER_N), -(-N // nx) + 1)
+    cells = rng.choice(nx * ny, size=N, replace=False)
+    x = (cells % nx + 0.5) * 2.0 * a
+    y = (cells // nx + 0.5) * 2.0 * a
+    z = a + rng.exponential((h_g_over_a - 1.0) * a, N)
+    pos = np.column_stack([x, y, z])
+    forces = rng.standard_normal((N, 3))
+    torques = rng.standard_normal((N, 3))
+    noise = rng.standard_normal(6 * N) if with_noise else None
+    cast = lambda v: None if v is None else np.ascontiguousarray(v.astype(dt))
+    return dict(N=N, a=a, pos=cast(pos), forces=cast(forces), torques=cast(torques), noise=cast(noise), wall_z=0.0)
