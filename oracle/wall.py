@@ -16,6 +16,10 @@ lanczos_sqrt_mdot_w  rpy.lanczos_sqrt_mdot_w with the wall op
 thermal_drift_rfd eq. (11), one realisation: (1/delta)[M(X + delta W/2) - M(X - delta W/2)] W
 divergence_fd     (d/dX).M by central differences of the dense matrix: what the mean of the RFD must equal
 wall_steric_forces eq. (13) PAPER.md:214-219 between a particle and the wall: r = height of the centre, d = a
+bd_step           eq. (14) PAPER.md:224-228 above a wall: X^{n+1} = X^n + dt (3/2 v^n - 1/2 v^{n-1}) + sqrt(2 kT dt) (M^n)^{1/2} W^n
+                  with v^n = M^n F^n + kT (d/dX).M^n, the drift taken as ONE random-finite-difference sample of eq. (11)
+                  ("we also include the thermal drift term in the deterministic part of the time stepping
+                  scheme"); F^n = particle-particle and particle-wall steric forces (eq. 13) + external forces
 
 Pins: tests/test_oracle_wall.py.  No function here is "parity unpinned".
 """
@@ -179,3 +183,33 @@ def wall_steric_forces(pos, U0: float, b: float, a: float = 1.0, wall_z: float =
     F = np.zeros_like(x)
     F[:, 2] = np.where(r < a, U0 / b, (U0 / b) * np.exp((a - r) / b))
     return F
+
+
+def bd_step(pos, v_prev, dt: float, kT: float, a: float = 1.0, eta: float = 1.0, wall_z: float = 0.0, U0: float = 0.0, b: float = 0.1,
+            ext_forces=None, ext_torques=None, noise=None, rfd_noise=None, delta: float = 1e-3, angular: bool = False,
+            sqrt_mode: str = "dense", tol: float = 1e-3, max_iter: int = 100):
+    """One step of eq. (14) above a wall.  Returns (new positions (N,3), v^n (N,3) to pass as ``v_prev`` next time, info).
+    The first step (v_prev None) is forward Euler (reading S17).  ``rfd_noise``: the 3N vector W~ of eq. (11) for
+    this step's drift sample, or None for no drift term; ``noise``: W^n (dof entries) or None."""
+    from . import bd
+    x = np.asarray(pos, dtype=np.float64).reshape(-1, 3)
+    N = x.shape[0]
+    F = np.zeros((N, 3))
+    if U0 != 0.0:
+        F += bd.steric_forces(x, U0, b, 2.0 * a) + wall_steric_forces(x, U0, b, a, wall_z)
+    if ext_forces is not None:
+        F += np.asarray(ext_forces, dtype=np.float64).reshape(N, 3)
+    T = None if ext_torques is None else np.asarray(ext_torques, dtype=np.float64).reshape(N, 3)
+    v, _ = mdot(x, F, T, a, eta, wall_z, angular)
+    if rfd_noise is not None and kT > 0.0:
+        v = v + kT * thermal_drift_rfd(x, rfd_noise, delta, a, eta, wall_z, angular)[0]
+    info = {"iterations": 0}
+    new = x + bd.ab_displacement(v, v_prev, dt)
+    if noise is not None and kT > 0.0:
+        if sqrt_mode == "dense":
+            y = dense_sqrt_mdot_w(x, noise, a, eta, wall_z, angular)
+        else:
+            y, k, _ = lanczos_sqrt_mdot_w(x, noise, tol, a, eta, wall_z, angular, max_iter=max_iter)
+            info["iterations"] = k
+        new = new + bd.noise_prefactor(kT, dt) * np.asarray(y).reshape(-1)[: 3 * N].reshape(N, 3)
+    return new, v, info

@@ -22,6 +22,8 @@ by what the paper's DEFINITION and the mathematics fix, with nothing taken from 
   W10 thermal drift: the RFD of eq. (11) summed over unit vectors is the central-difference divergence; the divergence
       of one sphere is d mu_perp / dh; a Monte-Carlo mean of RFD samples approaches it.
   W11 wall steric force of eq. (13) with d = a: minus the derivative of the potential.
+  W12 the time step of eq. (14) above a wall: one sphere settling (dt mu_perp F), its drift displacement
+      (dt kT d mu_perp/dh), Adams-Bashforth weights, noise term, and the free-space step far from the wall.
 """
 import math
 
@@ -475,3 +477,44 @@ def test_w11_wall_steric_force_is_minus_the_gradient_of_eq13():
         assert F[i, 2] == pytest.approx(-dU, rel=1e-6)
     assert F[1, 2] == pytest.approx(F[2, 2], rel=1e-6) == pytest.approx(U0 / b, rel=1e-6)     # C^1 potential: continuous force at r = d
     assert F[4, 2] < 1e-18 * U0 / b * 1e3 or F[4, 2] < 1e-15
+
+
+def test_w12_bd_step_above_a_wall():
+    a, eta, dt, kT = 1.0, 1.0, 1e-2, 0.3
+    h = 1.8
+    e = a / h
+    mu_perp = (1 - 9 / 8 * e + e ** 3 / 2 - e ** 5 / 8) / (6 * PI * eta * a)
+    dmu = (9 / 8 * e - 3 / 2 * e ** 3 + 5 / 8 * e ** 5) / h / (6 * PI * eta * a)
+    x0 = np.array([[0.0, 0.0, h]])
+    # settling under a force: forward Euler on the first step
+    x1, v0, _ = wall.bd_step(x0, None, dt, 0.0, ext_forces=np.array([[0.0, 0.0, -2.0]]))
+    np.testing.assert_allclose(x1, [[0, 0, h - dt * 2.0 * mu_perp]], rtol=1e-13)
+    np.testing.assert_allclose(v0, [[0, 0, -2.0 * mu_perp]], rtol=1e-13)
+    # the drift alone (rfd_noise = e_z makes the sample the central difference of mu_perp)
+    x1d, vd, _ = wall.bd_step(x0, None, dt, kT, rfd_noise=np.array([0.0, 0.0, 1.0]), delta=1e-4)
+    np.testing.assert_allclose(x1d[0, 2] - h, dt * kT * dmu, rtol=1e-6)
+    assert x1d[0, 2] > h                                            # pushes away from the wall
+    assert np.all(wall.bd_step(x0, None, dt, 0.0, rfd_noise=np.array([0.0, 0.0, 1.0]))[0] == x0)   # kT = 0: no drift
+    # second step: 3/2 v^1 - 1/2 v^0 (eq. (14)), v including the drift
+    x2, v1, _ = wall.bd_step(x1d, vd, dt, kT, ext_forces=np.array([[0.3, 0.0, -1.0]]), rfd_noise=np.array([0.0, 0.0, 1.0]), delta=1e-4)
+    _, v1_alone, _ = wall.bd_step(x1d, None, dt, kT, ext_forces=np.array([[0.3, 0.0, -1.0]]), rfd_noise=np.array([0.0, 0.0, 1.0]), delta=1e-4)
+    np.testing.assert_allclose(v1, v1_alone, rtol=1e-14)
+    np.testing.assert_allclose(x2, x1d + dt * (1.5 * v1 - 0.5 * vd), rtol=1e-14)
+    # noise term: sqrt(2 kT dt) M^{1/2} W with the dense root
+    rng = np.random.default_rng(1)
+    x = np.column_stack([rng.random(20) * 6, rng.random(20) * 6, 0.4 + rng.random(20) * 2])
+    W = rng.standard_normal(60)
+    xn, _, _ = wall.bd_step(x, None, dt, kT, noise=W)
+    np.testing.assert_allclose((xn - x).reshape(-1), math.sqrt(2 * kT * dt) * wall.dense_sqrt_mdot_w(x, W), rtol=1e-12, atol=1e-15)
+    xl, _, info = wall.bd_step(x, None, dt, kT, noise=W, sqrt_mode="lanczos", tol=1e-5)
+    assert info["iterations"] > 3 and np.linalg.norm(xl - xn) <= 5e-5 * np.linalg.norm(xn - x)
+    # steric forces: particle-particle at the true positions plus particle-wall
+    F = rng.standard_normal((20, 3))
+    xs, vs, _ = wall.bd_step(x, None, dt, 0.0, U0=4.0, b=0.1, ext_forces=F)
+    Ftot = bd.steric_forces(x, 4.0, 0.1, 2 * a) + wall.wall_steric_forces(x, 4.0, 0.1, a) + F
+    np.testing.assert_allclose(vs, wall.mdot(x, Ftot)[0], rtol=1e-13)
+    # far from the wall: the free-space step of oracle/bd
+    xf = x + np.array([0, 0, 1e7])
+    a1, _, _ = wall.bd_step(xf, None, dt, kT, U0=4.0, b=0.1, ext_forces=F, noise=W)
+    b1, _, _ = bd.bd_step(xf, None, dt, kT, U0=4.0, b=0.1, ext_forces=F, noise=W)
+    np.testing.assert_allclose(a1 - xf, b1 - xf, rtol=1e-4, atol=1e-9)
