@@ -172,6 +172,17 @@ int lm_bd_step(lm_solver* h, void* pos, const void* ext_forces, const void* ext_
 int lm_bd_step_host(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise,
                     double dt, double kT, double U0, double b, double tol, void* stream);
 int lm_bd_reset(lm_solver* h);                        /* forget the Adams-Bashforth history */
+/* lm_bd_step with the thermal-drift terms of eq. (14) ("we also include the thermal drift term in the
+ * deterministic part of the time stepping scheme as it has non-zero mean"): the deterministic velocity becomes
+ *   v^n = M^n F^n + kT * (1/rfd_delta) [ M(X^n + rfd_delta W~/2) - M(X^n - rfd_delta W~/2) ] W~,
+ * ONE random-finite-difference sample of kT d/dX . M^n (eq. (11)) with W~ = rfd_noise (3N values ~ N(0,1),
+ * independent of `noise`), and enters the Adams-Bashforth combination 3/2 v^n - 1/2 v^{n-1} as a whole.  Two more M.F
+ * applies per step.  rfd_noise == NULL (or kT == 0): exactly lm_bd_step.  Meant for lm_set_wall geometries; for open
+ * boundaries the term has zero mean. */
+int lm_bd_step_rfd(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise,
+                   const void* rfd_noise, double rfd_delta, double dt, double kT, double U0, double b, double tol, void* stream);
+int lm_bd_step_rfd_host(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise,
+                        const void* rfd_noise, double rfd_delta, double dt, double kT, double U0, double b, double tol, void* stream);
 
 /* ---- Thermal drift  d/dX . M  (the paper's divM) ----
  * lm_thermal_drift: the library default for open boundaries -- the divergence of the free-space mobility

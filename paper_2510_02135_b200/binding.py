@@ -43,6 +43,10 @@ SIGNATURES = {
     "lm_steric_forces": (c_int, [c_void_p, c_double, c_double, c_void_p, c_void_p, c_void_p]),
     "lm_bd_step": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_double, c_double, c_double, c_void_p]),
     "lm_bd_step_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_double, c_double, c_double, c_void_p]),
+    "lm_bd_step_rfd": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_double, c_double, c_double, c_double,
+                               c_void_p]),
+    "lm_bd_step_rfd_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_double, c_double, c_double, c_double, c_double,
+                                    c_double, c_void_p]),
     "lm_bd_reset": (c_int, [c_void_p]),
     "lm_thermal_drift": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p]),
     "lm_thermal_drift_rfd": (c_int, [c_void_p, c_void_p, c_double, c_void_p, c_void_p, c_void_p]),
@@ -263,6 +267,23 @@ class Solver:
         self._expect(noise, (6 if self.angular else 3) * self.N, True)
         return self._check(lib().lm_bd_step_host(self._h, _ptr(pos), _ptr(ext_forces), _ptr(ext_torques), _ptr(noise), float(dt), float(kT),
                                                  float(U0), float(b), float(tol), _stream_ptr(stream)), allow=(LM_E_NOCONV,) if allow_noconv else ())
+
+    def bd_step_rfd(self, pos, ext_forces, ext_torques, noise, rfd_noise, rfd_delta, dt, kT, U0, b, tol, stream=None, allow_noconv=False) -> int:
+        """lm_bd_step with the thermal-drift term of eq. (14) as one RFD sample (W~ = rfd_noise, 3N)."""
+        for x in (pos, ext_forces, ext_torques, rfd_noise):
+            self._expect(x, 3 * self.N, False)
+        self._expect(noise, (6 if self.angular else 3) * self.N, False)
+        return self._check(lib().lm_bd_step_rfd(self._h, _ptr(pos), _ptr(ext_forces), _ptr(ext_torques), _ptr(noise), _ptr(rfd_noise), float(rfd_delta),
+                                                float(dt), float(kT), float(U0), float(b), float(tol), _stream_ptr(stream)),
+                           allow=(LM_E_NOCONV,) if allow_noconv else ())
+
+    def bd_step_rfd_host(self, pos, ext_forces, ext_torques, noise, rfd_noise, rfd_delta, dt, kT, U0, b, tol, stream=None, allow_noconv=False) -> int:
+        for x in (pos, ext_forces, ext_torques, rfd_noise):
+            self._expect(x, 3 * self.N, True)
+        self._expect(noise, (6 if self.angular else 3) * self.N, True)
+        return self._check(lib().lm_bd_step_rfd_host(self._h, _ptr(pos), _ptr(ext_forces), _ptr(ext_torques), _ptr(noise), _ptr(rfd_noise),
+                                                     float(rfd_delta), float(dt), float(kT), float(U0), float(b), float(tol), _stream_ptr(stream)),
+                           allow=(LM_E_NOCONV,) if allow_noconv else ())
 
     def bd_reset(self):
         self._check(lib().lm_bd_reset(self._h))

@@ -401,8 +401,8 @@ int lm_bd_reset(lm_solver* h)
     return LM_OK;
 }
 
-int lm_bd_step(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise, double dt, double kT, double U0,
-               double b, double tol, void* stream)
+int lm_bd_step_rfd(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise, const void* rfd_noise,
+                   double rfd_delta, double dt, double kT, double U0, double b, double tol, void* stream)
 {
     if (!h) return LM_E_NULL;
     h->err.clear();
@@ -411,21 +411,30 @@ int lm_bd_step(lm_solver* h, void* pos, const void* ext_forces, const void* ext_
     if (!(dt > 0.0) || !std::isfinite(dt) || !(kT >= 0.0) || !std::isfinite(kT)) return fail(h, LM_E_INVALID, "dt must be > 0 and kT >= 0");
     if (U0 != 0.0 && (!(b > 0.0) || !std::isfinite(b) || !std::isfinite(U0))) return fail(h, LM_E_INVALID, "steric potential needs b > 0 and finite U0");
     if (noise && kT > 0.0 && (!(tol > 0.0) || !std::isfinite(tol))) return fail(h, LM_E_INVALID, "tol must be > 0");
+    if (rfd_noise && kT > 0.0 && (!(rfd_delta > 0.0) || !std::isfinite(rfd_delta))) return fail(h, LM_E_INVALID, "rfd_delta must be > 0");
     cudaStream_t st = (cudaStream_t)stream;
     return h->precision == LM_F32
-               ? bd_step_device<float>(h, (float*)pos, (const float*)ext_forces, (const float*)ext_torques, (const float*)noise, dt, kT, U0, b, tol, st)
-               : bd_step_device<double>(h, (double*)pos, (const double*)ext_forces, (const double*)ext_torques, (const double*)noise, dt, kT, U0, b, tol, st);
+               ? bd_step_device<float>(h, (float*)pos, (const float*)ext_forces, (const float*)ext_torques, (const float*)noise, (const float*)rfd_noise,
+                                       rfd_delta, dt, kT, U0, b, tol, st)
+               : bd_step_device<double>(h, (double*)pos, (const double*)ext_forces, (const double*)ext_torques, (const double*)noise,
+                                        (const double*)rfd_noise, rfd_delta, dt, kT, U0, b, tol, st);
 }
 
-int lm_bd_step_host(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise, double dt, double kT,
-                    double U0, double b, double tol, void* stream)
+int lm_bd_step(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise, double dt, double kT, double U0,
+               double b, double tol, void* stream)
+{
+    return lm_bd_step_rfd(h, pos, ext_forces, ext_torques, noise, nullptr, 0.0, dt, kT, U0, b, tol, stream);
+}
+
+int lm_bd_step_rfd_host(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise, const void* rfd_noise,
+                        double rfd_delta, double dt, double kT, double U0, double b, double tol, void* stream)
 {
     if (!h) return LM_E_NULL;
     h->err.clear();
     if (!pos) return fail(h, LM_E_NULL, "pos is NULL");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t bytes = (size_t)3 * h->N * esize(h);
-    void *dp = nullptr, *df, *dt_, *dn;
+    void *dp = nullptr, *df, *dt_, *dn, *dr;
     int rc = ensure(h, &h->bd[6], &h->bd_bytes[6], bytes);
     if (rc != LM_OK) return rc;
     dp = h->bd[6];
@@ -433,11 +442,18 @@ int lm_bd_step_host(lm_solver* h, void* pos, const void* ext_forces, const void*
     if ((rc = stage_in(h, 1, ext_forces, bytes, st, &df)) != LM_OK) return rc;
     if ((rc = stage_in(h, 2, ext_torques, bytes, st, &dt_)) != LM_OK) return rc;
     if ((rc = stage_in(h, 3, noise, (size_t)dof_of(h) * esize(h), st, &dn)) != LM_OK) return rc;
-    rc = lm_bd_step(h, dp, df, dt_, dn, dt, kT, U0, b, tol, stream);
+    if ((rc = stage_in(h, 4, rfd_noise, bytes, st, &dr)) != LM_OK) return rc;      // slot 4 (lin staging) is free in this call
+    rc = lm_bd_step_rfd(h, dp, df, dt_, dn, dr, rfd_delta, dt, kT, U0, b, tol, stream);
     if (rc != LM_OK && rc != LM_E_NOCONV) return rc;
     LM_CUDA(h, cudaMemcpyAsync(pos, dp, bytes, cudaMemcpyDeviceToHost, st));
     LM_CUDA(h, cudaStreamSynchronize(st));
     return rc;
+}
+
+int lm_bd_step_host(lm_solver* h, void* pos, const void* ext_forces, const void* ext_torques, const void* noise, double dt, double kT,
+                    double U0, double b, double tol, void* stream)
+{
+    return lm_bd_step_rfd_host(h, pos, ext_forces, ext_torques, noise, nullptr, 0.0, dt, kT, U0, b, tol, stream);
 }
 
 // ---------------------------------------------------------------- thermal drift

@@ -87,15 +87,21 @@ int rfd_device(lm_solver* h, const T* W, double delta, T* lin_out, T* ang_out, c
     return LM_OK;
 }
 
+// rfd_noise != null (and kT > 0): the thermal-drift term of eq. (14), kT (d/dX).M^n, joins v_n as ONE random-finite-
+// difference sample of eq. (11) with W~ = rfd_noise (zero mean for open boundaries, non-zero above a wall).
 template <typename T>
-int bd_step_device(lm_solver* h, T* pos, const T* ext_f, const T* ext_t, const T* noise, double dt, double kT, double U0, double b, double tol,
-                   cudaStream_t st)
+int bd_step_device(lm_solver* h, T* pos, const T* ext_f, const T* ext_t, const T* noise, const T* rfd_noise, double rfd_delta, double dt, double kT,
+                   double U0, double b, double tol, cudaStream_t st)
 {
     const int64_t n3 = 3 * h->N;
     const size_t bytes = (size_t)n3 * sizeof(T);
     int rc;
     for (int k = 0; k < 6; ++k)
         if ((rc = ensure(h, &h->bd[k], &h->bd_bytes[k], bytes)) != LM_OK) return rc;
+    const bool drift = rfd_noise && kT > 0.0;
+    if (drift)
+        for (int k = 7; k < 9; ++k)
+            if ((rc = ensure(h, &h->bd[k], &h->bd_bytes[k], bytes)) != LM_OK) return rc;
     T *F = (T*)h->bd[0], *vn = (T*)h->bd[1], *vprev = (T*)h->bd[2], *y = (T*)h->bd[3], *ang = (T*)h->bd[4], *yang = (T*)h->bd[5];
     if ((rc = set_positions_t<T>(h, pos, st)) != LM_OK) return rc;
     // F^n = steric(X^n) + external;  v_n = M^n [F^n; T]
@@ -126,6 +132,12 @@ int bd_step_device(lm_solver* h, T* pos, const T* ext_f, const T* ext_t, const T
             rc_noise = lanczos_device<T>(h, 1, noise, tol, y, h->angular ? yang : nullptr, 1.0, 0, nullptr, st);
             if (rc_noise != LM_OK && rc_noise != LM_E_NOCONV) return rc_noise;
         }
+    }
+    if (drift) {                                                     // v_n += kT * (one RFD sample of the divergence)
+        T *dl = (T*)h->bd[7], *da = (T*)h->bd[8];
+        if ((rc = rfd_device<T>(h, rfd_noise, rfd_delta, dl, h->angular ? da : nullptr, st)) != LM_OK) return rc;
+        add_scaled_kernel<T><<<grid_1d(n3), VEC_BLOCK, 0, st>>>(vn, dl, (T)kT, n3);
+        h->n_aux++;
     }
     const double cn = h->bd_have_prev ? 1.5 : 1.0, cp = h->bd_have_prev ? 0.5 : 0.0;
     bd_update_kernel<T><<<grid_1d(n3), VEC_BLOCK, 0, st>>>(pos, vn, vprev, noisy ? y : nullptr, n3, (T)(dt * cn), (T)(dt * cp),

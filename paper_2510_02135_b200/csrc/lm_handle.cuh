@@ -155,8 +155,9 @@ struct lm_solver {
     struct GraphKey { const void *V, *w, *vec, *partial, *pos; int kmax, variant, splits, prec; } lz_key = {nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0};
 
     // Brownian-dynamics step (lm_bd_step): F, v_n, v_{n-1}, noise velocity, angular scratch x2, position staging
-    void* bd[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    size_t bd_bytes[7] = {0, 0, 0, 0, 0, 0, 0};
+    // [7], [8]: the drift sample (linear, angular) of a step with a random-finite-difference term
+    void* bd[9] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    size_t bd_bytes[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     bool bd_have_prev = false;
     bool steric_attr_set = false;
     // random finite difference (lm_thermal_drift_rfd): displaced packed positions, U(X-) linear / angular

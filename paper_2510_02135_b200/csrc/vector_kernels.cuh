@@ -128,6 +128,14 @@ __global__ void __launch_bounds__(VEC_BLOCK) rfd_difference_kernel(T* __restrict
     if (i < n) up[i] = (up[i] - um[i]) * inv_delta;
 }
 
+// y += s x   (the drift term joining the deterministic velocity of eq. (14))
+template <typename T>
+__global__ void __launch_bounds__(VEC_BLOCK) add_scaled_kernel(T* __restrict__ y, const T* __restrict__ x, T s, int64_t n)
+{
+    const int64_t i = (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;
+    if (i < n) y[i] = fma(s, x[i], y[i]);
+}
+
 // ---------------------------------------------------------------- Lanczos vector operations (a7)
 // Reductions: warp shuffles -> one fp64 partial per block -> the last block to finish (ticket)
 // adds the block partials in index order, so the result is deterministic for a given grid.

@@ -226,3 +226,54 @@ def test_wall_steric_forces(lm, torch, prec):
     want = bd.steric_forces(c["pos"], U0, b, 2 * a) + wall.wall_steric_forces(c["pos"], U0, b, a, c["wall_z"]) + c["forces"].astype(np.float64)
     assert close(out.cpu().numpy(), want, 1e-12 if prec == "f64" else 2e-5), rel(out.cpu().numpy(), want)
     s.close()
+
+
+@pytest.mark.parametrize("prec,angular", [("f64", False), ("f64", True), ("f32", False), ("f32", True)])
+def test_wall_bd_step_with_drift_matches_oracle(lm, torch, prec, angular):
+    """eq. (14) above a wall: steric forces between particles and with the wall, external forces and
+    torques, the drift term as one RFD sample, the Lanczos noise -- three steps (Euler, then Adams-Bashforth) against
+    oracle/wall.bd_step (dense root), same W^n and W~^n on both sides; host variant bit-identical."""
+    N, dt, kT, U0, b, tol = 300, 2e-3, 0.4, 4.0, 0.1, (1e-6 if prec == "f64" else 1e-3)
+    delta = 1e-3 if prec == "f64" else 0.05
+    c = workloads.wall_slab_case(N, 14.0, 0.6, 2.5, 71, prec, angular, with_noise=True, wall_z=-2.0)
+    dtp = workloads.np_dtype(prec)
+    rng = np.random.default_rng(72)
+    Wn = [np.roll(c["noise"], 5 * n) for n in range(3)]
+    Wt = [rng.standard_normal(3 * N).astype(dtp) for n in range(3)]
+    s = lm.Solver(prec, N, 1.0, 1.0, angular)
+    s.set_wall(True, c["wall_z"])
+    s.set_max_iter(300)
+    X = dev(torch, c["pos"]).reshape(-1).clone()
+    F, T = dev(torch, c["forces"]).reshape(-1), (dev(torch, c["torques"]).reshape(-1) if angular else None)
+    traj = []
+    for n in range(3):
+        s.bd_step_rfd(X, F, T, dev(torch, Wn[n]), dev(torch, Wt[n]), delta, dt, kT, U0, b, tol)
+        traj.append(X.cpu().numpy().copy())
+    s.close()
+    sh = lm.Solver(prec, N, 1.0, 1.0, angular)
+    sh.set_wall(True, c["wall_z"])
+    sh.set_max_iter(300)
+    Xh = c["pos"].copy().reshape(-1)
+    for n in range(3):
+        sh.bd_step_rfd_host(Xh, c["forces"].reshape(-1), c["torques"].reshape(-1) if angular else None, Wn[n], Wt[n], delta, dt, kT, U0, b, tol)
+        np.testing.assert_array_equal(Xh, traj[n])
+    sh.close()
+    x, vprev = np.asarray(c["pos"], np.float64), None
+    x0 = x.reshape(-1).copy()
+    for n in range(3):
+        x, vprev, _ = wall.bd_step(x, vprev, dt, kT, wall_z=c["wall_z"], U0=U0, b=b, ext_forces=c["forces"], ext_torques=c["torques"] if angular else None,
+                                   noise=Wn[n], rfd_noise=Wt[n], delta=delta, angular=angular, sqrt_mode="dense")
+        # the displacement is dominated by the noise term (tolerance 3 tol, S4 iii); fp32: difference quotient of the drift
+        gate = 3 * tol + (0.0 if prec == "f64" else 2e-3)
+        assert rel(traj[n] - x0, x.reshape(-1) - x0) <= gate, (n, rel(traj[n] - x0, x.reshape(-1) - x0))
+    # deterministic part alone (no noise): tight
+    s = lm.Solver(prec, N, 1.0, 1.0, angular)
+    s.set_wall(True, c["wall_z"])
+    X = dev(torch, c["pos"]).reshape(-1).clone()
+    x, vprev = np.asarray(c["pos"], np.float64), None
+    for n in range(2):
+        s.bd_step_rfd(X, F, T, None, dev(torch, Wt[n]), delta, dt, kT, U0, b, tol)
+        x, vprev, _ = wall.bd_step(x, vprev, dt, kT, wall_z=c["wall_z"], U0=U0, b=b, ext_forces=c["forces"], ext_torques=c["torques"] if angular else None,
+                                   rfd_noise=Wt[n], delta=delta, angular=angular)
+        assert rel(X.cpu().numpy() - x0, x.reshape(-1) - x0) <= (1e-9 if prec == "f64" else 2e-3), (n, rel(X.cpu().numpy() - x0, x.reshape(-1) - x0))
+    s.close()
