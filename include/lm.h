@@ -237,11 +237,17 @@ int lm_mdot_rows(lm_solver* h, int64_t row_begin, int64_t row_count, const void*
  *                             every kernel directly.
  *   LM_OPT_SHARE_FIRST_APPLY  1 (default) | 0: in lm_hydrodynamic_velocities / lm_bd_step, M.[F;T] rides along with the
  *                             first Lanczos apply in one 2-right-hand-side launch, or is a launch of its own.
+ *   LM_OPT_SMALL_KERNEL       1 (default): small applies (N up to a few thousand) run as ONE launch of the cluster kernel
+ *                             of csrc/rpy_small.cuh (reads the caller's arrays, sums the source splits through
+ *                             distributed shared memory) where the launch chooser prefers it | 0: never (always pack,
+ *                             pair kernel, reduce) | (cluster << 8 | warps), cluster and warps in {1, 2, 4, 8}: always,
+ *                             with that shape (plan sweeps).  Same results up to summation order (PAPER.md:435-437:
+ *                             the small-N regime where launch overhead, not arithmetic, sets the time).
  * lm_lanczos_history: what the last Lanczos call measured for noise vector `vec` of its (last) group: for iteration
  *   i + 1 (i < cap): alpha[i], beta[i], step[i] = s_{i+1} (NaN for i = 0), estimate[i] = e_{i+1} (NaN for i < 2; NaN
  *   throughout under LM_RULE_STEP).  Any output may be NULL.  Returns the number of iterations recorded. */
 enum { LM_RULE_ESTIMATE = 0, LM_RULE_STEP = 1 };
-enum { LM_OPT_LANCZOS_RULE = 0, LM_OPT_GRAPH_REPLAY = 1, LM_OPT_SHARE_FIRST_APPLY = 2 };
+enum { LM_OPT_LANCZOS_RULE = 0, LM_OPT_GRAPH_REPLAY = 1, LM_OPT_SHARE_FIRST_APPLY = 2, LM_OPT_SMALL_KERNEL = 3 };
 int lm_set_option(lm_solver* h, int option, int value);
 int lm_set_max_iter(lm_solver* h, int max_iter);     /* default 100; 1 <= max_iter <= 1000 */
 int lm_last_iterations(const lm_solver* h);           /* iterations of the last Lanczos call (or < 0) */
@@ -260,9 +266,14 @@ int lm_get_stats(lm_solver* h, int64_t* pair_kernel_launches, int64_t* aux_launc
                  double* pairs);
 
 /* The launch configuration the next lm_mdot_batch(nrhs) would use: grid = i_tiles x j_splits CTAs
- * of `block` threads, `targets_per_thread` targets each, `smem_bytes` dynamic shared memory. */
+ * of `block` threads, `targets_per_thread` targets each, `smem_bytes` dynamic shared memory.  For the one-launch
+ * small-N kernel j_splits is the cluster size (the CTA's block / 32 warps split the sources further). */
 int lm_pair_launch_config(lm_solver* h, int nrhs, int* i_tiles, int* j_splits, int* block,
                           int* targets_per_thread, int* smem_bytes);
+
+/* Name of the O(N^2) kernel that launch would run (static storage): "rpy_small_kernel" (one launch per apply, small N,
+ * LM_OPT_SMALL_KERNEL) or "rpy_pair_kernel" (pack, pair kernel, split-j reduce); "" for an unsupported nrhs. */
+const char* lm_pair_kernel_name(lm_solver* h, int nrhs);
 
 /* Library version string (static storage). */
 const char* lm_version(void);

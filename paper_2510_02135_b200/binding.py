@@ -18,7 +18,7 @@ import numpy as np
 LM_F32, LM_F64 = 0, 1
 LM_OK, LM_E_INVALID, LM_E_NOPOS, LM_E_ANGULAR, LM_E_NULL, LM_E_CUDA, LM_E_NOCONV = 0, -1, -2, -3, -4, -5, -6
 LM_RULE_ESTIMATE, LM_RULE_STEP = 0, 1
-LM_OPT_LANCZOS_RULE, LM_OPT_GRAPH_REPLAY, LM_OPT_SHARE_FIRST_APPLY = 0, 1, 2
+LM_OPT_LANCZOS_RULE, LM_OPT_GRAPH_REPLAY, LM_OPT_SHARE_FIRST_APPLY, LM_OPT_SMALL_KERNEL = 0, 1, 2, 3
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liblm.so")
@@ -63,6 +63,7 @@ SIGNATURES = {
     "lm_reset_stats": (c_int, [c_void_p]),
     "lm_get_stats": (c_int, [c_void_p, POINTER(c_int64), POINTER(c_int64), POINTER(c_double), POINTER(c_double)]),
     "lm_pair_launch_config": (c_int, [c_void_p, c_int, POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int)]),
+    "lm_pair_kernel_name": (c_char_p, [c_void_p, c_int]),
     "lm_version": (c_char_p, []),
 }
 
@@ -346,4 +347,6 @@ class Solver:
         v = [c_int(0) for _ in range(5)]
         self._check(lib().lm_pair_launch_config(self._h, int(nrhs), *[ctypes.byref(x) for x in v]))
         keys = ("i_tiles", "j_splits", "block", "targets_per_thread", "smem_bytes")
-        return {k: x.value for k, x in zip(keys, v)}
+        out = {k: x.value for k, x in zip(keys, v)}
+        out["kernel"] = lib().lm_pair_kernel_name(self._h, int(nrhs)).decode()
+        return out

@@ -20,6 +20,7 @@
 
 #include "../../include/lm.h"
 #include "rpy_pair.cuh"
+#include "rpy_small.cuh"
 #include "steric_pair.cuh"
 #include "lanczos_host.h"
 #include "tridiag_host.h"
@@ -165,6 +166,7 @@ int lm_set_wall(lm_solver* h, int enabled, double wall_height)
     h->have_pos = false;                              // the packed copy (raised heights, damping factors) depends on the wall
     h->bd_have_prev = false;
     for (auto& slot : h->plan_cache) slot.valid = false;
+    for (auto& slot : h->small_cache) slot.valid = false;
     return LM_OK;
 }
 
@@ -178,6 +180,13 @@ int lm_set_option(lm_solver* h, int option, int value)
         return LM_OK;
     case LM_OPT_GRAPH_REPLAY: h->graph_replay = value != 0; return LM_OK;
     case LM_OPT_SHARE_FIRST_APPLY: h->share_first_apply = value != 0; return LM_OK;
+    case LM_OPT_SMALL_KERNEL: {
+        const int S = value >> 8, W = value & 255;
+        const bool shape = value > 1 && (S == 1 || S == 2 || S == 4 || S == 8) && (W == 1 || W == 2 || W == 4 || W == 8);
+        if (value != 0 && value != 1 && !shape) return fail(h, LM_E_INVALID, "LM_OPT_SMALL_KERNEL: 0, 1 or (cluster << 8 | warps) with cluster, warps in {1, 2, 4, 8}");
+        h->small_kernel = value;
+        return LM_OK;
+    }
     default: return fail(h, LM_E_INVALID, "unknown option");
     }
 }
@@ -581,9 +590,27 @@ int lm_get_stats(lm_solver* h, int64_t* pair_kernel_launches, int64_t* aux_launc
     return rc;
 }
 
+const char* lm_pair_kernel_name(lm_solver* h, int nrhs)
+{
+    if (!h) return "";
+    const SmallPlan sp = h->precision == LM_F32 ? choose_small<float>(h, nrhs) : choose_small<double>(h, nrhs);
+    if (sp.variant >= 0) return "rpy_small_kernel";
+    const LaunchPlan plan = h->precision == LM_F32 ? choose_plan<float>(h, nrhs) : choose_plan<double>(h, nrhs);
+    return plan.variant >= 0 ? "rpy_pair_kernel" : "";
+}
+
 int lm_pair_launch_config(lm_solver* h, int nrhs, int* i_tiles, int* j_splits, int* block, int* targets_per_thread, int* smem_bytes)
 {
     if (!h) return LM_E_NULL;
+    const SmallPlan sp = h->precision == LM_F32 ? choose_small<float>(h, nrhs) : choose_small<double>(h, nrhs);
+    if (sp.variant >= 0) {            // the one-launch kernel: j is split over the `cluster` CTAs of a cluster (and over each CTA's warps)
+        if (i_tiles) *i_tiles = sp.i_tiles;
+        if (j_splits) *j_splits = sp.cluster;
+        if (block) *block = sp.warps * 32;
+        if (targets_per_thread) *targets_per_thread = 2;
+        if (smem_bytes) *smem_bytes = (int)sp.smem;
+        return LM_OK;
+    }
     LaunchPlan plan;
     int blk = 0, tpt = 0, smem = 0;
     if (h->precision == LM_F32) {

@@ -108,9 +108,57 @@ int ensure_capture_stream(lm_solver* h)
     return LM_OK;
 }
 
+// launch_small: the whole apply as ONE launch of rpy_small_kernel (small N): reads the caller's arrays, sums the
+// source splits through the cluster's distributed shared memory, writes the caller's outputs.
+template <typename T>
+int launch_small(lm_solver* h, int nrhs, const SmallPlan& sp, const RhsIn<T>& in, const RhsOut<T>& out, cudaStream_t st, bool timed)
+{
+    const auto& v = small_variants<T>(h)[sp.variant];
+    SmallParams<T> p;
+    p.pos = (const T*)h->pos_soa;
+    p.in = in;
+    p.out = out;
+    p.N = h->N;
+    p.npad = h->npad;
+    p.i_begin = h->row_begin;
+    p.i_end = h->row_end;
+    p.src_per_warp = sp.src_per_warp;
+    p.len_scale = (T)h->len_scale;
+    p.ghost_z = h->wall ? (T)(h->a * h->len_scale) : T(0);
+    p.c = make_consts<T>(h->eta, h->a * h->len_scale, h->len_scale);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(sp.i_tiles, sp.cluster, 1);
+    cfg.blockDim = dim3(sp.warps * 32, 1, 1);
+    cfg.dynamicSmemBytes = sp.smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 1;
+    attr[0].val.clusterDim.y = sp.cluster;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (timed) {
+        e0 = get_event(h);
+        e1 = get_event(h);
+        LM_CUDA(h, cudaEventRecord(e0, st));
+    }
+    LM_CUDA(h, cudaLaunchKernelEx(&cfg, v.kernel, p));
+    if (timed) {
+        LM_CUDA(h, cudaEventRecord(e1, st));
+        h->pending.emplace_back(e0, e1);
+    }
+    h->n_pair++;
+    h->pairs += (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N;
+    return LM_OK;
+}
+
 template <typename T> int apply_device(lm_solver* h, int nrhs, const RhsIn<T>& in, const RhsOut<T>& out, cudaStream_t st)
 {
     const int nc = h->angular ? 6 : 3;
+    const SmallPlan sp = choose_small<T>(h, nrhs);
+    if (sp.variant >= 0) return launch_small<T>(h, nrhs, sp, in, out, st, h->profiling);
     LaunchPlan plan;
     int rc = prepare_apply<T>(h, nrhs, plan);
     if (rc != LM_OK) return rc;

@@ -65,6 +65,31 @@ struct LaunchPlan {
     int i_tiles = 0, j_splits = 0, n_units = 0;
 };
 
+// ---------------------------------------------------------------- one-launch small-N kernel (rpy_small.cuh)
+template <typename T> struct SmallVariant {
+    void (*kernel)(const SmallParams<T>);
+    int nrhs, ang, wall;
+    size_t (*smem)(int warps, int src_per_warp);
+};
+template <typename T, int NRHS, bool ANG, bool WALL> SmallVariant<T> make_fused()
+{
+    return {rpy_small_kernel<T, NRHS, ANG, WALL>, NRHS, ANG, WALL, small_smem_bytes<T, NRHS, ANG>};
+}
+template <typename T> std::vector<SmallVariant<T>> build_small_variants()
+{
+    return {make_fused<T, 1, false, false>(), make_fused<T, 2, false, false>(), make_fused<T, 4, false, false>(),
+            make_fused<T, 1, true, false>(),  make_fused<T, 2, true, false>(),
+            make_fused<T, 1, false, true>(),  make_fused<T, 2, false, true>(),
+            make_fused<T, 1, true, true>(),   make_fused<T, 2, true, true>()};
+}
+constexpr size_t SMALL_MAX_SMEM = 96 * 1024;      // dynamic shared memory the small kernel may ask for
+
+struct SmallPlan {
+    int variant = -1;
+    int i_tiles = 0, cluster = 0, warps = 0, src_per_warp = 0;
+    size_t smem = 0;
+};
+
 }  // namespace lm
 
 // ---------------------------------------------------------------- NCCL, loaded at run time (row-sharded applies only)
@@ -179,6 +204,12 @@ struct lm_solver {
     // variants (typed; only the handle's precision is populated)
     std::vector<Variant<float>> vf;
     std::vector<Variant<double>> vd;
+    std::vector<SmallVariant<float>> sf;
+    std::vector<SmallVariant<double>> sd;
+    // one-launch small-N kernel (LM_OPT_SMALL_KERNEL): 1 = where the launch chooser prefers it, 0 = never,
+    // (cluster << 8 | warps) = always, with that shape (plan sweeps)
+    int small_kernel = 1;
+    struct SmallSlot { bool valid = false; int64_t rb = 0, re = 0; int mode = 0; lm::SmallPlan plan; } small_cache[lm::MAX_RHS + 1];
 
     // launch plans are pure functions of (nrhs, row range): cached, the chooser's search is off the per-call path
     struct PlanSlot { bool valid = false; int64_t rb = 0, re = 0; lm::LaunchPlan plan; } plan_cache[lm::MAX_RHS + 1];
@@ -270,6 +301,10 @@ template <typename T> std::vector<Variant<T>>& variants(lm_solver* h);
 template <> std::vector<Variant<float>>& variants<float>(lm_solver* h) { return h->vf; }
 template <> std::vector<Variant<double>>& variants<double>(lm_solver* h) { return h->vd; }
 
+template <typename T> std::vector<SmallVariant<T>>& small_variants(lm_solver* h);
+template <> std::vector<SmallVariant<float>>& small_variants<float>(lm_solver* h) { return h->sf; }
+template <> std::vector<SmallVariant<double>>& small_variants<double>(lm_solver* h) { return h->sd; }
+
 template <typename T> int init_variants(lm_solver* h)
 {
     auto& vs = variants<T>(h);
@@ -280,7 +315,74 @@ template <typename T> int init_variants(lm_solver* h)
         LM_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)v.kernel, v.block, v.smem));
         v.ctas_per_sm = std::max(nb, 1);
     }
+    auto& ss = small_variants<T>(h);
+    ss = build_small_variants<T>();
+    for (auto& v : ss) LM_CUDA(h, cudaFuncSetAttribute((const void*)v.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMALL_MAX_SMEM));
     return LM_OK;
+}
+
+// FP-pipe issue cycles one warp spends per source (two targets per lane): the algorithmic lane-operations of
+// DESIGN.md sec. 7 x the issue cost of a packed fp32 instruction (2.1 cycles) or of two fp64 ones (2 x 2 cycles).
+inline double cycles_per_source(const lm_solver* h, int nrhs)
+{
+    const double ops = (h->angular ? 16.0 + 32.0 * nrhs : 11.0 + 10.0 * nrhs) + (h->precision == LM_F64 ? 5.0 : 0.0);
+    return ops * (h->wall ? 3.4 : 1.0) * (h->precision == LM_F64 ? 4.0 : 2.1);
+}
+
+// The shape of the one-launch kernel for this apply, or variant < 0 where the general path (TMA-staged tiles, 2-4
+// targets per thread, partials through global memory) is the better one.  A CTA owns 64 targets; its W warps and
+// the S CTAs of its cluster split the sources.  Cost model in SM cycles, fitted to phase timings on B200 (clock64
+// stamps, N = 256 ... 2048): a lone warp per SM sub-partition is latency-bound (1.3-1.6 x the issue cycles per
+// source), warps sharing a sub-partition are issue-bound (x 1.07 fp64, x 1.4 fp32: the packed fp32 body leaves issue
+// slots to MUFU / LDS / vote); staging costs ~900 cycles + ~500 per round of 2 elements per thread; the warp sums,
+// the push through distributed shared memory, the wait and the final sum ~1300.
+template <typename T> SmallPlan choose_small(lm_solver* h, int nrhs)
+{
+    SmallPlan best;
+    if (nrhs < 1 || nrhs > MAX_RHS || h->small_kernel == 0 || h->dist_ranks > 0) return best;
+    auto& slot = h->small_cache[nrhs];
+    if (slot.valid && slot.rb == h->row_begin && slot.re == h->row_end && slot.mode == h->small_kernel) return slot.plan;
+    const auto& vs = small_variants<T>(h);
+    int vi = -1;
+    for (int i = 0; i < (int)vs.size(); ++i)
+        if (vs[i].nrhs == nrhs && vs[i].ang == h->angular && vs[i].wall == h->wall) vi = i;
+    const int64_t rows = std::max<int64_t>(h->row_end - h->row_begin, 0);
+    const bool f64 = h->precision == LM_F64;
+    const double issue = cycles_per_source(h, nrhs), lone = issue * (f64 ? 1.3 : 1.6), shared = issue * (f64 ? 1.07 : 1.4);
+    const bool forced = h->small_kernel > 1;
+    // beyond this the general path wins (measured crossover: fp32 translational N ~ 5000, fp64 ~ 3500)
+    const bool in_range = forced || (double)rows * (double)h->N * issue <= 1.2e9;
+    if (vi >= 0 && rows > 0 && in_range) {
+        const int i_tiles = (int)((rows + SM_TARGETS - 1) / SM_TARGETS);
+        double best_cost = 1e300;
+        for (int S = 1; S <= SM_MAX_CLUSTER; S *= 2)
+            for (int W = 1; W <= SM_MAX_WARPS; W *= 2) {
+                if (forced && (S != (h->small_kernel >> 8) || W != (h->small_kernel & 255))) continue;
+                const int spw = (int)(((h->N + (int64_t)S * W - 1) / ((int64_t)S * W) + 3) / 4 * 4);
+                const size_t smem = vs[vi].smem(W, spw);
+                if (smem > SMALL_MAX_SMEM) continue;
+                const double per_sm = std::ceil((double)i_tiles * S / h->sm_count);
+                const double warps_sub = std::ceil(per_sm * W / 4.0);
+                const double loop = spw * std::max(lone, shared * warps_sub);
+                const double rounds = std::ceil(3.0 * spw / 64.0);
+                const double cost = loop + 900.0 + 500.0 * rounds + 1300.0 + 20.0 * (S + W);
+                if (cost < best_cost) {
+                    best_cost = cost;
+                    best.variant = vi;
+                    best.i_tiles = i_tiles;
+                    best.cluster = S;
+                    best.warps = W;
+                    best.src_per_warp = spw;
+                    best.smem = smem;
+                }
+            }
+    }
+    slot.valid = true;
+    slot.rb = h->row_begin;
+    slot.re = h->row_end;
+    slot.mode = h->small_kernel;
+    slot.plan = best;
+    return best;
 }
 
 // Pick the variant and the number of j-splits.  Sources are dealt to the splits in units of SUB, as

@@ -625,13 +625,17 @@ def test_sqrt_mdot_w_batch_noconv_and_errors(lm, torch):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_repeated_small_applies_replay_a_graph_on_current_data(lm, torch, prec):
+@pytest.mark.parametrize("small_kernel", [0, 1])
+def test_repeated_small_applies_replay_a_graph_on_current_data(lm, torch, prec, small_kernel):
     """Short applies called again with the same buffers are replayed as a CUDA graph: the
     replay must read the buffers' CURRENT contents (forces changed in place, positions re-set), and calls with
-    other buffers, other right-hand-side counts or a row range must not be served by a stale graph."""
+    other buffers, other right-hand-side counts or a row range must not be served by a stale graph.  With the
+    one-launch kernel off this size takes the graph-replayed general path (as N ~ 5000 ... 14000 always does); with
+    it on, the same sequence of calls runs on rpy_small_kernel."""
     N = 700
     c = workloads.random_case(N, 15.0, 77, prec, False)
     s = lm.Solver(prec, N)
+    s.set_option(lm.LM_OPT_SMALL_KERNEL, small_kernel)
     X, F = dev(torch, c["pos"]).reshape(-1), dev(torch, c["forces"]).reshape(-1).clone()
     U = torch.empty(3 * N, dtype=s.torch_dtype, device="cuda")
     s.set_positions(X)
