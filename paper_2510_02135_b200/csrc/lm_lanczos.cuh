@@ -123,6 +123,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     int remaining = nv;
     for (int q = 0; q < nv; ++q) {
         stop[q].set_gram_column(0, hg(q));
+        if (!std::isfinite((double)ab(q)[1])) return fail(h, LM_E_CUDA, "Lanczos: non-finite noise");
         znorm[q] = std::sqrt(ab(q)[1]);
         if (!(znorm[q] > 0.0)) { done[q] = conv[q] = 1; --remaining; }            // zero noise: M^{1/2} 0 = 0
     }
