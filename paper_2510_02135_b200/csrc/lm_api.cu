@@ -180,6 +180,11 @@ int lm_set_option(lm_solver* h, int option, int value)
         return LM_OK;
     case LM_OPT_GRAPH_REPLAY: h->graph_replay = value != 0; return LM_OK;
     case LM_OPT_SHARE_FIRST_APPLY: h->share_first_apply = value != 0; return LM_OK;
+    case LM_OPT_J_SPLITS:
+        if (value < 0) return fail(h, LM_E_INVALID, "LM_OPT_J_SPLITS: 0 (chosen by the library) or the number of j-splits");
+        h->force_splits = value;
+        for (auto& slot : h->plan_cache) slot.valid = false;
+        return LM_OK;
     case LM_OPT_SMALL_KERNEL: {
         const int S = value >> 8, W = value & 255;
         const bool shape = value > 1 && (S == 1 || S == 2 || S == 4 || S == 8) && (W == 1 || W == 2 || W == 4 || W == 8);

@@ -209,6 +209,7 @@ struct lm_solver {
     // one-launch small-N kernel (LM_OPT_SMALL_KERNEL): 1 = where the launch chooser prefers it, 0 = never,
     // (cluster << 8 | warps) = always, with that shape (plan sweeps)
     int small_kernel = 1;
+    int force_splits = 0;      // LM_OPT_J_SPLITS: > 0 fixes the number of j-splits of the general path (plan sweeps)
     struct SmallSlot { bool valid = false; int64_t rb = 0, re = 0; int mode = 0; lm::SmallPlan plan; } small_cache[lm::MAX_RHS + 1];
 
     // launch plans are pure functions of (nrhs, row range): cached, the chooser's search is off the per-call path
@@ -409,6 +410,7 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
         const int max_splits = std::min(units, 256);
         const int min_splits = (int)std::min<int64_t>(max_splits, (h->npad + MAX_SOURCES_PER_CTA - 1) / MAX_SOURCES_PER_CTA);
         for (int s = min_splits; s <= max_splits; ++s) {
+            if (h->force_splits > 0 && s != std::min(std::max(h->force_splits, min_splits), max_splits)) continue;
             const int64_t src = (int64_t)((units + s - 1) / s) * v.sub;            // sources of the largest split
             const int64_t ctas = (int64_t)i_tiles * s;
             const int64_t full = ctas / slots, rem = ctas % slots;
