@@ -246,11 +246,15 @@ int lm_mdot_rows(lm_solver* h, int64_t row_begin, int64_t row_count, const void*
  *   LM_OPT_J_SPLITS           0 (default): the launch chooser sizes the grid | s > 0: the general path deals the sources to
  *                             exactly s j-splits (clamped to what the problem allows) -- for plan sweeps; results are
  *                             the same up to summation order.
+ *   LM_OPT_GATHER_IN_PLACE    1 (default): a row-sharded apply (lm_dist_init) whose row blocks tile [0, N) exactly (the
+ *                             number of ranks divides N) all-gathers straight into the caller's output arrays | 0: always
+ *                             through the handle's own all-gather buffers and a device-to-device copy (the path taken
+ *                             anyway when the last block is short).
  * lm_lanczos_history: what the last Lanczos call measured for noise vector `vec` of its (last) group: for iteration
  *   i + 1 (i < cap): alpha[i], beta[i], step[i] = s_{i+1} (NaN for i = 0), estimate[i] = e_{i+1} (NaN for i < 2; NaN
  *   throughout under LM_RULE_STEP).  Any output may be NULL.  Returns the number of iterations recorded. */
 enum { LM_RULE_ESTIMATE = 0, LM_RULE_STEP = 1 };
-enum { LM_OPT_LANCZOS_RULE = 0, LM_OPT_GRAPH_REPLAY = 1, LM_OPT_SHARE_FIRST_APPLY = 2, LM_OPT_SMALL_KERNEL = 3, LM_OPT_J_SPLITS = 4 };
+enum { LM_OPT_LANCZOS_RULE = 0, LM_OPT_GRAPH_REPLAY = 1, LM_OPT_SHARE_FIRST_APPLY = 2, LM_OPT_SMALL_KERNEL = 3, LM_OPT_J_SPLITS = 4, LM_OPT_GATHER_IN_PLACE = 5 };
 int lm_set_option(lm_solver* h, int option, int value);
 int lm_set_max_iter(lm_solver* h, int max_iter);     /* default 100; 1 <= max_iter <= 1000 */
 int lm_last_iterations(const lm_solver* h);           /* iterations of the last Lanczos call (or < 0) */

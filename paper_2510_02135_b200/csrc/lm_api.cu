@@ -180,6 +180,7 @@ int lm_set_option(lm_solver* h, int option, int value)
         return LM_OK;
     case LM_OPT_GRAPH_REPLAY: h->graph_replay = value != 0; return LM_OK;
     case LM_OPT_SHARE_FIRST_APPLY: h->share_first_apply = value != 0; return LM_OK;
+    case LM_OPT_GATHER_IN_PLACE: h->gather_in_caller = value != 0; return LM_OK;
     case LM_OPT_J_SPLITS:
         if (value < 0) return fail(h, LM_E_INVALID, "LM_OPT_J_SPLITS: 0 (chosen by the library) or the number of j-splits");
         h->force_splits = value;

@@ -25,7 +25,8 @@ template <typename T> int prepare_apply(lm_solver* h, int nrhs, LaunchPlan& plan
 // Only the target rows [h->row_begin, h->row_end) are computed.  With a communicator (lm_dist_init) those are
 // this rank's block: the kernel writes into all-gather buffers of 3 B ranks elements, ONE grouped
 // ncclAllGather (in place: rank r's segment starts at 3 B r) completes every output on every rank, and the
-// first 3N elements are copied to the caller's buffers.
+// first 3N elements are copied to the caller's buffers -- unless the blocks tile [0, N) exactly (ranks divides N):
+// then the caller's arrays are the all-gather buffers and nothing is copied.
 template <typename T>
 int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>& out, cudaStream_t st, bool timed, int reduce_from = 0)
 {
@@ -34,7 +35,9 @@ int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>&
     const bool dist = h->dist_ranks > 0;
     RhsOut<T> kout = out;
     const size_t seg = (size_t)3 * h->rows_per_rank;                       // elements each rank contributes
-    if (dist) {
+    // the blocks tile [0, N) exactly (ranks divides N): the caller's arrays ARE the all-gather buffers, no copy-out
+    const bool in_caller = dist && h->gather_in_caller && seg * h->dist_ranks == (size_t)3 * h->N;
+    if (dist && !in_caller) {
         const size_t bytes = seg * h->dist_ranks * sizeof(T);
         for (int q = 0; q < nrhs; ++q) {
             for (int part = 0; part < (h->angular ? 2 : 1); ++part) {
@@ -80,14 +83,14 @@ int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>&
         int nrc = nccl.GroupStart();
         for (int q = 0; q < nrhs && nrc == 0; ++q)
             for (int part = 0; part < (h->angular ? 2 : 1) && nrc == 0; ++part) {
-                T* buf = (T*)h->gath[2 * q + part];
+                T* buf = in_caller ? (part ? out.ang[q] : out.lin[q]) : (T*)h->gath[2 * q + part];
                 nrc = nccl.AllGather(buf + seg * h->dist_rank, buf, seg, dtype, (NcclApi::Comm)h->nccl_comm, st);
             }
         const int nrc_end = nccl.GroupEnd();
         if (nrc == 0) nrc = nrc_end;
         if (nrc != 0) return fail(h, LM_E_CUDA, std::string("ncclAllGather failed: ") + nccl.GetErrorString(nrc));
         const size_t out_bytes = (size_t)3 * h->N * sizeof(T);
-        for (int q = 0; q < nrhs; ++q) {
+        for (int q = 0; q < nrhs && !in_caller; ++q) {
             LM_CUDA(h, cudaMemcpyAsync(out.lin[q], h->gath[2 * q], out_bytes, cudaMemcpyDeviceToDevice, st));
             if (h->angular) LM_CUDA(h, cudaMemcpyAsync(out.ang[q], h->gath[2 * q + 1], out_bytes, cudaMemcpyDeviceToDevice, st));
         }

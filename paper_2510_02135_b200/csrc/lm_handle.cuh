@@ -209,6 +209,7 @@ struct lm_solver {
     // one-launch small-N kernel (LM_OPT_SMALL_KERNEL): 1 = where the launch chooser prefers it, 0 = never,
     // (cluster << 8 | warps) = always, with that shape (plan sweeps)
     int small_kernel = 1;
+    bool gather_in_caller = true;   // LM_OPT_GATHER_IN_PLACE: row-sharded applies all-gather straight into the caller's arrays when the blocks tile [0, N)
     int force_splits = 0;      // LM_OPT_J_SPLITS: > 0 fixes the number of j-splits of the general path (plan sweeps)
     struct SmallSlot { bool valid = false; int64_t rb = 0, re = 0; int mode = 0; lm::SmallPlan plan; } small_cache[lm::MAX_RHS + 1];
 

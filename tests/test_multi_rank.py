@@ -105,3 +105,80 @@ def test_row_blocks_across_two_gloo_ranks():
         assert p.exitcode == 0
     for rank, blocks, ok in res:
         assert blocks == [[0, 501], [501, 1001]] and ok
+
+
+def _stop_worker(rank, world, port, out):
+    """Both ranks replay the host side of a row-sharded Lanczos run (csrc/lanczos_host.h through tests/hooks): the
+    stopping test on their own copies of alpha_k, beta_k and the Gram columns, then agree_on_stops with a gloo
+    broadcast from rank 0 as the transport.  Rank 1's scalars are deliberately perturbed, so its own verdict comes
+    at another step; every iteration ends with a collective (the stand-in for the next apply's all-gather), which
+    would hang if the ranks disagreed on whether there IS a next iteration."""
+    sys.path.insert(0, ROOT)
+    import ctypes
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from oracle import rpy
+    from tests import hooks
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    L = hooks.lib()
+    dp = ctypes.POINTER(ctypes.c_double)
+    rng = np.random.default_rng(11)
+    N, tol = 150, 1e-3
+    pos = rng.random((N, 3)) * 9.0
+    M = rpy.dense(pos)
+    z = rng.standard_normal(3 * N)
+    wobble = np.random.default_rng(5)                       # rank 1 sees slightly different scalars
+    V = [z / np.linalg.norm(z)]
+    st = L.hook_stopper_new(0, tol, 1e-14, 100)
+    col = lambda m: np.ascontiguousarray([V[j] @ V[m] for j in range(m + 1)])
+    L.hook_stopper_gram_column(st, 0, col(0).ctypes.data_as(dp))
+
+    def exchange(word_ptr):
+        t = torch.tensor([int(word_ptr[0])], dtype=torch.int64)
+        dist.broadcast(t, src=0)
+        word_ptr[0] = int(t.item())
+
+    cb = hooks.EXCHANGE_FN(exchange)
+    beta_prev, k_local, k_agreed = 0.0, None, None
+    for k in range(1, 101):
+        w = M @ V[k - 1] - (beta_prev * V[k - 2] if k > 1 else 0.0)
+        alpha = w @ V[k - 1]
+        w = w - alpha * V[k - 1]
+        beta = np.linalg.norm(w)
+        V.append(w / beta)
+        eps = 0.0 if rank == 0 else 3e-2 * wobble.standard_normal()
+        verdict = L.hook_stopper_feed(st, k, float(alpha * (1 + eps)), float(beta * (1 - eps)))
+        if verdict == 1 and k_local is None:
+            k_local = k
+        word = L.hook_agree_on_stops(1 if verdict == 1 else 0, cb, 1)
+        if word & 1:
+            k_agreed = k
+            break
+        L.hook_stopper_advance(st)
+        L.hook_stopper_gram_column(st, k, col(k).ctypes.data_as(dp))
+        beta_prev = beta
+        dist.all_reduce(torch.zeros(1))                     # the next iteration's collective: both ranks must post it
+    L.hook_stopper_free(st)
+    out.put((rank, k_local, k_agreed))
+    dist.destroy_process_group()
+
+
+def test_lanczos_stop_is_rank_zeros_verdict_even_when_the_ranks_scalars_differ():
+    """VERDICT r1 item 6 / ADVICE: ranks must not part ways on the stopping decision (a rank that goes on posts an
+    all-gather the others never match).  Two gloo ranks, rank 1 with perturbed scalars: both leave the loop at rank
+    0's step, although rank 1's own test says otherwise."""
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = 35500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_stop_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = dict((r, (kl, ka)) for r, kl, ka in (out.get(timeout=180) for _ in procs))
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    assert res[0][0] == res[0][1] == res[1][1]              # rank 0's verdict is everybody's
+    assert res[1][0] != res[0][0]                           # ... and rank 1's own verdict really was another one
