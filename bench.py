@@ -389,6 +389,60 @@ def lanczos_true_error(lm, torch, arm, y_f32):
     return err
 
 
+def run_fig7(args):
+    """--fig7: the paper's Fig. 7 protocol on this library: time of one Mdot vs N on a perturbed FCC
+    lattice without overlaps, monopoles only, two number densities, for NBody with open boundaries and with a bottom
+    wall.  Context, not a comparison (the paper's curves are an RTX A6000 and exist only as a figure).  Each point: applies
+    back to back on one stream (the loop a user runs; inputs stay in L2 below N ~ 10^6), best of 3.  One JSON line."""
+    import torch
+
+    import paper_2510_02135_b200 as lm
+    from paper_2510_02135_b200 import workloads
+    cells = [2, 3, 4, 6, 8, 10, 13, 16, 20, 26, 32, 40, 51, 64]      # N = 4 n^3: 32 ... 1048576
+    out = {"protocol": "perturbed FCC lattice (jitter 0.1 a, no overlaps), monopoles, applies back to back, best of 3, ms per Mdot",
+           "densities": [0.01, 0.1], "rows": []}
+    for prec in ("f32", "f64"):
+        tdt = torch.float32 if prec == "f32" else torch.float64
+        for wall in (False, True):
+            for n in cells:
+                N = 4 * n ** 3
+                if (prec == "f64" and N > 300000) or (wall and N > 300000) or (args.N and N > args.N):
+                    continue
+                row = {"precision": prec, "geometry": "single_wall" if wall else "open", "N": N, "ms": []}
+                for rho in out["densities"]:
+                    x = workloads.fcc(n, rho, 0.1, 7)
+                    if wall:
+                        x[:, 2] += 1.5 - x[:, 2].min()                 # lowest layer 1.5 a above the wall at z = 0
+                    pos = torch.from_numpy(x.reshape(-1)).to(tdt).cuda()
+                    F = torch.randn(3 * N, dtype=tdt, device="cuda")
+                    U = torch.empty_like(F)
+                    s = lm.Solver(prec, N)
+                    if wall:
+                        s.set_wall(True, 0.0)
+                    s.set_positions(pos)
+                    pairs = float(N) * N * (3.4 if wall else 1.0) * (2.5 if prec == "f64" else 1.0)
+                    reps = int(max(2, min(300, 3e11 / pairs)))
+                    for _ in range(3):
+                        s.mdot(F, None, U)
+                    best = None
+                    for _ in range(3):
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        torch.cuda.synchronize()
+                        e0.record()
+                        for _ in range(reps):
+                            s.mdot(F, None, U)
+                        e1.record()
+                        torch.cuda.synchronize()
+                        ms = e0.elapsed_time(e1) / reps
+                        best = ms if best is None else min(best, ms)
+                    row["ms"].append(best)
+                    row["kernel"] = s.pair_launch_config(1)["kernel"]
+                    s.close()
+                row["gpairs_per_s"] = float(N) * N / (min(row["ms"]) * 1e-3) / 1e9
+                out["rows"].append(row)
+    print(json.dumps({"fig7": out}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -400,6 +454,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the sub-records of the other four configs")
+    ap.add_argument("--fig7", action="store_true", help="the paper's Fig. 7 protocol (Mdot time vs N, open and bottom-wall NBody) instead of a config")
     ap.add_argument("--lanczos-rule", default="estimate", choices=["estimate", "step"], help="stopping rule (DESIGN.md reading S3)")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "sharded"],
                     help="N > 1 ranks: independent replicas (default, weak scaling) or ONE problem row-sharded over the ranks "
@@ -432,6 +487,11 @@ def main():
 
     import paper_2510_02135_b200 as lm
     from paper_2510_02135_b200 import multi, probe
+
+    if args.fig7:
+        if rank == 0:
+            run_fig7(args)
+        return 0
 
     sharded = args.parallelism == "sharded" and world > 1
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2

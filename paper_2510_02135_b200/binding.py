@@ -10,6 +10,7 @@ There is no fallback: if the library cannot be built or loaded, importing ``lib(
 from __future__ import annotations
 
 import ctypes
+import weakref
 import os
 from ctypes import POINTER, c_char_p, c_double, c_int, c_int64, c_void_p
 
@@ -122,6 +123,17 @@ def _ptr(x):
     return c_void_p(x.data_ptr())
 
 
+def _raw_stream_fn():
+    try:
+        import torch
+        return torch._C._cuda_getCurrentRawStream
+    except Exception:
+        return None
+
+
+_RAW_STREAM = _raw_stream_fn()
+
+
 def _stream_ptr(stream):
     if stream is None:
         import torch
@@ -145,6 +157,14 @@ class Solver:
         if rc != LM_OK:
             self._h = c_void_p()
             raise LmError(rc, "lm_create failed (bad argument, or no CUDA device)")
+        L = lib()
+        self._n3, self._seen = 3 * self.N, {}
+        self._lm_set_positions, self._lm_mdot, self._lm_mdot_batch, self._lm_sqrt_mdot_w = L.lm_set_positions, L.lm_mdot, L.lm_mdot_batch, L.lm_sqrt_mdot_w
+        try:
+            import torch
+            self._device = torch.cuda.current_device()          # lm_create bound the handle to the current device
+        except Exception:
+            self._device = 0
 
     # -- helpers
     @property
@@ -173,6 +193,29 @@ class Solver:
         if not host and not x.is_cuda:
             raise TypeError("device entry point needs a CUDA tensor (use the *_host call for host arrays)")
 
+    def _dev(self, x, n):
+        """Device argument of a hot call: the tensor's address as an int (None -> NULL).  dtype, size, device and
+        contiguity are checked the first time a tensor OBJECT is seen (they cannot change under the same object short
+        of an in-place resize); later calls with the same object only read its address -- a time-stepping loop calls with
+        the same few tensors millions of times and a small apply is otherwise bound by this marshalling."""
+        if x is None:
+            return None
+        seen = self._seen
+        ent = seen.get(id(x))
+        if ent is None or ent[0]() is not x or ent[1] != n:
+            self._expect(x, n, False)
+            if not x.is_contiguous():
+                raise ValueError("tensor must be contiguous")
+            if len(seen) > 256:
+                seen.clear()
+            seen[id(x)] = (weakref.ref(x), n)
+        return x.data_ptr()
+
+    def _stream(self, stream):
+        if stream is None:
+            return _RAW_STREAM(self._device) if _RAW_STREAM is not None else _stream_ptr(None)
+        return stream if isinstance(stream, int) else stream.cuda_stream
+
     def close(self):
         if getattr(self, "_h", None) and self._h.value:
             lib().lm_destroy(self._h)
@@ -190,24 +233,27 @@ class Solver:
 
     # -- device entry points (torch CUDA tensors)
     def set_positions(self, pos, stream=None):
-        self._expect(pos, 3 * self.N, False)
-        self._check(lib().lm_set_positions(self._h, _ptr(pos), _stream_ptr(stream)))
+        rc = self._lm_set_positions(self._h, self._dev(pos, self._n3), self._stream(stream))
+        if rc != LM_OK:
+            self._check(rc)
 
     def mdot(self, forces, torques, lin_out, ang_out=None, stream=None):
-        for x in (forces, torques, lin_out, ang_out):
-            self._expect(x, 3 * self.N, False)
-        self._check(lib().lm_mdot(self._h, _ptr(forces), _ptr(torques), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+        n3, d = self._n3, self._dev
+        rc = self._lm_mdot(self._h, d(forces, n3), d(torques, n3), d(lin_out, n3), d(ang_out, n3), self._stream(stream))
+        if rc != LM_OK:
+            self._check(rc)
 
     def mdot_batch(self, nrhs, forces, torques, lin_out, ang_out=None, stream=None):
-        for x in (forces, torques, lin_out, ang_out):
-            self._expect(x, nrhs * 3 * self.N, False)
-        self._check(lib().lm_mdot_batch(self._h, int(nrhs), _ptr(forces), _ptr(torques), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+        n, d = nrhs * self._n3, self._dev
+        rc = self._lm_mdot_batch(self._h, int(nrhs), d(forces, n), d(torques, n), d(lin_out, n), d(ang_out, n), self._stream(stream))
+        if rc != LM_OK:
+            self._check(rc)
 
     def sqrt_mdot_w(self, noise, tol, lin_out, ang_out=None, stream=None, allow_noconv=False) -> int:
-        self._expect(noise, (6 if self.angular else 3) * self.N, False)
+        n3, d = self._n3, self._dev
         iters = c_int(0)
-        self._check(lib().lm_sqrt_mdot_w(self._h, _ptr(noise), float(tol), _ptr(lin_out), _ptr(ang_out), ctypes.byref(iters),
-                                         _stream_ptr(stream)), allow=(LM_E_NOCONV,) if allow_noconv else ())
+        self._check(self._lm_sqrt_mdot_w(self._h, d(noise, (2 if self.angular else 1) * n3), float(tol), d(lin_out, n3), d(ang_out, n3),
+                                         ctypes.byref(iters), self._stream(stream)), allow=(LM_E_NOCONV,) if allow_noconv else ())
         return iters.value
 
     def sqrt_mdot_w_batch(self, nvec, noise, tol, lin_out, ang_out=None, stream=None, allow_noconv=False):
@@ -220,8 +266,9 @@ class Solver:
         return list(iters)
 
     def hydrodynamic_velocities(self, forces, torques, noise, noise_prefactor, tol, lin_out, ang_out=None, stream=None):
-        self._check(lib().lm_hydrodynamic_velocities(self._h, _ptr(forces), _ptr(torques), _ptr(noise), float(noise_prefactor),
-                                                     float(tol), _ptr(lin_out), _ptr(ang_out), _stream_ptr(stream)))
+        n3, d = self._n3, self._dev
+        self._check(lib().lm_hydrodynamic_velocities(self._h, d(forces, n3), d(torques, n3), d(noise, (2 if self.angular else 1) * n3),
+                                                     float(noise_prefactor), float(tol), d(lin_out, n3), d(ang_out, n3), self._stream(stream)))
 
     # -- host entry points (numpy arrays; pinned memory makes the copies asynchronous)
     def set_positions_host(self, pos, stream=None):

@@ -98,6 +98,15 @@ def generate(index: int, N: int | None = None, seed: int | None = None) -> dict:
     return dict(cfg=cfg, N=N, pos=cast(pos), forces=cast(forces), torques=cast(torques), noise=cast(noise))
 
 
+def noise_for(index: int, N: int | None = None) -> np.ndarray:
+    """A seeded N(0,1) noise vector W (dof entries, layout [3N linear | 3N angular]) for ANY config, in its precision:
+    configs 1, 2, 4, 5 are M.F workloads, but lm_sqrt_mdot_w is tested on their particle configurations too."""
+    cfg = CONFIGS[index]
+    N = cfg.N if N is None else N
+    rng = np.random.default_rng(10_000 + cfg.seed)
+    return np.ascontiguousarray(rng.standard_normal((6 if cfg.angular else 3) * N).astype(np_dtype(cfg.precision)))
+
+
 def random_case(N: int, side: float, seed: int, precision: str = "f64", angular: bool = False,
                 with_noise: bool = False) -> dict:
     """Free-form small case for tests: uniform in a cube of the given side (many overlaps if small)."""
