@@ -299,7 +299,8 @@ class Arm:
             best = us if best is None else min(best, us)
         instr, _ = work_per_pair(self.cfg.angular, 1, self.f64)
         return {"us_per_apply": best, "gpairs_per_s": float(self.N) * self.N / (best * 1e-6) / 1e9, "applies": reps,
-                "what": "applies back to back on one stream through the binding, no L2 flush, no set_positions (best of 3)"}
+                "what": "whole applies (launch overhead included) back to back on one stream through the binding, no L2 flush, no set_positions "
+                        "(best of 3); frac = the same lane-operations per pair over this time"}
 
     def measure(self, steps, warmup, flush, do_e2e, sampler=None):
         """value pass (profiling OFF: the code path a user gets, CUDA-graph replay included), a short profiled pass
@@ -554,6 +555,7 @@ def main():
                        "h2d_bytes_per_step": int(arm.h2d), "d2h_bytes_per_step": int(arm.d2h), "api": "lm_set_positions_host + lm_*_host (pinned host buffers)"}
     ss = arm.steady_state() if world == 1 else None
     if ss is not None:
+        ss["frac"] = roofline["lane_ops_per_pair"] * float(N) * N / (ss["us_per_apply"] * 1e-6) / 1e12 / roofline["peak"]
         line["steady_state"] = ss
     data_headline = arm.data
     arm.close()
@@ -581,6 +583,7 @@ def main():
             }
             ss2 = a2.steady_state()
             if ss2 is not None:
+                ss2["frac"] = r2["lane_ops_per_pair"] * float(a2.N) * a2.N / (ss2["us_per_apply"] * 1e-6) / 1e12 / r2["peak"]
                 sub[str(index)]["steady_state"] = ss2
             a2.close()
         line["configs"] = sub

@@ -114,12 +114,15 @@ int ensure_capture_stream(lm_solver* h)
 // launch_small: the whole apply as ONE launch of rpy_small_kernel (small N): reads the caller's arrays, sums the
 // source splits through the cluster's distributed shared memory, writes the caller's outputs.
 template <typename T>
-int launch_small(lm_solver* h, int nrhs, const SmallPlan& sp, const RhsIn<T>& in, const RhsOut<T>& out, cudaStream_t st, bool timed)
+int launch_small(lm_solver* h, int nrhs, const SmallPlan& sp, const RhsIn<T>& in, const RhsOut<T>& out, cudaStream_t st, bool timed,
+                 const int* in_index = nullptr, int64_t in_stride = 0, bool count = true)
 {
     const auto& v = small_variants<T>(h)[sp.variant];
     SmallParams<T> p;
     p.pos = (const T*)h->pos_soa;
     p.in = in;
+    p.in_index = in_index;
+    p.in_stride = in_stride;
     p.out = out;
     p.N = h->N;
     p.npad = h->npad;
@@ -152,8 +155,10 @@ int launch_small(lm_solver* h, int nrhs, const SmallPlan& sp, const RhsIn<T>& in
         LM_CUDA(h, cudaEventRecord(e1, st));
         h->pending.emplace_back(e0, e1);
     }
-    h->n_pair++;
-    h->pairs += (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N;
+    if (count) {
+        h->n_pair++;
+        h->pairs += (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N;
+    }
     return LM_OK;
 }
 

@@ -352,8 +352,12 @@ template <typename T> SmallPlan choose_small(lm_solver* h, int nrhs)
     const bool f64 = h->precision == LM_F64;
     const double issue = cycles_per_source(h, nrhs), lone = issue * (f64 ? 1.3 : 1.6), shared = issue * (f64 ? 1.07 : 1.4);
     const bool forced = h->small_kernel > 1;
-    // beyond this the general path wins (measured crossover: fp32 translational N ~ 5000, fp64 ~ 3500)
-    const bool in_range = forced || (double)rows * (double)h->N * issue <= 1.2e9;
+    // beyond this the general path wins (measured crossovers: fp32 translational N ~ 5000, fp64 ~ 3500;
+    // the register-heavy variants -- angular, several right-hand sides: NV = 6 ... 12 accumulated components -- hand over
+    // earlier, fp64 more so than fp32)
+    const int nv_comp = nrhs * (h->angular ? 6 : 3);
+    const double limit = 1.2e9 * (f64 ? 3.0 / nv_comp : std::min(1.0, 6.0 / nv_comp));
+    const bool in_range = forced || (double)rows * (double)h->N * issue <= limit;
     if (vi >= 0 && rows > 0 && in_range) {
         const int i_tiles = (int)((rows + SM_TARGETS - 1) / SM_TARGETS);
         double best_cost = 1e300;

@@ -78,7 +78,12 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     // launch plans: `plan` for the nv Lanczos vectors; `plan_det` for the first apply when a deterministic right-hand
     // side rides along (one more vector; only where a variant for nv + 1 exists).  Both sized before any launch.
     LaunchPlan plan, plan_det;
-    const bool share = det && choose_plan<T>(h, nv + 1).variant >= 0;
+    // Small N: the apply is ONE launch of rpy_small_kernel reading V[*newest] directly (no packed copy, no partials),
+    // and the vector part of an iteration ONE launch of lanczos_fused_step_kernel: 3 launches per
+    // iteration instead of 5-6.  M.[F;T] is then a (one-launch) apply of its own.
+    const SmallPlan sp = dof <= (int64_t)FUSED_BLOCK * 32 ? choose_small<T>(h, nv) : SmallPlan();
+    const bool small = sp.variant >= 0;
+    const bool share = det && !small && choose_plan<T>(h, nv + 1).variant >= 0;
     // no variant for nv + 1 vectors: M.[F;T] is a launch of its own, before the packed array holds v_1
     if (det && !share && (rc = apply_batch<T>(h, 1, det->f, det->t, det->lin, det->ang, st)) != LM_OK) return rc;
     if (share && (rc = prepare_apply<T>(h, nv + 1, plan_det)) != LM_OK) return rc;
@@ -145,7 +150,24 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     // the alpha kernel doubles as the split-j reduce of the apply (one launch less per vector and iteration),
     // except for row-sharded runs, where w must be all-gathered before any rank can use it
     auto fused = [&](const LaunchPlan& pl) { return pl.j_splits > 1 && pl.i_tiles > 0 && h->dist_ranks == 0; };
+    auto body_small = [&](cudaStream_t s2, bool timed) -> int {
+        RhsIn<T> in{};
+        for (int q = 0; q < nv; ++q) {
+            in.f[q] = Vq(q);
+            in.t[q] = h->angular ? Vq(q) + n3 : nullptr;
+        }
+        const int rc2 = launch_small<T>(h, nv, sp, in, out, s2, timed, h->d_newest, dof, false);
+        if (rc2 != LM_OK) return rc2;
+        for (int q = 0; q < nv; ++q)
+            lanczos_fused_step_kernel<T><<<1, FUSED_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q), dof, h->h_ab + (size_t)q * 2 * ld, q == nv - 1);
+        for (int q = 0; q < nv; ++q)
+            gram_column_kernel<T><<<dim3(gg, kmax + 1), VEC_BLOCK, 0, s2>>>(Vq(q), dof, h->d_newest, gchunk, h->d_gram_part, h->d_ticket,
+                                                                             h->h_gram + (size_t)q * ld * ld, ld);
+        LM_CUDA(h, cudaGetLastError());
+        return LM_OK;
+    };
     auto body = [&](cudaStream_t s2, bool timed, bool with_det) -> int {
+        if (small) return body_small(s2, timed);
         int rc2;
         const LaunchPlan& pl = with_det ? plan_det : plan;
         const int nr = with_det ? nv + 1 : nv;
@@ -177,7 +199,8 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     const bool lookahead = apply_cost < 2.0e9 && !dist;
     const bool use_graph = lookahead && !h->profiling && h->graph_replay;
     if (use_graph && remaining > 0) {
-        const lm_solver::GraphKey key = {h->V, h->w, h->vec_soa, h->partial, h->pos_soa, kmax, plan.variant, plan.j_splits, h->precision * 8 + nv};
+        const lm_solver::GraphKey key = {h->V, h->w, h->vec_soa, h->partial, h->pos_soa, kmax, small ? 1000 + sp.variant : plan.variant,
+                                         small ? sp.cluster * 16 + sp.warps : plan.j_splits, h->precision * 8 + nv};
         if (!h->lz_graph || std::memcmp(&key, &h->lz_key, sizeof key) != 0) {
             if (h->lz_graph) { LM_CUDA(h, cudaGraphExecDestroy(h->lz_graph)); h->lz_graph = nullptr; }
             cudaGraph_t graph = nullptr;
@@ -201,9 +224,15 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
             const int rc2 = body(st, h->profiling, with_det);
             if (rc2 != LM_OK) return rc2;
         }
-        if (with_det && plan_det.j_splits > 1 && fused(plan_det)) h->n_aux++;    // the deterministic vector's own reduce
-        count_apply(h, with_det ? plan_det : plan);
-        h->n_aux += 4 * nv;
+        if (small) {
+            h->n_pair++;
+            h->pairs += (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N;
+            h->n_aux += 2 * nv;
+        } else {
+            if (with_det && plan_det.j_splits > 1 && fused(plan_det)) h->n_aux++;    // the deterministic vector's own reduce
+            count_apply(h, with_det ? plan_det : plan);
+            h->n_aux += 4 * nv;
+        }
         ++enqueued;
         LM_CUDA(h, cudaEventRecord(h->lz_ev[k & 1], st));
         return LM_OK;

@@ -58,6 +58,8 @@ __device__ __forceinline__ void st_async(uint32_t raddr, double v, uint32_t rbar
 template <typename T> struct SmallParams {
     const T* __restrict__ pos;   // the handle's packed positions x | y | z (| h | b), each npad long
     RhsIn<T> in;                 // caller's arrays, interleaved xyz, 3N each; null = zeros
+    const int* in_index;         // null, or: every input array is read at in.f[q] + *in_index * in_stride (the Lanczos driver
+    int64_t in_stride;           //   passes its basis and the device-side index of the newest vector: one launch fits every iteration)
     RhsOut<T> out;               // caller's outputs, interleaved xyz
     int64_t N, npad;
     int64_t i_begin, i_end;      // target rows [i_begin, i_end)
@@ -128,6 +130,7 @@ __global__ void __launch_bounds__(SM_MAX_WARPS * 32) rpy_small_kernel(const Smal
     constexpr int STG_U = 2;
     const int B = blockDim.x;
     const int n3_here = 3 * (int)max((int64_t)0, min((int64_t)cta_src, p.N - j0));   // real values of this CTA per array
+    const int64_t in_off = (p.in_index ? (int64_t)(*p.in_index) * p.in_stride : 0) + 3 * j0;
     T* rhs = src + 3 * cta_src;                                // [NRHS][forces 3 cta_src (| torques 3 cta_src)]
     for (int base = tid; base < 3 * cta_src; base += STG_U * B) {        // positions need a third of the rounds
         T x[STG_U][3], f[NRHS][STG_U], t[ANG ? NRHS : 1][STG_U], b[STG_U];
@@ -144,8 +147,8 @@ __global__ void __launch_bounds__(SM_MAX_WARPS * 32) rpy_small_kernel(const Smal
             if constexpr (WALL) b[u] = real ? p.pos[4 * p.npad + j0 + idx / 3] : T(0);
 #pragma unroll
             for (int q = 0; q < NRHS; ++q) {
-                f[q][u] = (real && p.in.f[q]) ? p.in.f[q][3 * j0 + idx] : T(0);
-                if constexpr (ANG) t[q][u] = (real && p.in.t[q]) ? p.in.t[q][3 * j0 + idx] : T(0);
+                f[q][u] = (real && p.in.f[q]) ? p.in.f[q][in_off + idx] : T(0);
+                if constexpr (ANG) t[q][u] = (real && p.in.t[q]) ? p.in.t[q][in_off + idx] : T(0);
             }
         }
 #pragma unroll

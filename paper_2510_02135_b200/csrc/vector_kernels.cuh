@@ -280,6 +280,65 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__
     if (blockIdx.x == 0 && threadIdx.x == 0) host_ab[2 * (m + 1)] = a;
 }
 
+// Small N: the vector part of one Lanczos iteration -- lanczos_alpha_kernel, lanczos_beta_kernel and the scaling of
+// lanczos_scale_pack_kernel -- in ONE launch of one CTA (the vectors are a few thousand elements; three launches and
+// two grid-wide reductions cost more than the arithmetic).  Same operations and rounding points as those kernels:
+//   m = *newest;  w -= beta_{k-1} V[m-1] (m > 0);  alpha = w . V[m];  w -= alpha V[m];  beta^2 = |w|^2;  V[m+1] = w / beta;
+//   host_ab[2(m+1)] = alpha, host_ab[2(m+1)+1] = beta^2;  scal[1] = alpha, scal[2] = beta^2;  `advance`: *newest = m + 1.
+// No packed copy of V[m+1] is written: at these sizes the apply (rpy_small_kernel) reads V[*newest] itself.
+// Reductions: fp64, warp shuffles, then the 32 warp sums added in warp order by every thread (deterministic).
+constexpr int FUSED_BLOCK = 1024;
+__device__ __forceinline__ double cta_sum_1024(double v, double* warp_part)
+{
+    v = warp_sum(v);
+    __syncthreads();                                   // warp_part may still be read from the previous reduction
+    if ((threadIdx.x & 31) == 0) warp_part[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double s = 0.0;
+#pragma unroll
+    for (int w = 0; w < FUSED_BLOCK / 32; ++w) s += warp_part[w];
+    return s;
+}
+template <typename T>
+__global__ void __launch_bounds__(FUSED_BLOCK) lanczos_fused_step_kernel(T* __restrict__ w, T* __restrict__ V, int* newest, double* scal, int64_t n,
+                                                                         double* host_ab, int advance)
+{
+    __shared__ double warp_part[FUSED_BLOCK / 32];
+    const int m = *newest;
+    const T* v = V + (size_t)m * n;
+    const T* v_prev = m > 0 ? v - n : nullptr;
+    T* v_next = V + (size_t)(m + 1) * n;
+    const double bp = v_prev ? sqrt(scal[2]) : 0.0;
+    double s = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += FUSED_BLOCK) {
+        double wi = (double)w[i];
+        if (v_prev) {
+            wi = fma(-bp, (double)v_prev[i], wi);
+            w[i] = (T)wi;
+            wi = (double)w[i];                         // the dot product sees the stored (rounded) value
+        }
+        s = fma(wi, (double)v[i], s);
+    }
+    const double alpha = cta_sum_1024(s, warp_part);
+    s = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += FUSED_BLOCK) {
+        const T wi = (T)fma(-alpha, (double)v[i], (double)w[i]);
+        w[i] = wi;
+        s = fma((double)wi, (double)wi, s);
+    }
+    const double beta_sq = cta_sum_1024(s, warp_part);
+    const double nrm = sqrt(beta_sq);
+    const double inv = nrm > 0.0 ? 1.0 / nrm : 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += FUSED_BLOCK) v_next[i] = (T)((double)w[i] * inv);
+    if (threadIdx.x == 0) {
+        host_ab[2 * (m + 1)] = alpha;
+        host_ab[2 * (m + 1) + 1] = beta_sq;
+        scal[1] = alpha;
+        scal[2] = beta_sq;
+        if (advance) *newest = m + 1;
+    }
+}
+
 // Gram column for the stopping test (a9): with c = *newest the column of the vector just written,
 // g[j] = V[j] . V[c], j = 0..c, stored to host_gram[c * ld + j].  Lanczos without
 // re-orthogonalisation loses orthogonality of V, so |y_k - y_{k-1}| = |z| |V_k delta| is evaluated as

@@ -109,13 +109,16 @@ def test_steric_kernel(lm, torch, prec, N):
 
 
 @pytest.mark.parametrize("prec,angular", [("f64", False), ("f64", True), ("f32", False), ("f32", True)])
-@pytest.mark.parametrize("N,graph", [(300, 1), (300, 0), (9000, 0)])
-def test_lanczos_fixed_iterations(lm, torch, prec, angular, N, graph):
-    """Five Lanczos iterations (look-ahead; graph replay on or off; at N = 9000 the alpha kernel sums the j-split
-    partials itself) against the fp64 Lanczos oracle stopped at the same step."""
+@pytest.mark.parametrize("N,graph,small", [(300, 1, 1), (300, 0, 1), (300, 1, 0), (300, 0, 0), (9000, 0, 0)])
+def test_lanczos_fixed_iterations(lm, torch, prec, angular, N, graph, small):
+    """Five Lanczos iterations (look-ahead; graph replay on or off) against the fp64 Lanczos oracle stopped at the same
+    step, on the three driver paths: small N with the one-launch apply + fused vector step (rpy_small_kernel reading
+    V[*newest], lanczos_fused_step_kernel), small N on the general kernels, and N = 9000 where the alpha kernel sums the
+    j-split partials itself."""
     c = workloads.random_case(N, 2.0 * N ** (1.0 / 3.0), 9, prec, angular, with_noise=True)
     s = lm.Solver(prec, N, 1.0, 1.0, angular)
     s.set_option(lm.LM_OPT_GRAPH_REPLAY, graph)
+    s.set_option(lm.LM_OPT_SMALL_KERNEL, small)
     s.set_positions(dev(torch, c["pos"]))
     s.set_max_iter(5)
     y = torch.empty(3 * N, dtype=s.torch_dtype, device="cuda")

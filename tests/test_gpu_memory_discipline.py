@@ -120,13 +120,14 @@ def test_apply_touches_only_its_buffers_and_is_deterministic(lm, torch, prec, an
 
 
 @pytest.mark.parametrize("prec,angular", [("f64", False), ("f32", True)])
-@pytest.mark.parametrize("N,graph", [(300, 1), (300, 0), (9000, 0)])
-def test_lanczos_scratch_and_determinism(lm, torch, prec, angular, N, graph):
+@pytest.mark.parametrize("N,graph,small", [(300, 1, 1), (300, 0, 1), (300, 1, 0), (9000, 0, 0)])
+def test_lanczos_scratch_and_determinism(lm, torch, prec, angular, N, graph, small):
     """The Lanczos workspace (basis, w, packed vector, partials, Gram partials) after a NaN run; 6 repeats bit-identical."""
     c = workloads.random_case(N, 2.0 * N ** (1.0 / 3.0), 19, prec, angular, with_noise=True)
     s = lm.Solver(prec, N, 1.0, 1.0, angular)
     tdt = s.torch_dtype
     s.set_option(lm.LM_OPT_GRAPH_REPLAY, graph)
+    s.set_option(lm.LM_OPT_SMALL_KERNEL, small)
     dof = (6 if angular else 3) * N
     gpos, gz = Guarded(torch, 3 * N, tdt, c["pos"]), Guarded(torch, dof, tdt, c["noise"])
     gy, gya = Guarded(torch, 3 * N, tdt), (Guarded(torch, 3 * N, tdt) if angular else None)
