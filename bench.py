@@ -455,6 +455,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the sub-records of the other four configs")
+    ap.add_argument("--small-kernel", type=int, default=1, choices=[0, 1], help="LM_OPT_SMALL_KERNEL: 1 = the one-launch kernel where the library prefers it (default), 0 = never (A/B runs)")
     ap.add_argument("--fig7", action="store_true", help="the paper's Fig. 7 protocol (Mdot time vs N, open and bottom-wall NBody) instead of a config")
     ap.add_argument("--lanczos-rule", default="estimate", choices=["estimate", "step"], help="stopping rule (DESIGN.md reading S3)")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "sharded"],
@@ -498,6 +499,7 @@ def main():
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     arm = Arm(lm, torch, dist, args.config, args.N, rank, world, sharded)
     cfg, N = arm.cfg, arm.N
+    arm.solver.set_option(lm.LM_OPT_SMALL_KERNEL, args.small_kernel)
     if cfg.op == "sqrt+mdot":
         arm.solver.set_option(lm.LM_OPT_LANCZOS_RULE, lm.LM_RULE_STEP if args.lanczos_rule == "step" else lm.LM_RULE_ESTIMATE)
     sampler = ClockSampler(local_rank) if rank == 0 else None
