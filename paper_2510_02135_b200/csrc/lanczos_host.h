@@ -46,7 +46,9 @@ struct LanczosStopper {
     int ldg = 0;                                  // leading dimension of gram: max_iter + 1
     std::vector<double> gram;                     // gram[i * ldg + j] = V_i . V_j, filled one column per new basis vector
     std::vector<double> alphas, betas, c_prev, c_cur, steps, estimates;
+    std::vector<double> dvec, gvec;               // scratch of feed(): d = c_k - [c_{k-1}; 0] and G d
     double pending_beta = 0.0;
+    double den_cur = 0.0;                         // c_cur^T G c_cur = |y_k|^2 / |z|^2 of the newest iterate
 
     void reset(int rule_, double tol_, double breakdown_, int max_iter)
     {
@@ -78,10 +80,25 @@ struct LanczosStopper {
         c_cur.assign((size_t)k, 0.0);
         if (!tridiag_sqrt_e1(k, alphas.data(), betas.data(), c_cur.data())) return EIGENSOLVE_FAILED;
         bool stop = false;
+        if (k == 1) den_cur = quad(c_cur, 1);
         if (k >= 2) {
-            std::vector<double> d(c_cur);
-            for (int i = 0; i < k - 1; ++i) d[i] -= c_prev[i];
-            const double num = std::max(quad(d, k), 0.0), den = std::max(quad(c_prev, k - 1), 0.0);
+            // ONE product g = G d per iteration (the loop at small N waits for this host code): |y_k - y_{k-1}|^2 = d.g, and
+            // |y_k|^2 = |y_{k-1}|^2 + 2 c_{k-1}.g + d.g carries the denominator forward (it only normalises: its
+            // rounding, ~k eps, is immaterial; the numerator is formed directly, without cancellation)
+            dvec.assign(c_cur.begin(), c_cur.end());
+            for (int i = 0; i < k - 1; ++i) dvec[i] -= c_prev[i];
+            gvec.assign((size_t)k, 0.0);
+            for (int i = 0; i < k; ++i) {
+                const double* gi = &gram[(size_t)i * ldg];
+                double acc = 0.0;
+                for (int j = 0; j < k; ++j) acc += gi[j] * dvec[j];
+                gvec[i] = acc;
+            }
+            double dg = 0.0, cg = 0.0;
+            for (int i = 0; i < k; ++i) dg += dvec[i] * gvec[i];
+            for (int i = 0; i < k - 1; ++i) cg += c_prev[i] * gvec[i];
+            const double num = std::max(dg, 0.0), den = std::max(den_cur, 0.0);
+            den_cur = den_cur + 2.0 * cg + dg;
             // a zero previous iterate cannot happen for an SPD matrix (c_1 = sqrt(alpha_1) > 0); keep the ratio finite anyway
             steps.push_back(den > 0.0 ? std::sqrt(num / den) : (num > 0.0 ? HUGE_VAL : 0.0));
             if (rule == RULE_STEP) {

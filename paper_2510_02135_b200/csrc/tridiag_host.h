@@ -24,10 +24,13 @@ inline double pythag(double a, double b) { return std::sqrt(a * a + b * b); }
 inline bool tridiag_sqrt_e1(int n, const double* alpha, const double* beta, double* c_out)
 {
     struct Rot { int i; double c, s; };
-    std::vector<double> d(alpha, alpha + n), e(n, 0.0), row0(n, 0.0);
+    static thread_local std::vector<double> d, e, row0;   // reused across calls: no allocation on the per-iteration path
+    static thread_local std::vector<Rot> rots;
+    d.assign(alpha, alpha + n);
+    e.assign((size_t)n, 0.0);
+    row0.assign((size_t)n, 0.0);
     for (int i = 0; i + 1 < n; ++i) e[i] = beta[i];
     row0[0] = 1.0;
-    static thread_local std::vector<Rot> rots;           // reused across calls: no allocation on the per-iteration path
     rots.clear();
     rots.reserve((size_t)3 * n * n / 2 + 16);
     for (int l = 0; l < n && n > 1; ++l) {
