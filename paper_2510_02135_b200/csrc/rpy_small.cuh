@@ -49,12 +49,6 @@ __device__ __forceinline__ void st_async(uint32_t raddr, double v, uint32_t rbar
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.f64 [%0], %1, [%2];" ::"r"(raddr), "d"(v), "r"(rbar) : "memory");
 }
 
-#ifdef LM_SMALL_TIMING
-#define LM_STAMP(k) do { if (threadIdx.x == 0 && p.stamps) p.stamps[(blockIdx.y * gridDim.x + blockIdx.x) * 8 + (k)] = clock64(); } while (0)
-#else
-#define LM_STAMP(k) do { } while (0)
-#endif
-
 template <typename T> struct SmallParams {
     const T* __restrict__ pos;   // the handle's packed positions x | y | z (| h | b), each npad long
     RhsIn<T> in;                 // caller's arrays, interleaved xyz, 3N each; null = zeros
@@ -67,9 +61,6 @@ template <typename T> struct SmallParams {
     T len_scale;                 // torques are multiplied by the internal length unit
     T ghost_z;                   // height given to sources past N (single wall: a; else 0); their forces are zero
     PairConsts<T> c;
-#ifdef LM_SMALL_TIMING
-    long long* stamps;           // [CTA][8] clock64 at the phase boundaries (probe builds only)
-#endif
 };
 
 // dynamic shared memory: the CTA's sources (positions x | y | z, then each right-hand-side array interleaved), the warps' sums [W][NV][64], and the
@@ -96,7 +87,6 @@ __global__ void __launch_bounds__(SM_MAX_WARPS * 32) rpy_small_kernel(const Smal
     const int S = gridDim.y;                                   // = cluster size: the cluster spans the whole y extent
     const int rank = blockIdx.y;
     const int spw = p.src_per_warp, cta_src = W * spw;
-    LM_STAMP(0);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);     // counts the bytes pushed to this CTA by the cluster
     T* src = reinterpret_cast<T*>(smem_raw + 16);              // x | y | z, each cta_src long, then the right-hand sides
     T* red = src + (size_t)(3 + NV) * cta_src;                 // [W][NV][64]
@@ -171,7 +161,6 @@ __global__ void __launch_bounds__(SM_MAX_WARPS * 32) rpy_small_kernel(const Smal
 #pragma unroll
     for (int k = 0; k < NV; ++k) acc[k] = splat(T(0));
     __syncthreads();
-    LM_STAMP(1);
 
     // ---- the warp's sources, in groups of GS with one far / general vote per group (rpy_pair.cuh)
     const T* sx = src + warp * spw;
@@ -216,7 +205,6 @@ __global__ void __launch_bounds__(SM_MAX_WARPS * 32) rpy_small_kernel(const Smal
     // factored-out prefactor (single wall: times b_i) and writes the caller's array.
     // element e = ((q * PARTS + part) * 64 + t) * 3 + k3: consecutive e are consecutive addresses of one output array
     constexpr int PARTS = ANG ? 2 : 1;
-    LM_STAMP(2);
     T* my = red + (size_t)warp * E;
 #pragma unroll
     for (int k = 0; k < NV; ++k) {
@@ -224,9 +212,7 @@ __global__ void __launch_bounds__(SM_MAX_WARPS * 32) rpy_small_kernel(const Smal
         my[k * SM_TARGETS + 32 + lane] = hi(acc[k]);
     }
     __syncthreads();
-    LM_STAMP(3);
     cluster_wait_acquire();                                    // every CTA of the cluster is running and its mbarrier is initialised
-    LM_STAMP(4);
     const uint32_t recv_s = smem_u32(recv), bar_s = smem_u32(bar);
     for (int e = tid; e < E; e += blockDim.x) {
         const int k3 = e % 3, t = (e / 3) % SM_TARGETS, qp = e / (3 * SM_TARGETS), part = qp % PARTS, q = qp / PARTS;
@@ -240,9 +226,7 @@ __global__ void __launch_bounds__(SM_MAX_WARPS * 32) rpy_small_kernel(const Smal
         const int owner = e / per;
         st_async(map_to_rank(recv_s + (uint32_t)((rank * per + (e - owner * per)) * (int)sizeof(T)), owner), s, map_to_rank(bar_s, owner));
     }
-    LM_STAMP(5);
     if (mine > 0) mbar_wait(bar, 0u);                          // all S x mine values have landed (acquire)
-    LM_STAMP(6);
     for (int el = tid; el < mine; el += blockDim.x) {
         const int e = rank * per + el;
         const int k3 = e % 3, t = (e / 3) % SM_TARGETS, qp = e / (3 * SM_TARGETS), part = qp % PARTS, q = qp / PARTS;
@@ -258,7 +242,6 @@ __global__ void __launch_bounds__(SM_MAX_WARPS * 32) rpy_small_kernel(const Smal
         if constexpr (WALL) fac *= p.pos[4 * p.npad + i];
         (part ? p.out.ang[q] : p.out.lin[q])[3 * i + k3] = s * fac;
     }
-    LM_STAMP(7);
 }
 
 }  // namespace lm
