@@ -21,6 +21,9 @@ cpu_baseline = the CPU fp64 oracle (oracle/, untuned) on the box's host cores, b
 configs = the other four BASELINE.json configs measured in the same run (a few steps each; single GPU, default
           headline only): ms per launch, roofline fraction, e2e -- so that every number of BASELINE.md sec. 4 is on
           the driver's record, not only the headline.
+steady_state = small configs only (1, 2): whole applies back to back on the stream, no L2 flush -- the loop a
+          time-stepping user runs; reported beside the flushed per-step figures, never instead of them.
+--fig7  = the paper's Fig. 7 protocol (Mdot time vs N, open boundaries and bottom wall) as one JSON line, instead of a config.
 
 Multi-GPU (torchrun): "replicas only" by default: every rank runs an independent replica
 (seed + 1000 rank), scaling = "weak"; `--parallelism sharded` row-shards ONE problem over the ranks (lm_dist_init:
