@@ -96,7 +96,7 @@ def test_every_shape_matches_the_oracle(lm, torch, prec, angular, S, W):
 def test_chosen_shape_all_rhs_counts(lm, torch, prec, angular, nrhs, N, side):
     pos, F, T = case(N, side, nrhs, prec, angular, 7 * N + nrhs)
     U, Wv, cfg, st = run(lm, torch, prec, pos, F, T, angular, 1)
-    if N <= 1024:
+    if N <= 256 or (N <= 1024 and nrhs == 1 and not angular):
         assert st["aux_launches"] == 0, "these sizes take the one-launch kernel"
     for q in range(nrhs):
         Uo, Wo = oracle(pos, F[q], None if T is None else T[q], angular)
@@ -114,7 +114,8 @@ def test_single_wall(lm, torch, prec, angular, nrhs, mode):
     F = np.stack([c["forces"]] + [rng.standard_normal(c["forces"].shape).astype(c["forces"].dtype) for _ in range(nrhs - 1)])
     T = None if not angular else np.stack([c["torques"]] + [rng.standard_normal(c["forces"].shape).astype(c["forces"].dtype) for _ in range(nrhs - 1)])
     U, Wv, cfg, st = run(lm, torch, prec, c["pos"], F, T, angular, mode, wall_z=c["wall_z"])
-    assert st["aux_launches"] == 0
+    # a forced shape always runs the one-launch kernel; left to the chooser, the register-heavy fp64 variants hand over early
+    assert (st["aux_launches"] == 0) == (cfg["kernel"] == "rpy_small_kernel") and (mode == 1 or cfg["kernel"] == "rpy_small_kernel")
     for q in range(nrhs):
         Uo, Wo = oracle(c["pos"], F[q], None if T is None else T[q], angular, wall_z=c["wall_z"])
         assert close(U[q], Uo, TOL[prec]), (q, rel(U[q], Uo))
