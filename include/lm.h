@@ -250,11 +250,17 @@ int lm_mdot_rows(lm_solver* h, int64_t row_begin, int64_t row_count, const void*
  *                             number of ranks divides N) all-gathers straight into the caller's output arrays | 0: always
  *                             through the handle's own all-gather buffers and a device-to-device copy (the path taken
  *                             anyway when the last block is short).
+ *   LM_OPT_ACCUMULATE_F64     0 (default) | 1, fp32 handles only: mixed precision -- fp32 pair arithmetic, but the packed fp32
+ *                             accumulators are flushed every 32 sources into fp64 totals, the j-split partial sums are
+ *                             kept and added in fp64, and each result is rounded to fp32 once.  The error of an fp32
+ *                             apply is dominated by the length of its fp32 summation runs: measured on config 3
+ *                             (N = 131072) rel-L2 6.1e-7 -> 1.4e-7, the floor set by the fp32 pair arithmetic being 0.8e-7,
+ *                             for a few per cent of time.  Always the general path (no one-launch kernel).
  * lm_lanczos_history: what the last Lanczos call measured for noise vector `vec` of its (last) group: for iteration
  *   i + 1 (i < cap): alpha[i], beta[i], step[i] = s_{i+1} (NaN for i = 0), estimate[i] = e_{i+1} (NaN for i < 2; NaN
  *   throughout under LM_RULE_STEP).  Any output may be NULL.  Returns the number of iterations recorded. */
 enum { LM_RULE_ESTIMATE = 0, LM_RULE_STEP = 1 };
-enum { LM_OPT_LANCZOS_RULE = 0, LM_OPT_GRAPH_REPLAY = 1, LM_OPT_SHARE_FIRST_APPLY = 2, LM_OPT_SMALL_KERNEL = 3, LM_OPT_J_SPLITS = 4, LM_OPT_GATHER_IN_PLACE = 5 };
+enum { LM_OPT_LANCZOS_RULE = 0, LM_OPT_GRAPH_REPLAY = 1, LM_OPT_SHARE_FIRST_APPLY = 2, LM_OPT_SMALL_KERNEL = 3, LM_OPT_J_SPLITS = 4, LM_OPT_GATHER_IN_PLACE = 5, LM_OPT_ACCUMULATE_F64 = 6 };
 int lm_set_option(lm_solver* h, int option, int value);
 int lm_set_max_iter(lm_solver* h, int max_iter);     /* default 100; 1 <= max_iter <= 1000 */
 int lm_last_iterations(const lm_solver* h);           /* iterations of the last Lanczos call (or < 0) */

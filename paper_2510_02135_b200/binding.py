@@ -19,7 +19,7 @@ import numpy as np
 LM_F32, LM_F64 = 0, 1
 LM_OK, LM_E_INVALID, LM_E_NOPOS, LM_E_ANGULAR, LM_E_NULL, LM_E_CUDA, LM_E_NOCONV = 0, -1, -2, -3, -4, -5, -6
 LM_RULE_ESTIMATE, LM_RULE_STEP = 0, 1
-LM_OPT_LANCZOS_RULE, LM_OPT_GRAPH_REPLAY, LM_OPT_SHARE_FIRST_APPLY, LM_OPT_SMALL_KERNEL, LM_OPT_J_SPLITS, LM_OPT_GATHER_IN_PLACE = 0, 1, 2, 3, 4, 5
+LM_OPT_LANCZOS_RULE, LM_OPT_GRAPH_REPLAY, LM_OPT_SHARE_FIRST_APPLY, LM_OPT_SMALL_KERNEL, LM_OPT_J_SPLITS, LM_OPT_GATHER_IN_PLACE, LM_OPT_ACCUMULATE_F64 = 0, 1, 2, 3, 4, 5, 6
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liblm.so")

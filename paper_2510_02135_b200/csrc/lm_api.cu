@@ -180,6 +180,12 @@ int lm_set_option(lm_solver* h, int option, int value)
         return LM_OK;
     case LM_OPT_GRAPH_REPLAY: h->graph_replay = value != 0; return LM_OK;
     case LM_OPT_SHARE_FIRST_APPLY: h->share_first_apply = value != 0; return LM_OK;
+    case LM_OPT_ACCUMULATE_F64:
+        if (h->precision != LM_F32 && value != 0) return fail(h, LM_E_INVALID, "LM_OPT_ACCUMULATE_F64 is for fp32 handles (an fp64 handle accumulates in fp64 anyway)");
+        h->acc64 = value != 0;
+        for (auto& slot : h->plan_cache) slot.valid = false;
+        for (auto& slot : h->small_cache) slot.valid = false;
+        return LM_OK;
     case LM_OPT_GATHER_IN_PLACE: h->gather_in_caller = value != 0; return LM_OK;
     case LM_OPT_J_SPLITS:
         if (value < 0) return fail(h, LM_E_INVALID, "LM_OPT_J_SPLITS: 0 (chosen by the library) or the number of j-splits");

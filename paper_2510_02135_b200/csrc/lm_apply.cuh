@@ -14,7 +14,7 @@ template <typename T> int prepare_apply(lm_solver* h, int nrhs, LaunchPlan& plan
     int rc = ensure(h, &h->vec_soa, &h->vec_soa_bytes, (size_t)nrhs * nc * h->npad * sizeof(T));
     if (rc != LM_OK) return rc;
     if (plan.j_splits > 1) {
-        rc = ensure(h, &h->partial, &h->partial_bytes, (size_t)plan.j_splits * nrhs * nc * h->npad * sizeof(T));
+        rc = ensure(h, &h->partial, &h->partial_bytes, (size_t)plan.j_splits * nrhs * nc * h->npad * (h->acc64 ? sizeof(double) : sizeof(T)));
         if (rc != LM_OK) return rc;
     }
     return LM_OK;
@@ -73,9 +73,15 @@ int launch_pair(lm_solver* h, int nrhs, const LaunchPlan& plan, const RhsOut<T>&
         h->pending.emplace_back(e0, e1);
     }
     // split-j reduce of the right-hand sides [reduce_from, nrhs); the caller's next kernel sums the partials of the others itself
-    if (plan.i_tiles > 0 && plan.j_splits > 1 && reduce_from < nrhs)
-        reduce_partials_kernel<T><<<dim3(grid_1d(h->row_end - h->row_begin), (nrhs - reduce_from) * nc), VEC_BLOCK, 0, st>>>(
-            (const T*)h->partial, plan.j_splits, nrhs, nc, reduce_from, h->row_begin, h->row_end, h->npad, kout);
+    if (plan.i_tiles > 0 && plan.j_splits > 1 && reduce_from < nrhs) {
+        const dim3 grid(grid_1d(h->row_end - h->row_begin), (nrhs - reduce_from) * nc);
+        if (h->acc64)
+            reduce_partials_kernel<T, double><<<grid, VEC_BLOCK, 0, st>>>((const double*)h->partial, plan.j_splits, nrhs, nc, reduce_from, h->row_begin,
+                                                                          h->row_end, h->npad, kout);
+        else
+            reduce_partials_kernel<T><<<grid, VEC_BLOCK, 0, st>>>((const T*)h->partial, plan.j_splits, nrhs, nc, reduce_from, h->row_begin, h->row_end,
+                                                                  h->npad, kout);
+    }
     LM_CUDA(h, cudaGetLastError());
     if (dist) {
         NcclApi& nccl = nccl_api();
@@ -226,7 +232,7 @@ int apply_batch(lm_solver* h, int nrhs, const T* forces, const T* torques, T* li
     int q = 0;
     while (q < nrhs) {
         int chunk = nrhs - q >= 4 ? 4 : (nrhs - q >= 2 ? 2 : 1);
-        if (h->angular && chunk > 2) chunk = 2;     // angular variants exist for 1 and 2 right-hand sides
+        if ((h->angular || h->wall) && chunk > 2) chunk = 2;     // angular and single-wall variants exist for 1 and 2 right-hand sides
         RhsIn<T> in{};
         RhsOut<T> out{};
         for (int r = 0; r < chunk; ++r) {

@@ -20,19 +20,20 @@ template <typename T> struct Variant {
     int ctas_per_sm;      // filled at first use (occupancy API)
     double efficiency;    // relative per-pair throughput used by the launch chooser
     int wall;             // 1: the single-wall variant (free-space pair + wall correction)
+    int acc64;            // 1: fp32 pair math with fp64 accumulation (LM_OPT_ACCUMULATE_F64)
 };
 
-template <typename T, int NRHS, bool ANG, int TPT, int SUB, int MINB, bool WALL = false> Variant<T> make_large()
+template <typename T, int NRHS, bool ANG, int TPT, int SUB, int MINB, bool WALL = false, bool ACC64 = false> Variant<T> make_large()
 {
-    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB>;
+    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB, ACC64>;
     static_assert(NPAD_QUANTUM % SUB == 0, "every SUB divides NPAD_QUANTUM");
-    return {rpy_pair_kernel<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB, MINB, WALL>, NRHS, ANG, L_BLOCK, TPT, L_TJ, SUB, Tr::SMEM_BYTES, 0, 1.0, WALL};
+    return {rpy_pair_kernel<T, NRHS, ANG, TPT, L_BLOCK, L_TJ, L_STAGES, SUB, MINB, WALL, ACC64>, NRHS, ANG, L_BLOCK, TPT, L_TJ, SUB, Tr::SMEM_BYTES, 0, 1.0, WALL, ACC64};
 }
 template <typename T, int NRHS, bool ANG, int SUB, int MINB, bool WALL = false> Variant<T> make_small()
 {
     using Tr = PairKernelTraits<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB>;
     static_assert(NPAD_QUANTUM % SUB == 0, "every SUB divides NPAD_QUANTUM");
-    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB, MINB, WALL>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, SUB, Tr::SMEM_BYTES, 0, 0.8, WALL};
+    return {rpy_pair_kernel<T, NRHS, ANG, S_TPT, S_BLOCK, S_TJ, S_STAGES, SUB, MINB, WALL>, NRHS, ANG, S_BLOCK, S_TPT, S_TJ, SUB, Tr::SMEM_BYTES, 0, 0.8, WALL, 0};
 }
 
 template <typename T> std::vector<Variant<T>> build_variants();
@@ -46,7 +47,12 @@ template <> std::vector<Variant<float>> build_variants<float>()
             make_large<float, 1, false, 2, 32, 2, true>(), make_large<float, 2, false, 2, 32, 1, true>(),
             make_large<float, 1, true, 2, 32, 1, true>(),  make_large<float, 2, true, 2, 32, 1, true>(),
             make_small<float, 1, false, 32, 6, true>(), make_small<float, 2, false, 32, 6, true>(),
-            make_small<float, 1, true, 32, 4, true>(),  make_small<float, 2, true, 32, 4, true>()};
+            make_small<float, 1, true, 32, 4, true>(),  make_small<float, 2, true, 32, 4, true>(),
+            // fp32 pair math, fp64 accumulation (LARGE shape only: the option is for large sums; any N is still served)
+            make_large<float, 1, false, 4, 32, 2, false, true>(), make_large<float, 2, false, 4, 32, 1, false, true>(), make_large<float, 4, false, 4, 32, 1, false, true>(),
+            make_large<float, 1, true, 2, 32, 2, false, true>(),  make_large<float, 2, true, 2, 32, 1, false, true>(),
+            make_large<float, 1, false, 2, 32, 2, true, true>(), make_large<float, 2, false, 2, 32, 1, true, true>(),
+            make_large<float, 1, true, 2, 32, 1, true, true>(),  make_large<float, 2, true, 2, 32, 1, true, true>()};
 }
 template <> std::vector<Variant<double>> build_variants<double>()
 {
@@ -209,6 +215,7 @@ struct lm_solver {
     // one-launch small-N kernel (LM_OPT_SMALL_KERNEL): 1 = where the launch chooser prefers it, 0 = never,
     // (cluster << 8 | warps) = always, with that shape (plan sweeps)
     int small_kernel = 1;
+    bool acc64 = false;             // LM_OPT_ACCUMULATE_F64 (fp32 handles): fp64 accumulation of the fp32 pair terms
     bool gather_in_caller = true;   // LM_OPT_GATHER_IN_PLACE: row-sharded applies all-gather straight into the caller's arrays when the blocks tile [0, N)
     int force_splits = 0;      // LM_OPT_J_SPLITS: > 0 fixes the number of j-splits of the general path (plan sweeps)
     struct SmallSlot { bool valid = false; int64_t rb = 0, re = 0; int mode = 0; lm::SmallPlan plan; } small_cache[lm::MAX_RHS + 1];
@@ -341,7 +348,7 @@ inline double cycles_per_source(const lm_solver* h, int nrhs)
 template <typename T> SmallPlan choose_small(lm_solver* h, int nrhs)
 {
     SmallPlan best;
-    if (nrhs < 1 || nrhs > MAX_RHS || h->small_kernel == 0 || h->dist_ranks > 0) return best;
+    if (nrhs < 1 || nrhs > MAX_RHS || h->small_kernel == 0 || h->dist_ranks > 0 || h->acc64) return best;
     auto& slot = h->small_cache[nrhs];
     if (slot.valid && slot.rb == h->row_begin && slot.re == h->row_end && slot.mode == h->small_kernel) return slot.plan;
     const auto& vs = small_variants<T>(h);
@@ -406,7 +413,7 @@ template <typename T> LaunchPlan choose_plan(lm_solver* h, int nrhs)
     double best_cost = 1e300;
     for (int vi = 0; vi < (int)vs.size(); ++vi) {
         const auto& v = vs[vi];
-        if (v.nrhs != nrhs || v.ang != h->angular || v.wall != h->wall) continue;
+        if (v.nrhs != nrhs || v.ang != h->angular || v.wall != h->wall || v.acc64 != (h->acc64 ? 1 : 0)) continue;
         const int targets = v.block * v.tpt;
         const int64_t rows = std::max<int64_t>(h->row_end - h->row_begin, 0);          // target rows of this rank / call
         const int i_tiles = (int)((rows + targets - 1) / targets);

@@ -149,7 +149,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     }
     // the alpha kernel doubles as the split-j reduce of the apply (one launch less per vector and iteration),
     // except for row-sharded runs, where w must be all-gathered before any rank can use it
-    auto fused = [&](const LaunchPlan& pl) { return pl.j_splits > 1 && pl.i_tiles > 0 && h->dist_ranks == 0; };
+    auto fused = [&](const LaunchPlan& pl) { return pl.j_splits > 1 && pl.i_tiles > 0 && h->dist_ranks == 0 && !h->acc64; };
     auto body_small = [&](cudaStream_t s2, bool timed) -> int {
         RhsIn<T> in{};
         for (int q = 0; q < nv; ++q) {

@@ -390,7 +390,13 @@ template <> struct Vec16<double> { static constexpr int N = 2; using type = doub
 __device__ __forceinline__ float vget(const float4& v, int k) { return k == 0 ? v.x : (k == 1 ? v.y : (k == 2 ? v.z : v.w)); }
 __device__ __forceinline__ double vget(const double2& v, int k) { return k == 0 ? v.x : v.y; }
 
-template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES, int SUB>
+// ACC64 (fp32 kernels only; SURVEY.md sec. 8(f) NEXT-4 "mixed precision: fp32 pair math, fp64 accumulation"): the packed fp32
+// accumulators are flushed every ACC64_RUN sources into per-thread fp64 totals kept in shared memory, the j-split
+// partials are written in fp64 and the result is rounded to fp32 once.  The fp32 error of a sum is dominated by the
+// LENGTH of the fp32 runs: runs of 32 instead of 512 + 7 + 37 take config 3 from 6.0e-7 to 1.4e-7.
+constexpr int ACC64_RUN = 32;
+
+template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES, int SUB, bool ACC64 = false>
 struct PairKernelTraits {
     static_assert(TPT % 2 == 0, "targets are held as packed pairs");
     static_assert(TJ % SUB == 0 && SUB % Vec16<T>::N == 0, "source units");
@@ -401,14 +407,17 @@ struct PairKernelTraits {
     static constexpr int NP = TPT / 2;                 // packed target pairs per thread
     static constexpr int ARRAYS = 3 + NV;              // x, y, z + vector components
     static constexpr int STAGE_BYTES = ARRAYS * TJ * (int)sizeof(T);
-    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + STAGES * 8 + STAGES * 8;   // tiles | full mbarriers | empty mbarriers
+    static constexpr int BAR_BYTES = STAGES * 8 + STAGES * 8;                           // full mbarriers | empty mbarriers
+    static constexpr int TOT64_BYTES = ACC64 ? TPT * NV * BLOCK * 8 : 0;               // fp64 totals [TPT * NV][BLOCK]
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + TOT64_BYTES;
     static constexpr int TARGETS = BLOCK * TPT;        // targets per CTA
+    static_assert(!ACC64 || (std::is_same<T, float>::value && SUB % ACC64_RUN == 0 && ACC64_RUN % Vec16<T>::N == 0), "ACC64: fp32 kernels, runs aligned with the source units");
 };
 
-template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES, int SUB, int MINB, bool WALL = false>
+template <typename T, int NRHS, bool ANG, int TPT, int BLOCK, int TJ, int STAGES, int SUB, int MINB, bool WALL = false, bool ACC64 = false>
 __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<T> p)
 {
-    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, BLOCK, TJ, STAGES, SUB>;
+    using Tr = PairKernelTraits<T, NRHS, ANG, TPT, BLOCK, TJ, STAGES, SUB, ACC64>;
     constexpr int NC = Tr::NC, NV = Tr::NV, NP = Tr::NP, ARRAYS = Tr::ARRAYS;
     constexpr int VN = Vec16<T>::N, GS = Tr::GS;
     constexpr bool EARLY = ANG || NRHS >= 4;
@@ -417,6 +426,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
     T* tiles = reinterpret_cast<T*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + STAGES * Tr::STAGE_BYTES);
     uint64_t* empty = full + STAGES;                  // per stage: the BLOCK / 32 warps that have finished with it
+    double* tot64 = reinterpret_cast<double*>(smem_raw + STAGES * Tr::STAGE_BYTES + Tr::BAR_BYTES);   // ACC64: [TPT * NV][BLOCK], thread-private columns
     constexpr unsigned int NWARPS = BLOCK / 32;
 
     const int tid = threadIdx.x;
@@ -475,6 +485,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
     for (int q = 0; q < NP; ++q)
 #pragma unroll
         for (int k = 0; k < NV; ++k) total[q][k] = splat(T(0));
+    if constexpr (ACC64) {
+#pragma unroll
+        for (int s = 0; s < TPT * NV; ++s) tot64[s * BLOCK + tid] = 0.0;
+    }
 
     using Near = typename NearOf<T>::type;
 
@@ -493,8 +507,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
 
         // sources are walked in groups of GS; the geometry of the whole group (GS x NP packed pairs)
         // comes first, one warp vote on its minimum r^2 picks the far-field or the general body
-#pragma unroll 1
-        for (int j = 0; j < tile_count; j += VN) {
+        auto walk = [&](int j) {                      // VN sources of the tile, from source j on
             const V16 X = *reinterpret_cast<const V16*>(sx + j);
             const V16 Y = *reinterpret_cast<const V16*>(sx + TJ + j);
             const V16 Z = *reinterpret_cast<const V16*>(sx + 2 * TJ + j);
@@ -529,12 +542,33 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
                 if (!hit) body(std::true_type{});
                 else body(std::false_type{});
             }
+        };
+        if constexpr (!ACC64) {
+#pragma unroll 1
+            for (int j = 0; j < tile_count; j += VN) walk(j);
+            // flush the per-tile packed accumulators
+#pragma unroll
+            for (int q = 0; q < NP; ++q)
+#pragma unroll
+                for (int k = 0; k < NV; ++k) total[q][k] = add2(total[q][k], acc[q][k]);
+        } else {
+            // fp32 runs of ACC64_RUN sources, each flushed into this thread's fp64 totals (tile_count is a multiple of SUB)
+#pragma unroll 1
+            for (int j0 = 0; j0 < tile_count; j0 += ACC64_RUN) {
+#pragma unroll 1
+                for (int j = j0; j < j0 + ACC64_RUN; j += VN) walk(j);
+#pragma unroll
+                for (int q = 0; q < NP; ++q)
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) {
+                        double* t0 = tot64 + ((2 * q) * NV + k) * BLOCK + tid;
+                        double* t1 = tot64 + ((2 * q + 1) * NV + k) * BLOCK + tid;
+                        *t0 += (double)lo(acc[q][k]);
+                        *t1 += (double)hi(acc[q][k]);
+                        acc[q][k] = splat(T(0));
+                    }
+            }
         }
-        // flush the per-tile packed accumulators
-#pragma unroll
-        for (int q = 0; q < NP; ++q)
-#pragma unroll
-            for (int k = 0; k < NV; ++k) total[q][k] = add2(total[q][k], acc[q][k]);
 
         // release the stage without a CTA-wide barrier: every warp arrives on the stage's `empty` mbarrier, the LAST
         // one to leave refills the stage (TMA) -- no warp ever waits for another except on the data it needs
@@ -546,6 +580,41 @@ __global__ void __launch_bounds__(BLOCK, MINB) rpy_pair_kernel(const PairParams<
     }
 
     // ---- epilogue: apply the factored-out Oseen prefactor once per target (single wall: times the damping factor b_i)
+    if constexpr (ACC64) {
+        // fp64 totals -> caller's arrays (rounded once) or fp64 j-split partials [split][NV][npad]
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                const int64_t i = i0 + (2 * q + half) * BLOCK + tid;
+                double fl = (double)p.c.C1_lin, fa = (double)p.c.C1_ang;
+                if constexpr (WALL) {
+                    const double b = (double)p.damp[min(i, p.npad - 1)];
+                    fl *= b;
+                    fa *= b;
+                }
+                const double* mine = tot64 + ((2 * q + half) * NV) * BLOCK + tid;
+                if (gridDim.y == 1) {
+                    if (i < p.i_end) {
+#pragma unroll
+                        for (int r = 0; r < NRHS; ++r) {
+#pragma unroll
+                            for (int k = 0; k < 3; ++k) p.out.lin[r][3 * i + k] = (T)(mine[(r * NC + k) * BLOCK] * fl);
+                            if constexpr (ANG) {
+#pragma unroll
+                                for (int k = 0; k < 3; ++k) p.out.ang[r][3 * i + k] = (T)(mine[(r * NC + 3 + k) * BLOCK] * fa);
+                            }
+                        }
+                    }
+                } else if (i < p.npad) {
+                    double* part = reinterpret_cast<double*>(p.partial) + (size_t)blockIdx.y * NV * p.npad;
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) part[(size_t)k * p.npad + i] = mine[k * BLOCK] * ((k % NC) < 3 ? fl : fa);
+                }
+            }
+        }
+        return;
+    }
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
         P2<T> fl = splat(p.c.C1_lin), fa = splat(p.c.C1_ang);

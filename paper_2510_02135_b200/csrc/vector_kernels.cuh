@@ -72,27 +72,29 @@ __global__ void __launch_bounds__(VEC_BLOCK) pack_rhs_kernel(RhsIn<T> in, int nr
 // sides [q_begin, nrhs) (the Lanczos driver reduces its own vectors inside its alpha kernel).
 // One thread per (right-hand side, component, particle): consecutive threads read consecutive
 // addresses of one partial array; the loads of the splits are independent and unrolled.
-template <typename T>
-__global__ void __launch_bounds__(VEC_BLOCK) reduce_partials_kernel(const T* __restrict__ partial, int splits, int nrhs, int nc, int q_begin,
+// TP = type of the partials: T, or double when the pair kernel accumulates in fp64 (LM_OPT_ACCUMULATE_F64): summed in TP,
+// rounded to T once.
+template <typename T, typename TP = T>
+__global__ void __launch_bounds__(VEC_BLOCK) reduce_partials_kernel(const TP* __restrict__ partial, int splits, int nrhs, int nc, int q_begin,
                                                                     int64_t i_begin, int64_t i_end, int64_t npad, RhsOut<T> out)
 {
     const int64_t i = i_begin + (int64_t)blockIdx.x * VEC_BLOCK + threadIdx.x;   // target rows [i_begin, i_end)
     if (i >= i_end) return;
     const int qk = q_begin * nc + blockIdx.y, q = qk / nc, k = qk % nc;          // right-hand sides [q_begin, nrhs): gridDim.y = (nrhs - q_begin) nc
     const size_t stride = (size_t)nrhs * nc * npad;
-    const T* p = partial + (size_t)qk * npad + i;
-    T s = T(0);
+    const TP* p = partial + (size_t)qk * npad + i;
+    TP s = TP(0);
     int sidx = 0;
     for (; sidx + 8 <= splits; sidx += 8) {
-        T v[8];
+        TP v[8];
 #pragma unroll
         for (int u = 0; u < 8; ++u) v[u] = p[(size_t)(sidx + u) * stride];
 #pragma unroll
         for (int u = 0; u < 8; ++u) s += v[u];
     }
     for (; sidx < splits; ++sidx) s += p[(size_t)sidx * stride];
-    if (k < 3) out.lin[q][3 * i + k] = s;
-    else       out.ang[q][3 * i + (k - 3)] = s;
+    if (k < 3) out.lin[q][3 * i + k] = (T)s;
+    else       out.ang[q][3 * i + (k - 3)] = (T)s;
 }
 
 // eq. (11) PAPER.md:151-155 (random finite difference): packed positions displaced along W,

@@ -56,8 +56,7 @@ SHAPES = {"cluster": (333, 1, "rpy_small_kernel", None), "small": (333, 0, "rpy_
 @pytest.mark.parametrize("with_wall", [False, True])
 @pytest.mark.parametrize("shape", ["cluster", "small", "large"])
 def test_pair_kernel_variant(lm, torch, prec, angular, nrhs, with_wall, shape):
-    if with_wall and nrhs == 4:
-        pytest.skip("single-wall variants exist for 1 and 2 right-hand sides (lm_mdot_batch chunks 4 into 2 + 2)")
+    # (single-wall variants exist for 1 and 2 right-hand sides: lm_mdot_batch serves 4 as 2 + 2)
     N, mode, kernel, block = SHAPES[shape]
     side = 1.6 * N ** (1.0 / 3.0)                              # ~10 % volume fraction: overlapping and far pairs
     if with_wall:
@@ -73,7 +72,7 @@ def test_pair_kernel_variant(lm, torch, prec, angular, nrhs, with_wall, shape):
         s.set_wall(True, c["wall_z"])
     s.set_option(lm.LM_OPT_SMALL_KERNEL, mode)
     s.set_positions(dev(torch, c["pos"]))
-    cfg = s.pair_launch_config(nrhs)
+    cfg = s.pair_launch_config(2 if (with_wall and nrhs == 4) else nrhs)
     assert cfg["kernel"] == kernel and (block is None or cfg["block"] == block), cfg
     if shape == "large":
         assert cfg["j_splits"] > 1                              # partial sums + reduce kernel on this path

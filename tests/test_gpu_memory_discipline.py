@@ -66,8 +66,6 @@ SHAPES = {"cluster": (333, 1), "small": (333, 0), "large": (9000, 0)}
 @pytest.mark.parametrize("with_wall", [False, True])
 @pytest.mark.parametrize("shape", ["cluster", "small", "large"])
 def test_apply_touches_only_its_buffers_and_is_deterministic(lm, torch, prec, angular, nrhs, with_wall, shape):
-    if with_wall and nrhs == 4:
-        pytest.skip("single-wall variants exist for 1 and 2 right-hand sides")
     N, mode = SHAPES[shape]
     side = 1.6 * N ** (1.0 / 3.0)
     if with_wall:

@@ -108,7 +108,7 @@ def test_wall_any_unit_system(lm, torch, prec, a, eta):
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("angular", [False, True])
-@pytest.mark.parametrize("nrhs", [2, 3])
+@pytest.mark.parametrize("nrhs", [2, 3, 4, 5])
 def test_wall_mdot_batch(lm, torch, prec, angular, nrhs):
     N = 1300
     dt = workloads.np_dtype(prec)
