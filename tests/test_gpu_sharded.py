@@ -77,13 +77,15 @@ def test_nccl_world_of_one_equals_the_undistributed_handle(lm, torch):
     port = 33500 + os.getpid() % 2000
     dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1, device_id=torch.device("cuda", 0))
     try:
-        for prec, angular, in_place in (("f32", False, 1), ("f64", True, 1), ("f32", True, 0), ("f64", False, 0)):
+        for prec, angular, in_place, acc64 in (("f32", False, 1, 0), ("f64", True, 1, 0), ("f32", True, 0, 0), ("f64", False, 0, 0), ("f32", False, 1, 1)):
             N = 3000
             c = workloads.random_case(N, 30.0, 62, prec, angular, with_noise=True)
             ref, sh = lm.Solver(prec, N, 1.0, 1.0, angular), lm.Solver(prec, N, 1.0, 1.0, angular)
             # a sharded handle always takes the general path (its outputs go through the all-gather buffers); the
             # reference is held to the same kernels so that the comparison can be bit for bit
             ref.set_option(lm.LM_OPT_SMALL_KERNEL, 0)
+            for s_ in (ref, sh):
+                s_.set_option(lm.LM_OPT_ACCUMULATE_F64, acc64)           # mixed precision: fp64 partials through the same all-gather path
             sh.set_option(lm.LM_OPT_GATHER_IN_PLACE, in_place)   # all-gather into the caller's arrays / through the handle's buffers
             assert multi.init_sharded(sh) == (0, N)
             with pytest.raises(lm.LmError):
