@@ -4,8 +4,8 @@
 // The general path (pack_rhs -> rpy_pair_kernel -> reduce_partials) needs three launches and a round trip of the j-split
 // partial sums through global memory; below a few thousand particles those launches ARE the cost.  Here one kernel does
 // all of it:
-//   * it reads the caller's interleaved force / torque arrays directly and de-interleaves them into shared memory
-//     (the whole source range of a CTA fits many times over), so there is no packing launch;
+//   * it reads the caller's interleaved force / torque arrays directly into shared memory, kept interleaved (the whole
+//     source range of a CTA fits many times over), so there is no packing launch;
 //   * a CTA owns 64 targets (one packed target pair per lane, as in rpy_pair_kernel) and its WARPS split the CTA's
 //     sources, so even N = 1024 spreads over every SM sub-partition;
 //   * the sources are further split over the CTAs of a THREAD-BLOCK CLUSTER (cluster dims (1, S, 1)); every CTA adds
@@ -14,13 +14,9 @@
 //     in rank order (deterministic) -- no global partials, no reduce launch, no fence, no remote load;
 //   * the pair arithmetic is rpy_pair.cuh's (pair_geom / pair_apply / wall_apply, far / general vote per source group).
 #pragma once
-#include <cooperative_groups.h>
-
 #include "rpy_pair.cuh"
 
 namespace lm {
-
-namespace cg = cooperative_groups;
 
 constexpr int SM_TARGETS = 64;        // targets per CTA: 32 lanes x one packed pair
 constexpr int SM_MAX_WARPS = 8;
