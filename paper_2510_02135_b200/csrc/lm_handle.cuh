@@ -215,6 +215,7 @@ struct lm_solver {
     // one-launch small-N kernel (LM_OPT_SMALL_KERNEL): 1 = where the launch chooser prefers it, 0 = never,
     // (cluster << 8 | warps) = always, with that shape (plan sweeps)
     int small_kernel = 1;
+    int max_cluster = 1;       // largest cluster size (<= 8) the device can co-schedule for the one-launch kernel (occupancy API, at lm_create)
     bool acc64 = false;             // LM_OPT_ACCUMULATE_F64 (fp32 handles): fp64 accumulation of the fp32 pair terms
     bool gather_in_caller = true;   // LM_OPT_GATHER_IN_PLACE: row-sharded applies all-gather straight into the caller's arrays when the blocks tile [0, N)
     int force_splits = 0;      // LM_OPT_J_SPLITS: > 0 fixes the number of j-splits of the general path (plan sweeps)
@@ -327,6 +328,25 @@ template <typename T> int init_variants(lm_solver* h)
     auto& ss = small_variants<T>(h);
     ss = build_small_variants<T>();
     for (auto& v : ss) LM_CUDA(h, cudaFuncSetAttribute((const void*)v.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMALL_MAX_SMEM));
+    // Can the device co-schedule clusters of this size at all (a MIG slice or a reduced-SM part may not)?  Ask once,
+    // for the heaviest shape the chooser may pick; the chooser never exceeds the answer (1 = no clusters: still one launch).
+    h->max_cluster = 1;
+    for (int S = SM_MAX_CLUSTER; S > 1; S /= 2) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(1, S, 1);
+        cfg.blockDim = dim3(SM_MAX_WARPS * 32, 1, 1);
+        cfg.dynamicSmemBytes = SMALL_MAX_SMEM / 2;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 1;
+        attr[0].val.clusterDim.y = S;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, (const void*)ss[0].kernel, &cfg) == cudaSuccess && n > 0) { h->max_cluster = S; break; }
+        (void)cudaGetLastError();
+    }
     return LM_OK;
 }
 
@@ -368,9 +388,9 @@ template <typename T> SmallPlan choose_small(lm_solver* h, int nrhs)
     if (vi >= 0 && rows > 0 && in_range) {
         const int i_tiles = (int)((rows + SM_TARGETS - 1) / SM_TARGETS);
         double best_cost = 1e300;
-        for (int S = 1; S <= SM_MAX_CLUSTER; S *= 2)
+        for (int S = 1; S <= h->max_cluster; S *= 2)
             for (int W = 1; W <= SM_MAX_WARPS; W *= 2) {
-                if (forced && (S != (h->small_kernel >> 8) || W != (h->small_kernel & 255))) continue;
+                if (forced && (S != std::min(h->small_kernel >> 8, h->max_cluster) || W != (h->small_kernel & 255))) continue;
                 const int spw = (int)(((h->N + (int64_t)S * W - 1) / ((int64_t)S * W) + 3) / 4 * 4);
                 const size_t smem = vs[vi].smem(W, spw);
                 if (smem > SMALL_MAX_SMEM) continue;
