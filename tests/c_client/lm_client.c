@@ -19,8 +19,49 @@
 
 static int close_to(double got, double want, double tol) { return fabs(got - want) <= tol * fmax(fabs(want), 1e-300); }
 
-int main(void)
+/* --time: microseconds per lm_mdot called back to back from C (no Python marshalling), fp32 and fp64, a few sizes */
+static int time_applies(void)
 {
+    const int sizes[] = {64, 256, 1024, 2048, 4096};
+    for (int prec = 0; prec < 2; ++prec)
+        for (unsigned si = 0; si < sizeof sizes / sizeof sizes[0]; ++si) {
+            const int N = sizes[si];
+            const size_t es = prec ? 8 : 4, bytes = (size_t)3 * N * es;
+            void *pos = malloc(bytes), *d_pos, *d_f, *d_u;
+            const double side = cbrt(N * 4.0 * PI / 3.0 / 0.05);
+            srand(7);
+            for (int i = 0; i < 3 * N; ++i) {
+                const double v = side * rand() / (double)RAND_MAX;
+                if (prec) ((double*)pos)[i] = v; else ((float*)pos)[i] = (float)v;
+            }
+            cudaMalloc(&d_pos, bytes); cudaMalloc(&d_f, bytes); cudaMalloc(&d_u, bytes);
+            cudaMemcpy(d_pos, pos, bytes, cudaMemcpyHostToDevice);
+            cudaMemcpy(d_f, pos, bytes, cudaMemcpyHostToDevice);          /* any finite values serve as forces */
+            lm_solver* s = NULL;
+            CHECK(lm_create(&s, prec ? LM_F64 : LM_F32, N, 1.0, 1.0, 0) == LM_OK, "lm_create");
+            CHECK(lm_set_positions(s, d_pos, NULL) == LM_OK, "%s", lm_last_error(s));
+            cudaEvent_t e0, e1;
+            cudaEventCreate(&e0); cudaEventCreate(&e1);
+            float best = 1e30f;
+            for (int rep = 0; rep < 4; ++rep) {
+                const int n = 500;
+                cudaEventRecord(e0, 0);
+                for (int i = 0; i < n; ++i) CHECK(lm_mdot(s, d_f, NULL, d_u, NULL, NULL) == LM_OK, "%s", lm_last_error(s));
+                cudaEventRecord(e1, 0);
+                cudaEventSynchronize(e1);
+                float ms; cudaEventElapsedTime(&ms, e0, e1);
+                if (rep && ms / n < best) best = ms / n;
+            }
+            printf("{\"precision\": \"%s\", \"N\": %d, \"us_per_mdot_from_c\": %.3f, \"kernel\": \"%s\"}\n", prec ? "f64" : "f32", N, best * 1e3, lm_pair_kernel_name(s, 1));
+            lm_destroy(s);
+            cudaFree(d_pos); cudaFree(d_f); cudaFree(d_u); free(pos);
+        }
+    return 0;
+}
+
+int main(int argc, char** argv)
+{
+    if (argc > 1 && strcmp(argv[1], "--time") == 0) return time_applies();
     const double eta = 1.3, a = 0.7;
     const double mu_t = 1.0 / (6.0 * PI * eta * a), mu_r = 1.0 / (8.0 * PI * eta * a * a * a);
     double *d_pos, *d_f, *d_t, *d_u, *d_w;
