@@ -242,7 +242,9 @@ int lm_mdot_rows(lm_solver* h, int64_t row_begin, int64_t row_count, const void*
  *                             distributed shared memory) where the launch chooser prefers it | 0: never (always pack,
  *                             pair kernel, reduce) | (cluster << 8 | warps), cluster and warps in {1, 2, 4, 8}: always,
  *                             with that shape (plan sweeps).  Same results up to summation order (PAPER.md:435-437:
- *                             the small-N regime where launch overhead, not arithmetic, sets the time).
+ *                             the small-N regime where launch overhead, not arithmetic, sets the time).  An apply on
+ *                             this path takes no host decision and synchronises nothing, so a caller may capture
+ *                             batches of lm_mdot / lm_mdot_batch calls into a CUDA graph of their own and replay them.
  *   LM_OPT_J_SPLITS           0 (default): the launch chooser sizes the grid | s > 0: the general path deals the sources to
  *                             exactly s j-splits (clamped to what the problem allows) -- for plan sweeps; results are
  *                             the same up to summation order.

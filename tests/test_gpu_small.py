@@ -181,3 +181,33 @@ def test_option_values(lm, torch):
     s.set_option(lm.LM_OPT_SMALL_KERNEL, (2 << 8) | 4)
     assert s.pair_launch_config(1)["block"] == 128 and s.pair_launch_config(1)["j_splits"] == 2
     s.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_applies_can_be_captured_in_a_callers_cuda_graph(lm, torch, prec):
+    """The one-launch apply makes no host decisions and synchronises nothing: a caller may capture a whole batch of
+    lm_mdot calls in a CUDA graph of their own (graph kernel nodes are not subject to the 2.048 us stream-launch grid,
+    DESIGN.md sec. 5) and replay it on new data."""
+    pos, F, T = case(900, 13.0, 1, prec, False, 21)
+    N = pos.shape[0]
+    s = lm.Solver(prec, N)
+    s.set_positions(dev(torch, pos))
+    Fd = dev(torch, F[0]).reshape(-1).clone()
+    U1 = torch.empty(3 * N, dtype=s.torch_dtype, device="cuda")
+    U2 = torch.empty_like(U1)
+    s.mdot(Fd, None, U1)                                        # warm-up outside the capture (plans, attributes)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        with torch.cuda.graph(g, stream=st):
+            s.mdot(Fd, None, U1)                                # U1 = M F
+            s.mdot(U1, None, U2)                                # U2 = M M F: the second node depends on the first
+    for scale in (1.0, -2.5):
+        Fd.copy_(dev(torch, F[0]).reshape(-1) * scale)
+        g.replay()
+        torch.cuda.synchronize()
+        Uo, _ = oracle(pos, F[0].astype(np.float64) * scale, None, False)
+        UUo, _ = oracle(pos, Uo, None, False)
+        assert close(U1.cpu().numpy(), Uo, TOL[prec]) and close(U2.cpu().numpy(), UUo, 2 * TOL[prec])
+    s.close()
