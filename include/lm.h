@@ -256,8 +256,8 @@ int lm_mdot_rows(lm_solver* h, int64_t row_begin, int64_t row_count, const void*
  *                             accumulators are flushed every 32 sources into fp64 totals, the j-split partial sums are
  *                             kept and added in fp64, and each result is rounded to fp32 once.  The error of an fp32
  *                             apply is dominated by the length of its fp32 summation runs: measured on config 3
- *                             (N = 131072) rel-L2 6.1e-7 -> 1.4e-7, the floor set by the fp32 pair arithmetic being 0.8e-7,
- *                             for a few per cent of time.  Always the general path (no one-launch kernel).
+ *                             (N = 131072) rel-L2 5.5e-7 -> 1.6e-7, the floor set by the fp32 pair arithmetic being 0.8e-7,
+ *                             for 2.7 % more time.  Always the general path (no one-launch kernel).
  * lm_lanczos_history: what the last Lanczos call measured for noise vector `vec` of its (last) group: for iteration
  *   i + 1 (i < cap): alpha[i], beta[i], step[i] = s_{i+1} (NaN for i = 0), estimate[i] = e_{i+1} (NaN for i < 2; NaN
  *   throughout under LM_RULE_STEP).  Any output may be NULL.  Returns the number of iterations recorded. */
