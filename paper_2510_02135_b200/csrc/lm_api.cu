@@ -80,7 +80,7 @@ int stage_out_alloc(lm_solver* h, int slot, const void* host, size_t bytes, void
 // ================================================================ C ABI
 extern "C" {
 
-const char* lm_version(void) { return "liblm 0.1 (sm_100a)"; }
+const char* lm_version(void) { return "liblm 0.2 (sm_100a)"; }
 
 int lm_create(lm_solver** out, int precision, int64_t N, double eta, double a, int include_angular)
 {
