@@ -100,12 +100,14 @@ int rpy_mdot(int64_t N, double a, double eta, const double *x, const double *F, 
 {
     int nthreads = 1;
 #ifdef _OPENMP
-#pragma omp parallel
+    /* tiny problems run on one thread (the pins call this thousands of times with N ~ 5: thread wake-ups would be the cost) */
+    const int par = (double)N * (double)N >= 65536.0;
+#pragma omp parallel if (par)
     {
 #pragma omp single
         nthreads = omp_get_num_threads();
     }
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if (par)
 #endif
     for (int64_t i = 0; i < N; ++i)
         row_apply(i, N, a, eta, x, F, T, U + 3 * i, W ? W + 3 * i : NULL);
@@ -119,12 +121,13 @@ int rpy_mdot_rows(int64_t N, double a, double eta, const double *x, const double
 {
     int nthreads = 1;
 #ifdef _OPENMP
-#pragma omp parallel
+    const int par = (double)nrows * (double)N >= 65536.0;      /* tiny problems run on one thread */
+#pragma omp parallel if (par)
     {
 #pragma omp single
         nthreads = omp_get_num_threads();
     }
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if (par)
 #endif
     for (int64_t k = 0; k < nrows; ++k)
         row_apply(rows[k], N, a, eta, x, F, T, U + 3 * k, W ? W + 3 * k : NULL);

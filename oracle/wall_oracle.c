@@ -172,12 +172,13 @@ int wall_mdot_rows(int64_t N, double a, double eta, double wall_z, const double 
 {
     int nthreads = 1;
 #ifdef _OPENMP
-#pragma omp parallel
+    const int par = (double)nrows * (double)N >= 65536.0;      /* tiny problems run on one thread */
+#pragma omp parallel if (par)
     {
 #pragma omp single
         nthreads = omp_get_num_threads();
     }
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if (par)
 #endif
     for (int64_t k = 0; k < nrows; ++k)
         wall_row_apply(rows ? rows[k] : k, N, a, eta, wall_z, x, F, T, U + 3 * k, W ? W + 3 * k : NULL);
