@@ -281,9 +281,9 @@ class Arm:
 
     def steady_state(self, reps=200):
         """Small configs only (working set far below the L2): `reps` applies back to back on the stream -- no L2 flush, no
-        set_positions, the loop a time-stepping user runs -- under ONE event pair.  Reported beside the flushed per-step
-        figure, never instead of it: with a 2 us apply the flush (cold DRAM misses behind 256 MiB of dirty lines)
-        and the per-step event pair dominate the contract's number."""
+        set_positions, the loop a time-stepping user runs -- under ONE event pair.  Reported beside the per-step figures,
+        never instead of them: an event pair around ONE launch of a few microseconds mostly measures the stream-launch
+        grid of this B200 (2.048 us per dependent stream operation, the two event records included)."""
         if self.cfg.op != "mdot" or self.N > 20000:
             return None
         torch, s, dev = self.torch, self.solver, self.dev
