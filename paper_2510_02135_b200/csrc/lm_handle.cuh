@@ -394,11 +394,19 @@ template <typename T> SmallPlan choose_small(lm_solver* h, int nrhs)
                 const int spw = (int)(((h->N + (int64_t)S * W - 1) / ((int64_t)S * W) + 3) / 4 * 4);
                 const size_t smem = vs[vi].smem(W, spw);
                 if (smem > SMALL_MAX_SMEM) continue;
-                const double per_sm = std::ceil((double)i_tiles * S / h->sm_count);
-                const double warps_sub = std::ceil(per_sm * W / 4.0);
-                const double loop = spw * std::max(lone, shared * warps_sub);
+                // CTAs that fit on one SM at a time (registers, shared memory, threads): more than that run in waves
+                int occ = 0;
+                if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)vs[vi].kernel, W * 32, smem) != cudaSuccess || occ < 1) {
+                    (void)cudaGetLastError();
+                    continue;
+                }
+                const double ctas = (double)i_tiles * S, slots = (double)h->sm_count * occ;
+                const double full = std::floor(ctas / slots), rem_per_sm = std::ceil((ctas - full * slots) / h->sm_count);
                 const double rounds = std::ceil(3.0 * spw / 64.0);
-                const double cost = loop + 900.0 + 500.0 * rounds + 1300.0 + 20.0 * (S + W);
+                auto wave = [&](double resident) {            // `resident` CTAs share an SM: their warps share its four sub-partitions
+                    return resident > 0 ? spw * std::max(lone, shared * std::ceil(resident * W / 4.0)) + 900.0 + 500.0 * rounds + 1300.0 : 0.0;
+                };
+                const double cost = full * wave(occ) + wave(rem_per_sm) + 20.0 * (S + W);
                 if (cost < best_cost) {
                     best_cost = cost;
                     best.variant = vi;
