@@ -117,7 +117,7 @@ def test_config5_geometry_fixed_k_at_reduced_size(lm, torch):
         s.close()
 
 
-@pytest.mark.parametrize("index,tol,nrows", [(5, 1e-3, 48), (4, 1e-2, 32)])
+@pytest.mark.parametrize("index,tol,nrows", [(5, 1e-3, 48), (4, 1e-3, 32)])
 def test_full_size_square_root_twice_is_m(lm, torch, index, tol, nrows):
     """S(S z) = M z at the full config size; the rows of M z come from the oracle (exact for those rows).  An iterate
     with relative error e gives S(S z) with ~2e, so the gate is 5 tol."""
