@@ -121,7 +121,7 @@ int ensure_capture_stream(lm_solver* h)
 // source splits through the cluster's distributed shared memory, writes the caller's outputs.
 template <typename T>
 int launch_small(lm_solver* h, int nrhs, const SmallPlan& sp, const RhsIn<T>& in, const RhsOut<T>& out, cudaStream_t st, bool timed,
-                 const int* in_index = nullptr, int64_t in_stride = 0, bool count = true)
+                 const int* in_index = nullptr, int64_t in_stride = 0, bool count = true, double* const* gram_out = nullptr, int gram_ld = 0)
 {
     const auto& v = small_variants<T>(h)[sp.variant];
     SmallParams<T> p;
@@ -129,6 +129,9 @@ int launch_small(lm_solver* h, int nrhs, const SmallPlan& sp, const RhsIn<T>& in
     p.in = in;
     p.in_index = in_index;
     p.in_stride = in_stride;
+    for (int q = 0; q < MAX_RHS; ++q) p.gram_out[q] = gram_out && q < nrhs ? gram_out[q] : nullptr;
+    p.gram_n = in_stride;
+    p.gram_ld = gram_ld;
     p.out = out;
     p.N = h->N;
     p.npad = h->npad;

@@ -156,13 +156,13 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
             in.f[q] = Vq(q);
             in.t[q] = h->angular ? Vq(q) + n3 : nullptr;
         }
-        const int rc2 = launch_small<T>(h, nv, sp, in, out, s2, timed, h->d_newest, dof, false);
+        // the apply of V[c] also forms Gram column c (needed by the stopping test of the NEXT iteration): no Gram launch
+        double* gout[MAX_RHS] = {nullptr, nullptr, nullptr, nullptr};
+        for (int q = 0; q < nv; ++q) gout[q] = h->h_gram + (size_t)q * ld * ld;
+        const int rc2 = launch_small<T>(h, nv, sp, in, out, s2, timed, h->d_newest, dof, false, gout, ld);
         if (rc2 != LM_OK) return rc2;
         for (int q = 0; q < nv; ++q)
             lanczos_fused_step_kernel<T><<<1, FUSED_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q), dof, h->h_ab + (size_t)q * 2 * ld, q == nv - 1);
-        for (int q = 0; q < nv; ++q)
-            gram_column_kernel<T><<<dim3(gg, kmax + 1), VEC_BLOCK, 0, s2>>>(Vq(q), dof, h->d_newest, gchunk, h->d_gram_part, h->d_ticket,
-                                                                             h->h_gram + (size_t)q * ld * ld, ld);
         LM_CUDA(h, cudaGetLastError());
         return LM_OK;
     };
@@ -227,7 +227,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
         if (small) {
             h->n_pair++;
             h->pairs += (double)std::max<int64_t>(h->row_end - h->row_begin, 0) * (double)h->N;
-            h->n_aux += 2 * nv;
+            h->n_aux += nv;
         } else {
             if (with_det && plan_det.j_splits > 1 && fused(plan_det)) h->n_aux++;    // the deterministic vector's own reduce
             count_apply(h, with_det ? plan_det : plan);
@@ -244,6 +244,9 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
         if (lookahead && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
         LM_CUDA(h, cudaEventSynchronize(h->lz_ev[k & 1]));
         ++consumed;
+        if (small && k >= 2)                                    // the apply of this iteration wrote the Gram column of the vector it applied
+            for (int q = 0; q < nv; ++q)
+                if (!done[q]) stop[q].set_gram_column(k - 1, hg(q) + (size_t)(k - 1) * ld);
         // this rank's verdicts: bit q = vector q stops at this k (converged, or k == kmax); bit 31 = a failure
         unsigned word = 0u;
         int local_fail = LM_OK;
@@ -279,7 +282,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
                 continue;
             }
             stop[q].advance();
-            stop[q].set_gram_column(k, hg(q) + (size_t)k * ld);
+            if (!small) stop[q].set_gram_column(k, hg(q) + (size_t)k * ld);      // small N: column k is written by the NEXT apply
         }
         if (!lookahead && remaining > 0 && k < kmax && (rc = enqueue(k + 1)) != LM_OK) return rc;
     }

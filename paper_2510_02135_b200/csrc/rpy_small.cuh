@@ -50,6 +50,12 @@ template <typename T> struct SmallParams {
     RhsIn<T> in;                 // caller's arrays, interleaved xyz, 3N each; null = zeros
     const int* in_index;         // null, or: every input array is read at in.f[q] + *in_index * in_stride (the Lanczos driver
     int64_t in_stride;           //   passes its basis and the device-side index of the newest vector: one launch fits every iteration)
+    // Lanczos driver only: while applying M to V[c] (c = *in_index) the kernel also forms column c of the Gram matrix of
+    // the basis, gram_out[q][c gram_ld + j] = V_q[j] . V_q[c], j <= c (one CTA per column) -- the stopping test needs it
+    // one iteration later, so it rides along instead of being a launch of its own.  gram_out[0] == null: no Gram work.
+    double* gram_out[MAX_RHS];
+    int64_t gram_n;              // length of a basis vector (dof)
+    int gram_ld;
     RhsOut<T> out;               // caller's outputs, interleaved xyz
     int64_t N, npad;
     int64_t i_begin, i_end;      // target rows [i_begin, i_end)
@@ -237,6 +243,43 @@ __global__ void __launch_bounds__(SM_MAX_WARPS * 32) rpy_small_kernel(const Smal
         T fac = part ? p.c.C1_ang : p.c.C1_lin;
         if constexpr (WALL) fac *= p.pos[4 * p.npad + i];
         (part ? p.out.ang[q] : p.out.lin[q])[3 * i + k3] = s * fac;
+    }
+
+    // ---- Gram column of the vector being applied (Lanczos driver): CTA b takes the columns j = b, b + #CTAs, ...
+    if (p.gram_out[0]) {
+        __shared__ double gpart[SM_MAX_WARPS];
+        const int c = *p.in_index;
+        const int cta = blockIdx.y * gridDim.x + blockIdx.x, ncta = gridDim.x * gridDim.y;
+#pragma unroll
+        for (int q = 0; q < NRHS; ++q) {
+            const T* Vq = p.in.f[q];                           // basis of vector q: V[j] = Vq + j gram_n  (in_stride == gram_n)
+            const T* vc = Vq + (int64_t)c * p.gram_n;
+            for (int j = cta; j <= c; j += ncta) {
+                const T* vj = Vq + (int64_t)j * p.gram_n;
+                double t = 0.0;
+                for (int64_t i0 = tid; i0 < p.gram_n; i0 += 4 * blockDim.x) {      // 8 independent loads in flight per thread
+                    T a[4], b[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int64_t i = i0 + (int64_t)u * blockDim.x;
+                        a[u] = i < p.gram_n ? vj[i] : T(0);
+                        b[u] = i < p.gram_n ? vc[i] : T(0);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) t = fma((double)a[u], (double)b[u], t);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                __syncthreads();                               // gpart may still be read from the previous column
+                if (lane == 0) gpart[warp] = t;
+                __syncthreads();
+                if (tid == 0) {
+                    double sum = 0.0;
+                    for (int w2 = 0; w2 < W; ++w2) sum += gpart[w2];
+                    p.gram_out[q][(size_t)c * p.gram_ld + j] = sum;
+                }
+            }
+        }
     }
 }
 
