@@ -161,8 +161,15 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
         for (int q = 0; q < nv; ++q) gout[q] = h->h_gram + (size_t)q * ld * ld;
         const int rc2 = launch_small<T>(h, nv, sp, in, out, s2, timed, h->d_newest, dof, false, gout, ld);
         if (rc2 != LM_OK) return rc2;
-        for (int q = 0; q < nv; ++q)
-            lanczos_fused_step_kernel<T><<<1, FUSED_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q), dof, h->h_ab + (size_t)q * 2 * ld, q == nv - 1);
+        const int ept = (int)((dof + FUSED_BLOCK - 1) / FUSED_BLOCK);
+        for (int q = 0; q < nv; ++q) {
+            double* habq = h->h_ab + (size_t)q * 2 * ld;
+            const int adv = q == nv - 1;
+            if (ept <= 4)       lanczos_fused_step_kernel<T, 4><<<1, FUSED_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q), dof, habq, adv);
+            else if (ept <= 8)  lanczos_fused_step_kernel<T, 8><<<1, FUSED_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q), dof, habq, adv);
+            else if (ept <= 16) lanczos_fused_step_kernel<T, 16><<<1, FUSED_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q), dof, habq, adv);
+            else                lanczos_fused_step_kernel<T, 32><<<1, FUSED_BLOCK, 0, s2>>>(wq(q), Vq(q), h->d_newest, scal(q), dof, habq, adv);
+        }
         LM_CUDA(h, cudaGetLastError());
         return LM_OK;
     };

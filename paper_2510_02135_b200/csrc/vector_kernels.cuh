@@ -284,7 +284,7 @@ __global__ void __launch_bounds__(VEC_BLOCK) lanczos_beta_kernel(T* __restrict__
 
 // Small N: the vector part of one Lanczos iteration -- lanczos_alpha_kernel, lanczos_beta_kernel and the scaling of
 // lanczos_scale_pack_kernel -- in ONE launch of one CTA (the vectors are a few thousand elements; three launches and
-// two grid-wide reductions cost more than the arithmetic).  Same operations and rounding points as those kernels:
+// two grid-wide reductions cost more than the arithmetic; the Gram column is formed by the apply, rpy_small.cuh).  Same operations and rounding points as those kernels:
 //   m = *newest;  w -= beta_{k-1} V[m-1] (m > 0);  alpha = w . V[m];  w -= alpha V[m];  beta^2 = |w|^2;  V[m+1] = w / beta;
 //   host_ab[2(m+1)] = alpha, host_ab[2(m+1)+1] = beta^2;  scal[1] = alpha, scal[2] = beta^2;  `advance`: *newest = m + 1.
 // No packed copy of V[m+1] is written: at these sizes the apply (rpy_small_kernel) reads V[*newest] itself.
@@ -301,8 +301,11 @@ __device__ __forceinline__ double cta_sum_1024(double v, double* warp_part)
     for (int w = 0; w < FUSED_BLOCK / 32; ++w) s += warp_part[w];
     return s;
 }
-template <typename T>
-__global__ void __launch_bounds__(FUSED_BLOCK) lanczos_fused_step_kernel(T* __restrict__ w, T* __restrict__ V, int* newest, double* scal, int64_t n,
+// EPT = elements per thread (n <= EPT x 1024): every thread keeps its elements of w and V[m] in REGISTERS from the first load
+// to the last store -- one global-memory round trip instead of three; w itself is not written back (nothing reads it
+// before the next apply overwrites it).
+template <typename T, int EPT>
+__global__ void __launch_bounds__(FUSED_BLOCK) lanczos_fused_step_kernel(const T* __restrict__ w, T* __restrict__ V, int* newest, double* scal, int64_t n,
                                                                          double* host_ab, int advance)
 {
     __shared__ double warp_part[FUSED_BLOCK / 32];
@@ -311,27 +314,36 @@ __global__ void __launch_bounds__(FUSED_BLOCK) lanczos_fused_step_kernel(T* __re
     const T* v_prev = m > 0 ? v - n : nullptr;
     T* v_next = V + (size_t)(m + 1) * n;
     const double bp = v_prev ? sqrt(scal[2]) : 0.0;
+    T wr[EPT], vr[EPT];
     double s = 0.0;
-    for (int64_t i = threadIdx.x; i < n; i += FUSED_BLOCK) {
-        double wi = (double)w[i];
-        if (v_prev) {
-            wi = fma(-bp, (double)v_prev[i], wi);
-            w[i] = (T)wi;
-            wi = (double)w[i];                         // the dot product sees the stored (rounded) value
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int64_t i = (int64_t)e * FUSED_BLOCK + threadIdx.x;
+        wr[e] = T(0);
+        vr[e] = T(0);
+        if (i < n) {
+            vr[e] = v[i];
+            double wi = (double)w[i];
+            if (v_prev) wi = (double)(T)fma(-bp, (double)v_prev[i], wi);     // rounded to T where the general kernel stores it
+            wr[e] = (T)wi;
+            s = fma((double)wr[e], (double)vr[e], s);
         }
-        s = fma(wi, (double)v[i], s);
     }
     const double alpha = cta_sum_1024(s, warp_part);
     s = 0.0;
-    for (int64_t i = threadIdx.x; i < n; i += FUSED_BLOCK) {
-        const T wi = (T)fma(-alpha, (double)v[i], (double)w[i]);
-        w[i] = wi;
-        s = fma((double)wi, (double)wi, s);
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        wr[e] = (T)fma(-alpha, (double)vr[e], (double)wr[e]);                // elements past n stay zero
+        s = fma((double)wr[e], (double)wr[e], s);
     }
     const double beta_sq = cta_sum_1024(s, warp_part);
     const double nrm = sqrt(beta_sq);
     const double inv = nrm > 0.0 ? 1.0 / nrm : 0.0;
-    for (int64_t i = threadIdx.x; i < n; i += FUSED_BLOCK) v_next[i] = (T)((double)w[i] * inv);
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int64_t i = (int64_t)e * FUSED_BLOCK + threadIdx.x;
+        if (i < n) v_next[i] = (T)((double)wr[e] * inv);
+    }
     if (threadIdx.x == 0) {
         host_ab[2 * (m + 1)] = alpha;
         host_ab[2 * (m + 1) + 1] = beta_sq;
