@@ -161,12 +161,13 @@ def test_row_ranges(lm, torch, prec):
     s = lm.Solver(prec, N, 1.0, 1.0, False)
     s.set_positions(dev(torch, pos))
     Uo, _ = oracle(pos, F[0], None, False)
-    for b, n in ((0, 1), (0, 64), (37, 900), (1499, 1), (700, 800)):
+    for b, n in ((0, 1), (0, 64), (37, 900), (1499, 1), (700, 800), (5, 0), (1500, 0)):      # incl. empty row ranges: nothing written
         U = torch.full((3 * N,), 7.0, dtype=s.torch_dtype, device="cuda")
         s.mdot_rows(b, n, dev(torch, F[0]), None, U)
         torch.cuda.synchronize()
         got = U.cpu().numpy().reshape(N, 3)
-        assert close(got[b:b + n], Uo[b:b + n], TOL[prec])
+        if n:
+            assert close(got[b:b + n], Uo[b:b + n], TOL[prec])
         assert np.all(got[:b] == 7.0) and np.all(got[b + n:] == 7.0)
     s.close()
 
