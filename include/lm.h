@@ -290,6 +290,35 @@ int lm_pair_launch_config(lm_solver* h, int nrhs, int* i_tiles, int* j_splits, i
  * LM_OPT_SMALL_KERNEL) or "rpy_pair_kernel" (pack, pair kernel, split-j reduce); "" for an unsupported nrhs. */
 const char* lm_pair_kernel_name(lm_solver* h, int nrhs);
 
+/* ---- M.F without any allocation (csrc/lm_static.cu) ----
+ * For callers that cannot let a library allocate device memory: an engine or framework allocator that claimed the whole
+ * card for its own arena (a later cudaMalloc fails or eats its headroom), a latency-tuned stepping loop (cudaMalloc and
+ * cudaFree synchronise the whole device at a moment the caller does not choose), a process held to a fixed device-memory
+ * budget.  A handle (lm_create) owns cudaMalloc'ed buffers and may grow them on a later call; this call owns none:
+ *   lm_mdot_static : lin_out = M_uF . forces for N equal spheres in free space (the translational block of lm_mdot:
+ *       PAPER.md:173, eq. (8)), precision LM_F32 or LM_F64, on the CURRENT device.  positions, forces,
+ *       lin_out: DEVICE pointers, 3N reals of that precision, interleaved xyz, owned by the caller; inputs are not
+ *       modified; lin_out is overwritten.  Asynchronous on `stream`.  Results equal lm_mdot's up to summation order.
+ *       It calls no cudaMalloc / cudaFree / allocating library routine, on the first call or later.  Its scratch (packed
+ *       positions and forces, j-split partial sums) is a static device array of LM_STATIC_SCRATCH_BYTES inside the
+ *       library image: every GPU the process touches with liblm loaded holds those bytes until exit.
+ *       Limit: 1 <= N <= LM_STATIC_MAX_N, otherwise LM_E_INVALID and nothing is launched.  Other errors: LM_E_INVALID
+ *       (precision, eta, a), LM_E_NULL (a NULL pointer), LM_E_CUDA.  lm_mdot_static_error() gives the message of the
+ *       calling thread's last lm_mdot_static call ("" after success; static thread-local storage).
+ *       Sharing: ONE array per GPU serves every call.  Calls whose kernels may overlap on the GPU (two streams, two
+ *       unordered host threads) race on it; order them on one stream or with events.  The array keeps the previous call's
+ *       contents; a call reads only what it has itself written, so nothing needs clearing between calls.
+ *       First call on each device: one-time set-up with that device current (resolves the array's device address with
+ *       cudaGetSymbolAddress, sets kernel attributes, queries occupancy).  Make that first call before any stream
+ *       capture begins; later calls only launch three kernels (pack, pair kernel, split reduce).
+ *   lm_mdot_static_max_n : LM_STATIC_MAX_N, for callers that bind at run time. */
+#define LM_STATIC_MAX_N 65536
+#define LM_STATIC_SCRATCH_BYTES (16u << 20)
+int lm_mdot_static(int precision, int64_t N, double eta, double a, const void* positions, const void* forces,
+                   void* lin_out, void* stream);
+int64_t lm_mdot_static_max_n(void);
+const char* lm_mdot_static_error(void);
+
 /* Library version string (static storage). */
 const char* lm_version(void);
 

@@ -65,6 +65,9 @@ SIGNATURES = {
     "lm_get_stats": (c_int, [c_void_p, POINTER(c_int64), POINTER(c_int64), POINTER(c_double), POINTER(c_double)]),
     "lm_pair_launch_config": (c_int, [c_void_p, c_int, POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int)]),
     "lm_pair_kernel_name": (c_char_p, [c_void_p, c_int]),
+    "lm_mdot_static": (c_int, [c_int, c_int64, c_double, c_double, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "lm_mdot_static_max_n": (c_int64, []),
+    "lm_mdot_static_error": (c_char_p, []),
     "lm_version": (c_char_p, []),
 }
 
@@ -108,6 +111,28 @@ def lm_dist_unique_id() -> bytes:
     if rc != LM_OK:
         raise LmError(rc, "lm_dist_unique_id: NCCL unavailable")
     return buf.raw
+
+
+def lm_mdot_static_max_n() -> int:
+    return int(lib().lm_mdot_static_max_n())
+
+
+def mdot_static(precision, N: int, eta: float, a: float, positions, forces, lin_out, stream=None) -> None:
+    """lm_mdot_static: lin_out = M_uF . forces (free space, translational) on the current device, WITHOUT any device
+    allocation by the library -- for callers whose memory is spoken for (an engine that owns the whole card, a
+    latency-critical loop that cannot take cudaMalloc's device-wide synchronisation, a fixed memory budget).  The scratch
+    is a static array inside liblm.so (16 MiB per GPU, held until exit), hence the limit N <= lm_mdot_static_max_n().
+    All calls on a GPU share that array: keep them on one stream (or order them), overlapping calls race.
+    Torch CUDA tensors of 3N elements in the precision's dtype; argument marshalling only."""
+    import torch
+    prec = {"f32": LM_F32, "f64": LM_F64}.get(precision, precision)
+    dt = torch.float32 if prec == LM_F32 else torch.float64
+    for name, x in (("positions", positions), ("forces", forces), ("lin_out", lin_out)):
+        if x is None or not x.is_cuda or x.dtype != dt or x.numel() != 3 * int(N) or not x.is_contiguous():
+            raise TypeError(f"{name}: need a contiguous CUDA tensor of {3 * int(N)} elements of dtype {dt}")
+    rc = lib().lm_mdot_static(int(prec), int(N), float(eta), float(a), _ptr(positions), _ptr(forces), _ptr(lin_out), _stream_ptr(stream))
+    if rc != LM_OK:
+        raise LmError(rc, lib().lm_mdot_static_error().decode())
 
 
 def _ptr(x):

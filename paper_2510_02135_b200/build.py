@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblm.so")
-SOURCES = [os.path.join(CSRC, "lm_api.cu")]
+SOURCES = [os.path.join(CSRC, "lm_api.cu"), os.path.join(CSRC, "lm_static.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("rpy_pair.cuh", "rpy_small.cuh", "steric_pair.cuh", "vector_kernels.cuh", "lm_common.cuh", "tridiag_host.h",
                                                     "lanczos_host.h", "lm_handle.cuh", "lm_apply.cuh", "lm_lanczos.cuh", "lm_bd.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "lm.h")]
