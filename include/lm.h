@@ -59,7 +59,8 @@ enum { LM_F32 = 0, LM_F64 = 1 };
 
 enum {
     LM_OK = 0,
-    LM_E_INVALID = -1, /* bad argument: N <= 0, eta <= 0, a <= 0, unknown precision, nrhs < 1, tol <= 0 */
+    LM_E_INVALID = -1, /* bad argument: N <= 0, eta <= 0, a <= 0, unknown precision, nrhs < 1, tol <= 0; non-finite values in the
+                          noise or the positions given to a Lanczos call (seen as a non-finite |z|, alpha_k or beta_k) */
     LM_E_NOPOS = -2,   /* compute call before lm_set_positions */
     LM_E_ANGULAR = -3, /* torques / angular output given but include_angular == 0, or angular output missing */
     LM_E_NULL = -4,    /* a required pointer is NULL */
@@ -114,12 +115,14 @@ int lm_mdot_batch(lm_solver* h, int nrhs, const void* forces, const void* torque
  * tol: relative error requested of the iterate, as estimated by the stopping rule (LM_OPT_LANCZOS_RULE below;
  * DESIGN.md reading S3: the default rule's estimate is within x0.5 ... x2 of the true error).
  * lin_out 3N, ang_out 3N (iff include_angular).  iters_out: HOST int*, may be NULL.
- * LM_E_NOCONV if max_iter is reached (result still written). */
+ * LM_E_NOCONV if max_iter is reached (result still written).  The iteration also ends, with an exact result, on
+ * breakdown beta_k <= eps |alpha_k| (invariant subspace): eps = 1e-6 on fp32 handles (beta_k carries fp32 rounding of
+ * relative size ~1e-7), 1e-14 on fp64 handles.  A non-finite value in the noise or the positions -> LM_E_INVALID. */
 int lm_sqrt_mdot_w(lm_solver* h, const void* noise, double tol, void* lin_out, void* ang_out,
                    int* iters_out, void* stream);
 
 /* nvec independent noise vectors sharing one position set: y_q = M^{1/2} W_q, q < nvec.  The Lanczos
- * recurrences run in lockstep in groups of 4 / 2 / 1 vectors (angular: 2 / 1) so that ONE multi-right-
+ * recurrences run in lockstep in groups of 4 / 2 / 1 vectors (angular or single wall: 2 / 1) so that ONE multi-right-
  * hand-side pair-kernel launch per iteration serves a whole group (the pair geometry is evaluated once
  * per pair, as in lm_mdot_batch); each vector has its own alpha, beta, Gram matrix and stopping test
  * and stops contributing to the result at its own step.  noise: [nvec][dof]; lin_out / ang_out:
@@ -187,7 +190,9 @@ int lm_bd_step_rfd_host(lm_solver* h, void* pos, const void* ext_forces, const v
 /* ---- Thermal drift  d/dX . M  (the paper's divM) ----
  * lm_thermal_drift: the library default for open boundaries -- the divergence of the free-space mobility
  * is identically zero ("the default implementation simply sets the thermal drift to
- * zero"): writes zeros to lin_out (3N) and ang_out (3N, iff include_angular).
+ * zero"): writes zeros to lin_out (3N) and ang_out (3N, iff include_angular).  After lm_set_wall(h, 1, ...) the
+ * divergence is not zero and the call returns LM_E_INVALID, writing nothing: use lm_thermal_drift_rfd
+ * (or lm_bd_step_rfd) there.
  * lm_thermal_drift_rfd: ONE realisation of the random finite difference of eq. (11),
  *   (1/delta) [ M(X + delta W/2) W - M(X - delta W/2) W ],
  * at the positions X of the last lm_set_positions (which stay set), W = noise: 3N values ~ N(0,1)
@@ -241,7 +246,10 @@ int lm_mdot_rows(lm_solver* h, int64_t row_begin, int64_t row_count, const void*
  *                             of csrc/rpy_small.cuh (reads the caller's arrays, sums the source splits through
  *                             distributed shared memory) where the launch chooser prefers it | 0: never (always pack,
  *                             pair kernel, reduce) | (cluster << 8 | warps), cluster and warps in {1, 2, 4, 8}: always,
- *                             with that shape (plan sweeps).  Same results up to summation order (PAPER.md:435-437:
+ *                             with that shape (plan sweeps; a shape whose shared memory does not fit falls back to the
+ *                             general path and a cluster size above what the device can co-schedule is clamped:
+ *                             lm_pair_kernel_name / lm_pair_launch_config report what the next apply will really run --
+ *                             check them after forcing a shape).  Same results up to summation order (PAPER.md:435-437:
  *                             the small-N regime where launch overhead, not arithmetic, sets the time).  An apply on
  *                             this path takes no host decision and synchronises nothing, so a caller may capture
  *                             batches of lm_mdot / lm_mdot_batch calls into a CUDA graph of their own and replay them.

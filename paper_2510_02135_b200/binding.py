@@ -188,8 +188,9 @@ class Solver:
         try:
             import torch
             self._device = torch.cuda.current_device()          # lm_create bound the handle to the current device
+            self._tdtype = torch.float32 if self.precision == LM_F32 else torch.float64
         except Exception:
-            self._device = 0
+            self._device, self._tdtype = 0, None
 
     # -- helpers
     @property
@@ -219,21 +220,24 @@ class Solver:
             raise TypeError("device entry point needs a CUDA tensor (use the *_host call for host arrays)")
 
     def _dev(self, x, n):
-        """Device argument of a hot call: the tensor's address as an int (None -> NULL).  dtype, size, device and
-        contiguity are checked the first time a tensor OBJECT is seen (they cannot change under the same object short
-        of an in-place resize); later calls with the same object only read its address -- a time-stepping loop calls with
-        the same few tensors millions of times and a small apply is otherwise bound by this marshalling."""
+        """Device argument of a hot call: the tensor's address as an int (None -> NULL).  Size, dtype and device are
+        checked on EVERY call (three attribute reads: a tensor can change under the same Python object -- resize_, set_,
+        `.data =` -- and a stale length would be an out-of-bounds device access, not a TypeError); only the contiguity
+        walk is remembered per tensor object and re-done when the object, its size or its storage offset changes.  A
+        time-stepping loop calls with the same few tensors millions of times and a small apply is otherwise bound by this
+        marshalling."""
         if x is None:
             return None
+        if x.numel() != n or x.dtype != self._tdtype or not x.is_cuda:
+            self._expect(x, n, False)          # raises with the precise reason
         seen = self._seen
         ent = seen.get(id(x))
-        if ent is None or ent[0]() is not x or ent[1] != n:
-            self._expect(x, n, False)
+        if ent is None or ent[0]() is not x or ent[1] != x.stride():
             if not x.is_contiguous():
                 raise ValueError("tensor must be contiguous")
             if len(seen) > 256:
                 seen.clear()
-            seen[id(x)] = (weakref.ref(x), n)
+            seen[id(x)] = (weakref.ref(x), x.stride())
         return x.data_ptr()
 
     def _stream(self, stream):

@@ -129,15 +129,20 @@ struct LanczosStopper {
 // Cross-rank agreement on the stopping decision (row-sharded runs).  Every rank evaluates the
 // test on its own copy of the scalars; if the copies ever differed in the last bit (another driver, GPU bin,
 // reduction grid), one rank would enqueue an all-gather the others never post.  So the verdicts of one iteration
-// are packed into a word (bit q = vector q stops now) and rank 0's word is adopted by everybody: `exchange`
-// broadcasts it from rank 0 (ncclBroadcast in the library, a gloo broadcast in the CPU test).  Returns the agreed
-// word; with one rank (exchange == nullptr) it is the local word.
+// are packed into a word (bit q = vector q stops now, bit 31 = this rank hit a failure) and the ranks agree on
+//   * the STOP bits of rank 0 (a broadcast), and
+//   * the OR of everybody's FAILURE bit (a max-reduction): a failure seen on any rank -- not only on rank 0 -- makes all
+//     ranks leave the loop together instead of one returning while the others post the next collective.
+// `exchange(words)` is the transport (ncclBroadcast + ncclAllReduce in the library, gloo in the CPU test):
+//   in:  words[0] = this rank's stop bits, words[1] = this rank's failure flag (0 / 1)
+//   out: words[0] = rank 0's stop bits,    words[1] = max over ranks of the failure flags.
+// Returns the agreed word; with one rank (distributed == false) it is the local word.
 template <typename Exchange> inline unsigned agree_on_stops(unsigned local_word, Exchange&& exchange, bool distributed)
 {
     if (!distributed) return local_word;
-    unsigned word = local_word;
-    exchange(&word);                 // in: this rank's word; out: rank 0's
-    return word;
+    unsigned words[2] = {local_word & 0x7fffffffu, local_word >> 31};
+    exchange(words);
+    return (words[0] & 0x7fffffffu) | (words[1] ? 0x80000000u : 0u);
 }
 
 }  // namespace lm

@@ -173,6 +173,7 @@ int lm_set_wall(lm_solver* h, int enabled, double wall_height)
 int lm_set_option(lm_solver* h, int option, int value)
 {
     if (!h) return LM_E_NULL;
+    h->err.clear();
     switch (option) {
     case LM_OPT_LANCZOS_RULE:
         if (value != LM_RULE_ESTIMATE && value != LM_RULE_STEP) return fail(h, LM_E_INVALID, "LM_OPT_LANCZOS_RULE: LM_RULE_ESTIMATE or LM_RULE_STEP");
@@ -268,10 +269,10 @@ int lm_sqrt_mdot_w_batch(lm_solver* h, int nvec, const void* noise, double tol, 
     const int64_t dof = dof_of(h), n3 = 3 * h->N;
     int worst = LM_OK, max_iters = 0;
     std::string noconv;
-    // groups of 4, 2, 1 vectors (angular: 2, 1): the right-hand-side counts the pair kernel is built for
+    // groups of 4, 2, 1 vectors (angular or single wall: 2, 1): the right-hand-side counts the pair kernel is built for
     for (int q = 0; q < nvec;) {
         int g = nvec - q >= 4 ? 4 : (nvec - q >= 2 ? 2 : 1);
-        if (h->angular && g > 2) g = 2;
+        if ((h->angular || h->wall) && g > 2) g = 2;
         const char* nz = (const char*)noise + (size_t)q * dof * es;
         char* lo = (char*)lin_out + (size_t)q * n3 * es;
         char* ao = ang_out ? (char*)ang_out + (size_t)q * n3 * es : nullptr;
@@ -482,6 +483,9 @@ int lm_thermal_drift(lm_solver* h, void* lin_out, void* ang_out, void* stream)
 {
     int rc = check_io(h, nullptr, nullptr, lin_out, ang_out, false);
     if (rc != LM_OK) return rc;
+    // above a wall the divergence of the mobility is NOT zero: zeros would be silently wrong physics
+    if (h->wall)
+        return fail(h, LM_E_INVALID, "lm_thermal_drift is the zero default of open boundaries; with lm_set_wall use lm_thermal_drift_rfd or lm_bd_step_rfd (eq. 11)");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t bytes = (size_t)3 * h->N * esize(h);
     LM_CUDA(h, cudaMemsetAsync(lin_out, 0, bytes, st));

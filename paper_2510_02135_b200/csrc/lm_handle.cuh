@@ -110,6 +110,7 @@ struct NcclApi {
     int (*CommDestroy)(Comm) = nullptr;
     int (*AllGather)(const void*, void*, size_t, int, Comm, cudaStream_t) = nullptr;
     int (*Broadcast)(const void*, void*, size_t, int, int, Comm, cudaStream_t) = nullptr;
+    int (*AllReduce)(const void*, void*, size_t, int, int, Comm, cudaStream_t) = nullptr;
     int (*GroupStart)() = nullptr;
     int (*GroupEnd)() = nullptr;
     const char* (*GetErrorString)(int) = nullptr;
@@ -117,6 +118,7 @@ struct NcclApi {
     std::string why;
 };
 constexpr int NCCL_INT32 = 2, NCCL_FLOAT32 = 7, NCCL_FLOAT64 = 8;   // ncclDataType_t values (nccl.h)
+constexpr int NCCL_MAX = 2;                                          // ncclRedOp_t value (nccl.h: ncclSum, ncclProd, ncclMax, ...)
 
 inline NcclApi& nccl_api()
 {
@@ -133,10 +135,11 @@ inline NcclApi& nccl_api()
     api.CommDestroy = (int (*)(NcclApi::Comm))sym("ncclCommDestroy");
     api.AllGather = (int (*)(const void*, void*, size_t, int, NcclApi::Comm, cudaStream_t))sym("ncclAllGather");
     api.Broadcast = (int (*)(const void*, void*, size_t, int, int, NcclApi::Comm, cudaStream_t))sym("ncclBroadcast");
+    api.AllReduce = (int (*)(const void*, void*, size_t, int, int, NcclApi::Comm, cudaStream_t))sym("ncclAllReduce");
     api.GroupStart = (int (*)())sym("ncclGroupStart");
     api.GroupEnd = (int (*)())sym("ncclGroupEnd");
     api.GetErrorString = (const char* (*)(int))sym("ncclGetErrorString");
-    api.ok = api.GetUniqueId && api.CommInitRank && api.CommDestroy && api.AllGather && api.Broadcast && api.GroupStart && api.GroupEnd && api.GetErrorString;
+    api.ok = api.GetUniqueId && api.CommInitRank && api.CommDestroy && api.AllGather && api.Broadcast && api.AllReduce && api.GroupStart && api.GroupEnd && api.GetErrorString;
     return api;
 }
 }  // namespace lm

@@ -14,21 +14,28 @@ template <typename T> struct DetShare {
     T* ang = nullptr;          // 3N (angular handles)
 };
 
-// rank 0's word for everybody (row-sharded runs; lanczos_host.h agree_on_stops)
-int broadcast_word(lm_solver* h, unsigned* word, cudaStream_t st)
+// the transport of agree_on_stops (lanczos_host.h) in a row-sharded run: words[0] <- rank 0's stop bits (ncclBroadcast),
+// words[1] <- max over ranks of the failure flags (ncclAllReduce), both in one NCCL group
+int exchange_words(lm_solver* h, unsigned* words, cudaStream_t st)
 {
     if (!h->d_word) {
-        LM_CUDA(h, cudaMalloc((void**)&h->d_word, sizeof(unsigned)));
-        LM_CUDA(h, cudaHostAlloc((void**)&h->h_word, sizeof(unsigned), cudaHostAllocDefault));
+        LM_CUDA(h, cudaMalloc((void**)&h->d_word, 2 * sizeof(unsigned)));
+        LM_CUDA(h, cudaHostAlloc((void**)&h->h_word, 2 * sizeof(unsigned), cudaHostAllocDefault));
     }
     NcclApi& nccl = nccl_api();
-    *h->h_word = *word;
-    LM_CUDA(h, cudaMemcpyAsync(h->d_word, h->h_word, sizeof(unsigned), cudaMemcpyHostToDevice, st));
-    const int nrc = nccl.Broadcast(h->d_word, h->d_word, 1, NCCL_INT32, 0, (NcclApi::Comm)h->nccl_comm, st);
-    if (nrc != 0) return fail(h, LM_E_CUDA, std::string("ncclBroadcast failed: ") + nccl.GetErrorString(nrc));
-    LM_CUDA(h, cudaMemcpyAsync(h->h_word, h->d_word, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+    h->h_word[0] = words[0];
+    h->h_word[1] = words[1];
+    LM_CUDA(h, cudaMemcpyAsync(h->d_word, h->h_word, 2 * sizeof(unsigned), cudaMemcpyHostToDevice, st));
+    int nrc = nccl.GroupStart();
+    if (nrc == 0) nrc = nccl.Broadcast(h->d_word, h->d_word, 1, NCCL_INT32, 0, (NcclApi::Comm)h->nccl_comm, st);
+    if (nrc == 0) nrc = nccl.AllReduce(h->d_word + 1, h->d_word + 1, 1, NCCL_INT32, NCCL_MAX, (NcclApi::Comm)h->nccl_comm, st);
+    const int nrc_end = nccl.GroupEnd();
+    if (nrc == 0) nrc = nrc_end;
+    if (nrc != 0) return fail(h, LM_E_CUDA, std::string("ncclBroadcast / ncclAllReduce of the stopping word failed: ") + nccl.GetErrorString(nrc));
+    LM_CUDA(h, cudaMemcpyAsync(h->h_word, h->d_word, 2 * sizeof(unsigned), cudaMemcpyDeviceToHost, st));
     LM_CUDA(h, cudaStreamSynchronize(st));
-    *word = *h->h_word;
+    words[0] = h->h_word[0];
+    words[1] = h->h_word[1];
     return LM_OK;
 }
 
@@ -128,7 +135,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
     int remaining = nv;
     for (int q = 0; q < nv; ++q) {
         stop[q].set_gram_column(0, hg(q));
-        if (!std::isfinite((double)ab(q)[1])) return fail(h, LM_E_CUDA, "Lanczos: non-finite noise");
+        if (!std::isfinite((double)ab(q)[1])) return fail(h, LM_E_INVALID, "Lanczos: the noise vector holds a non-finite value");
         znorm[q] = std::sqrt(ab(q)[1]);
         if (!(znorm[q] > 0.0)) { done[q] = conv[q] = 1; --remaining; }            // zero noise: M^{1/2} 0 = 0
     }
@@ -261,7 +268,7 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
         for (int q = 0; q < nv; ++q) {
             if (done[q]) continue;
             const double alpha = ab(q)[2 * k], beta = std::sqrt(std::max((double)ab(q)[2 * k + 1], 0.0));
-            if (!std::isfinite(alpha) || !std::isfinite(beta)) { local_fail = LM_E_CUDA; word |= 0x80000000u; break; }
+            if (!std::isfinite(alpha) || !std::isfinite(beta)) { local_fail = LM_E_INVALID; word |= 0x80000000u; break; }
             const LanczosStopper::Verdict v = stop[q].feed(k, alpha, beta);
             if (v == LanczosStopper::EIGENSOLVE_FAILED) { local_fail = LM_E_NOCONV; word |= 0x80000000u; break; }
             verdict[q] = v == LanczosStopper::CONVERGED;
@@ -269,13 +276,13 @@ int lanczos_device(lm_solver* h, int nv, const T* noise, double tol, T* lin_out,
         }
         const unsigned local_word = word;
         int rc_x = LM_OK;
-        word = agree_on_stops(local_word, [&](unsigned* wd) { rc_x = broadcast_word(h, wd, st); }, dist && h->dist_ranks > 1);
+        word = agree_on_stops(local_word, [&](unsigned* wd) { rc_x = exchange_words(h, wd, st); }, dist && h->dist_ranks > 1);
         if (rc_x != LM_OK) return rc_x;
         if ((word | local_word) & 0x80000000u) {
             cudaStreamSynchronize(st);
             if (local_fail == LM_E_NOCONV) return fail(h, LM_E_NOCONV, "Lanczos: tridiagonal eigensolve did not converge");
-            if (local_fail == LM_E_CUDA) return fail(h, LM_E_CUDA, "Lanczos: non-finite alpha/beta (non-finite input?)");
-            return fail(h, LM_E_CUDA, "Lanczos: rank 0 reported a failure");
+            if (local_fail == LM_E_INVALID) return fail(h, LM_E_INVALID, "Lanczos: non-finite alpha/beta -- the positions (or the noise) hold a non-finite value");
+            return fail(h, LM_E_CUDA, "Lanczos: another rank reported a failure (its lm_last_error has the reason); all ranks left the loop together");
         }
         for (int q = 0; q < nv; ++q) {
             if (done[q]) continue;

@@ -37,8 +37,8 @@ int hook_stopper_coefficients(void* p, double* c, int cap)
     return (int)v.size();
 }
 
-// agree_on_stops with the transport supplied by the test (a gloo broadcast from rank 0)
-typedef void (*hook_exchange_fn)(unsigned* word);
+// agree_on_stops with the transport supplied by the test (gloo: broadcast of words[0] from rank 0, max-reduction of words[1])
+typedef void (*hook_exchange_fn)(unsigned* words);
 unsigned hook_agree_on_stops(unsigned local_word, hook_exchange_fn exchange, int distributed)
 {
     return lm::agree_on_stops(local_word, [&](unsigned* w) { exchange(w); }, distributed != 0);

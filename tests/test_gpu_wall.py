@@ -173,6 +173,53 @@ def test_wall_lanczos_and_hydrodynamic_velocities(lm, torch, prec, angular):
     s.close()
 
 
+@pytest.mark.parametrize("prec,angular,nvec", [("f64", False, 4), ("f32", False, 5), ("f64", True, 3)])
+def test_wall_sqrt_mdot_w_batch(lm, torch, prec, angular, nvec):
+    """Several noise vectors above a wall: the wall variants of the pair kernel serve 1 and 2 right-hand sides, so a batch of
+    4 or more must be grouped 2 + 2 (+ 1), not refused; every vector against the exact dense root of the damped wall mobility."""
+    N, tol = 300, 1e-3
+    c = workloads.wall_slab_case(N, 14.0, 0.3, 3.0, 61, prec, angular, with_noise=True, wall_z=0.25)
+    dof = (6 if angular else 3) * N
+    W = np.random.default_rng(200 + nvec).standard_normal((nvec, dof)).astype(workloads.np_dtype(prec))
+    W[0] = c["noise"]
+    s = lm.Solver(prec, N, 1.0, 1.0, angular)
+    s.set_wall(True, c["wall_z"])
+    s.set_positions(dev(torch, c["pos"]))
+    lin = torch.empty(nvec * 3 * N, dtype=s.torch_dtype, device="cuda")
+    ang = torch.empty(nvec * 3 * N, dtype=s.torch_dtype, device="cuda") if angular else None
+    iters = s.sqrt_mdot_w_batch(nvec, dev(torch, W).reshape(-1), tol, lin, ang)
+    torch.cuda.synchronize()
+    lin = lin.cpu().numpy().reshape(nvec, 3 * N)
+    ang = ang.cpu().numpy().reshape(nvec, 3 * N) if angular else None
+    for q in range(nvec):
+        y = lin[q] if not angular else np.concatenate([lin[q], ang[q]])
+        exact = wall.dense_sqrt_mdot_w(c["pos"], W[q], wall_z=c["wall_z"], angular=angular)
+        assert 3 <= iters[q] < 100 and rel(y, exact) <= 3 * tol, (q, iters[q], rel(y, exact))
+    s.close()
+
+
+def test_wall_default_thermal_drift_is_refused(lm, torch):
+    """lm_thermal_drift is the zero default of open boundaries; above a wall the divergence is not zero
+    (PAPER.md:87), so the call must say so instead of returning zeros."""
+    N = 64
+    c = workloads.wall_slab_case(N, 8.0, 0.5, 3.0, 5, "f64", False)
+    s = lm.Solver("f64", N)
+    s.set_wall(True, 0.0)
+    s.set_positions(dev(torch, c["pos"]))
+    lin = torch.full((3 * N,), 5.0, dtype=torch.float64, device="cuda")
+    with pytest.raises(lm.LmError) as e:
+        s.thermal_drift(lin)
+    assert e.value.code == lm.LM_E_INVALID and "lm_thermal_drift_rfd" in str(e.value)
+    torch.cuda.synchronize()
+    assert bool((lin == 5.0).all())
+    s.set_wall(False, 0.0)
+    s.set_positions(dev(torch, c["pos"]))
+    s.thermal_drift(lin)
+    torch.cuda.synchronize()
+    assert float(lin.abs().max()) == 0.0
+    s.close()
+
+
 @pytest.mark.parametrize("prec,angular,delta", [("f64", False, 1e-3), ("f64", True, 1e-3), ("f32", False, 0.05), ("f32", True, 0.05)])
 def test_wall_thermal_drift_rfd(lm, torch, prec, angular, delta):
     """eq. (11) with the wall mobility, same W on both sides; and its non-zero mean for one sphere:

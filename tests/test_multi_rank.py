@@ -136,10 +136,12 @@ def _stop_worker(rank, world, port, out):
     col = lambda m: np.ascontiguousarray([V[j] @ V[m] for j in range(m + 1)])
     L.hook_stopper_gram_column(st, 0, col(0).ctypes.data_as(dp))
 
-    def exchange(word_ptr):
-        t = torch.tensor([int(word_ptr[0])], dtype=torch.int64)
-        dist.broadcast(t, src=0)
-        word_ptr[0] = int(t.item())
+    def exchange(words):                                    # the protocol of lanczos_host.h agree_on_stops
+        t = torch.tensor([int(words[0])], dtype=torch.int64)
+        dist.broadcast(t, src=0)                            # rank 0's stop bits
+        f = torch.tensor([int(words[1])], dtype=torch.int64)
+        dist.all_reduce(f, op=dist.ReduceOp.MAX)            # anybody's failure flag
+        words[0], words[1] = int(t.item()), int(f.item())
 
     cb = hooks.EXCHANGE_FN(exchange)
     beta_prev, k_local, k_agreed = 0.0, None, None
@@ -182,3 +184,55 @@ def test_lanczos_stop_is_rank_zeros_verdict_even_when_the_ranks_scalars_differ()
         assert p.exitcode == 0
     assert res[0][0] == res[0][1] == res[1][1]              # rank 0's verdict is everybody's
     assert res[1][0] != res[0][0]                           # ... and rank 1's own verdict really was another one
+
+
+def _fail_worker(rank, world, port, out):
+    """Iteration 1: nobody stops, nobody fails.  Iteration 2: rank 1 (NOT rank 0) reports a failure (bit 31) while rank 0 wants to
+    go on.  Every rank must come out of agree_on_stops with bit 31 set -- otherwise rank 0 would post the next all-gather
+    and wait for ever for rank 1, which has returned."""
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+    from tests import hooks
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    L = hooks.lib()
+
+    def exchange(words):
+        t = torch.tensor([int(words[0])], dtype=torch.int64)
+        dist.broadcast(t, src=0)
+        f = torch.tensor([int(words[1])], dtype=torch.int64)
+        dist.all_reduce(f, op=dist.ReduceOp.MAX)
+        words[0], words[1] = int(t.item()), int(f.item())
+
+    cb = hooks.EXCHANGE_FN(exchange)
+    seen = []
+    local_words = [[0x0, 0x0], [0x2, 0x80000001]]           # [iteration][rank]: rank 0 stops vector 1 in iteration 2, rank 1 fails
+    for it in range(2):
+        word = L.hook_agree_on_stops(local_words[it][rank], cb, 1)
+        seen.append(int(word))
+        if word & 0x80000000:
+            break
+        dist.all_reduce(torch.zeros(1))                     # the next apply's collective
+    out.put((rank, seen))
+    dist.destroy_process_group()
+
+
+def test_a_failure_on_a_rank_other_than_zero_stops_every_rank():
+    """only rank 0's word used to be broadcast, so a failure seen on another rank made that rank return while the
+    others enqueued the next collective (deadlock).  The failure flag is now max-reduced over the ranks; the stop bits
+    stay rank 0's."""
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = 37500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_fail_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = dict(out.get(timeout=180) for _ in procs)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    # iteration 1: rank 0's stop bits (none) everywhere; iteration 2: rank 0's stop bits (0x2) + the failure flag, on BOTH ranks
+    assert res[0] == res[1] == [0x0, 0x80000002]
+
