@@ -199,7 +199,8 @@ def lanczos_sqrt_mdot_w(pos, noise, tol: float, a: float = 1.0, eta: float = 1.0
                        rule "step" (ref. [35] as SURVEY O4 writes it): k >= 2 and s_k <= tol
                      or beta_k ~ 0 (invariant subspace: y_k is exact).
     ``apply`` overrides the operator (default: the O(N^2) oracle apply).  ``history``, if given, receives
-    "steps" = [s_2..s_k] and "estimates" = [e_3..e_k] (test diagnostics)."""
+    "steps" = [s_2..s_k], "estimates" = [e_3..e_k], "alphas" = [alpha_1..alpha_k] and "betas" = [beta_1..] (the lists the
+    loop below fills anyway: test diagnostics, no arithmetic of their own)."""
     if rule not in ("estimate", "step"):
         raise ValueError("rule must be 'estimate' or 'step'")
     z = np.asarray(noise, dtype=np.float64).reshape(-1)
@@ -214,6 +215,8 @@ def lanczos_sqrt_mdot_w(pos, noise, tol: float, a: float = 1.0, eta: float = 1.0
         return np.zeros_like(z), 0, True
     V = [z / znorm]
     alphas, betas = [], []
+    if history is not None:
+        history["alphas"], history["betas"] = alphas, betas
     y_prev = None
     for k in range(1, max_iter + 1):
         w = apply(V[k - 1])
