@@ -128,8 +128,7 @@ __global__ void __launch_bounds__(STERIC_BLOCK, 2) steric_pair_kernel(const Ster
         }
         __syncwarp();
         if ((tid & 31) == 0 && mbar_arrive_is_last(&empty[stage]) && lt + STAGES < my_tiles) {
-            if (!mbar_test(&empty[stage], (uint32_t)((lt / STAGES) & 1))) __trap();   // completed by this very arrival: acquire (never seen incomplete; a skipped refill would hang the CTA)
-            issue(lt + STAGES);
+            if (mbar_test(&empty[stage], (uint32_t)((lt / STAGES) & 1))) issue(lt + STAGES);   // completed by this arrival: acquire, then refill
         }
     }
 
